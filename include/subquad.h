@@ -1,0 +1,179 @@
+/*
+ * subquad.h -- C ABI of the B200-native SubQuad candidate-pair affinity path
+ * (arxiv/paper_2602_17330).  One shared library, libsubquad.so, hand-written CUDA for
+ * sm_100a.  No torch types, no exceptions, no printing, NO CPU FALLBACK: every entry point
+ * runs CUDA kernels or returns an error code.
+ *
+ * The path (Alg. 1 steps 1-2 and 7-8, L157-158 and L177-178):
+ *     S  --sq_pack-->  packed residues  --sq_minhash-->  signatures
+ *        --sq_lsh_candidates-->  CAND (unique pairs i<j)  --sq_edit_distance-->  d(s_i, s_j)
+ * plus the exhaustive tile path sq_all_pairs (App. F.1, L733-738 Eq. 45).
+ * What each step computes is fixed by SURVEY.md section 8(c) (spec C1-C3), restated in
+ * DESIGN.md; the paper itself gives only the recurrence (Eq. 46) and the sketch sizes.
+ *
+ * Conventions
+ *  - Unless a parameter says "host", every pointer is a DEVICE pointer owned by the caller
+ *    (e.g. a torch tensor).  Inputs are borrowed and never modified.  The library never
+ *    allocates or frees device memory: all scratch, and the packed copy of the sequences,
+ *    live in the workspace the caller hands over with sq_set_workspace, which must outlive
+ *    every later call on the context.
+ *  - All work is enqueued on the CUDA stream given to sq_create.  Calls that return a count
+ *    or an error detected on the device (sq_pack, sq_lsh_candidates, sq_all_pairs, and the
+ *    *_host entry points) synchronise that stream before returning; sq_minhash and
+ *    sq_edit_distance are asynchronous.
+ *  - Pairs are (i, j), i < j, 0-based indices in input order, stored as uint32[n][2].
+ *  - Return value: 0 = SQ_OK, negative = error (see below).  On SQ_ERR_CAPACITY the count
+ *    returned through the host pointer is the REQUIRED count, so the caller can retry.
+ */
+#ifndef SUBQUAD_H_
+#define SUBQUAD_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SQ_OK                 0
+#define SQ_ERR_INVALID_ARG   -1   /* null pointer, k<1, 5k>32, bands*rows>H, cap<1, ...      */
+#define SQ_ERR_BAD_RESIDUE   -2   /* a residue code >= alphabet (detected by sq_pack)        */
+#define SQ_ERR_NOT_PACKED    -3   /* an op that needs the packed sequences ran before sq_pack */
+#define SQ_ERR_CAPACITY      -4   /* output did not fit; required count returned             */
+#define SQ_ERR_WORKSPACE     -5   /* workspace missing or too small                          */
+#define SQ_ERR_UNSUPPORTED   -6   /* sequence longer than SQ_MAX_LEN, H > SQ_MAX_H, ...      */
+#define SQ_ERR_CUDA          -7   /* a CUDA runtime call failed; see sq_last_cuda_error      */
+
+#define SQ_MAX_LEN    240   /* longest sequence the packed layout and the DP kernels accept   */
+#define SQ_MAX_H      256   /* largest signature length ({64,128,256})        */
+#define SQ_MAX_BANDS   64
+
+/* operations, for sq_workspace_bytes */
+#define SQ_OP_PACK            0
+#define SQ_OP_MINHASH         1
+#define SQ_OP_LSH             2
+#define SQ_OP_EDIT_DISTANCE   3
+#define SQ_OP_ALL_PAIRS       4
+#define SQ_OP_PIPELINE_HOST   5
+
+/* flags of sq_lsh_candidates */
+#define SQ_LSH_SORTED     0   /* pairs_out ascending by (i, j) (default)                      */
+#define SQ_LSH_UNORDERED  1   /* same SET of pairs, order unspecified (skips the final sort)  */
+
+typedef struct sq_ctx sq_ctx;   /* opaque; owns only small host metadata + 2 pinned words */
+
+/* Problem sizes for sq_workspace_bytes.  Fields an op does not use may be 0. */
+typedef struct sq_sizes {
+  int64_t n;             /* number of sequences                                              */
+  int64_t total_len;     /* sum of lengths                                                   */
+  int32_t max_len;       /* upper bound on the sequence length (<= SQ_MAX_LEN)               */
+  int32_t H;             /* signature length                                                 */
+  int32_t bands;         /* LSH bands                                                        */
+  int32_t bucket_cap;    /* LSH bucket cap                                                   */
+  int64_t pair_capacity; /* capacity of the pair output (LSH / all-pairs / pipeline)         */
+} sq_sizes;
+
+/* Create / destroy a context bound to `device` and to `cuda_stream` (a cudaStream_t cast to
+ * void*; NULL = the legacy default stream).  Fails with SQ_ERR_CUDA if there is no device. */
+int  sq_create(sq_ctx** out, int device, void* cuda_stream);
+void sq_destroy(sq_ctx* ctx);
+
+/* Bytes of workspace needed so that `op` (and the packed copy made by sq_pack, which every
+ * op needs) fits.  Pure host arithmetic.  Returns 0 for an unknown op. */
+size_t sq_workspace_bytes(const sq_ctx* ctx, int op, const sq_sizes* sizes);
+
+/* Hand over the workspace (device memory, 256-byte aligned).  Invalidates a previous pack. */
+int  sq_set_workspace(sq_ctx* ctx, void* dev_ptr, size_t bytes);
+
+/* a1  Pack (App. F.2 "contiguous memory blocks with proper alignment";
+ * L157 "trim/pad").  seqs = uint8 residue codes, concatenated; offsets = int64[n+1], sequence
+ * i is seqs[offsets[i]..offsets[i+1]).  Validates every code < alphabet (<= 32) and every
+ * length <= max_len (<= SQ_MAX_LEN); writes the internal layout into the workspace: one
+ * fixed-stride slot per sequence, stride = round_up(max_len + 1, 16) bytes, residues at
+ * [0, len), 0xFF padding, the length in the slot's last byte -- so a slot is read with
+ * aligned 16-byte vector loads and a CDR3 (len <= 31) is exactly one 32-byte sector.
+ * Also builds the length-sorted processing order used by sq_minhash.
+ * n = 0 and empty sequences are legal.  Synchronises. */
+int  sq_pack(sq_ctx* ctx, const uint8_t* seqs, const int64_t* offsets, int64_t n,
+             int alphabet, int max_len);
+
+/* a2  MinHash sketch (Alg. 1 step 1; sketch sizes L269; spec C2).
+ * k-mer value x_p = sum_t code[p+t] * 32^(k-1-t) (needs 5k <= 32);
+ * g(x): x^=x>>16; x*=0x6A09E667; x^=x>>15; x*=0xBB67AE85; x^=x>>16   (mod 2^32)
+ * a_j = g(lo ^ g(2j+1)) | 1,  b_j = g(hi ^ g(2j+2))   (lo/hi = 32-bit halves of seed)
+ * sig_out[i][j] = min_p ( a_j * g(x_p) + b_j mod 2^32 );  all 0xFFFFFFFF if len_i < k.
+ * sig_out: uint32[n][H] row-major, H a multiple of 32, 32 <= H <= SQ_MAX_H.  Asynchronous. */
+int  sq_minhash(sq_ctx* ctx, int k, int H, uint64_t seed, uint32_t* sig_out);
+
+/* a3-a5  LSH banding -> capped buckets -> unique candidate pairs (Alg. 1
+ * step 2, L273 "MinHash LSH index"; spec C3).  sig: uint32[n][H] (n = the packed n).
+ * Band b is the tuple sig[i][b*rows .. b*rows+rows); its 64-bit key is
+ *   acc = 0x6A09E667F3BCC908; for v in tuple: acc = (acc ^ v) * 0x9E3779B97F4A7C15;
+ *   acc ^= acc >> 29;
+ * a bucket is the set of sequences with equal (b, key); of each bucket the `bucket_cap`
+ * smallest indices are kept; CAND = all i<j kept together in some bucket, as a set.
+ * Sequences whose signature is all 0xFFFFFFFF take no part.  Needs bands*rows <= H,
+ * 1 <= bands <= SQ_MAX_BANDS, bucket_cap >= 1.
+ * pairs_out: uint32[capacity][2]; *n_pairs (host) = number of unique candidates.
+ * flags: SQ_LSH_SORTED or SQ_LSH_UNORDERED.  Synchronises.  SQ_ERR_CAPACITY if
+ * *n_pairs > capacity (pairs_out then holds nothing useful). */
+int  sq_lsh_candidates(sq_ctx* ctx, const uint32_t* sig, int H, int bands, int rows,
+                       int bucket_cap, int flags, uint32_t* pairs_out, int64_t capacity,
+                       int64_t* n_pairs);
+
+/* a6  Batched exact Levenshtein distance (Eq. 46, unit costs, boundary
+ * D[x][0]=x, D[0][y]=y; spec C1) by Myers/Hyyro bit-parallel DP.
+ * pairs: uint32[n_pairs][2], any order, any i,j < n (i == j allowed, gives 0).
+ * dist_out[p] = min(d, max_d + 1) for max_d >= 0, the exact distance for max_d < 0,
+ * in input order.  Asynchronous. */
+int  sq_edit_distance(sq_ctx* ctx, const uint32_t* pairs, int64_t n_pairs, int max_d,
+                      uint16_t* dist_out);
+
+/* a7  Exhaustive tile path over all i<j (Eq. 45, read as a self-join).
+ * max_d < 0 : dist_out = uint16[n(n-1)/2], condensed row-major (0,1),(0,2)..(n-2,n-1);
+ *             pairs_out ignored (may be NULL); capacity must be >= n(n-1)/2.
+ * max_d >= 0: hits with d <= max_d, ascending by (i,j): pairs_out uint32[capacity][2],
+ *             dist_out uint16[capacity]; *n_out (host) = number of hits.
+ * Synchronises. */
+int  sq_all_pairs(sq_ctx* ctx, int max_d, uint32_t* pairs_out, uint16_t* dist_out,
+                  int64_t capacity, int64_t* n_out);
+
+/* The whole path from HOST buffers (the end-to-end entry point bench.py times as `e2e`):
+ * copies seqs/offsets host->device, runs pack, minhash, lsh (sorted), edit distance, and
+ * copies pairs + distances device->host.  All device buffers come from the workspace
+ * (size it with SQ_OP_PIPELINE_HOST).  Host buffers should be pinned for full copy speed.
+ * pairs_out_host: uint32[capacity][2], dist_out_host: uint16[capacity].  Synchronises. */
+int  sq_pipeline_host(sq_ctx* ctx, const uint8_t* seqs_host, const int64_t* offsets_host,
+                      int64_t n, int alphabet, int max_len, int k, int H, uint64_t seed,
+                      int bands, int rows, int bucket_cap, int max_d,
+                      uint32_t* pairs_out_host, uint16_t* dist_out_host, int64_t capacity,
+                      int64_t* n_pairs);
+
+/* Introspection (host values, valid after the call they describe). */
+int64_t sq_packed_n(const sq_ctx* ctx);          /* n of the current pack, -1 if none        */
+int     sq_packed_stride(const sq_ctx* ctx);     /* slot stride in bytes                     */
+int64_t sq_last_raw_pairs(const sq_ctx* ctx);    /* pairs before cross-band dedupe (last LSH) */
+int64_t sq_kernel_launches(const sq_ctx* ctx);   /* kernels launched by this context so far  */
+const char* sq_last_cuda_error(const sq_ctx* ctx);
+const char* sq_strerror(int code);
+
+/* Built-in per-kernel timer: when enabled, every kernel launch of the context is bracketed by
+ * CUDA events on the context's stream and its duration is accumulated per kernel class
+ * (0 pack, 1 minhash, 2 band_key, 3 sort_hist, 4 scan, 5 sort_scatter, 6 segment, 7 emit,
+ * 8 edit_distance, 9 all_pairs, 10 misc).  sq_profile_read synchronises the pending events and
+ * returns the accumulated milliseconds and launch count of one class (host values). */
+int  sq_profile_enable(sq_ctx* ctx, int on);
+int  sq_profile_reset(sq_ctx* ctx);
+int  sq_profile_read(sq_ctx* ctx, int kernel_class, double* ms, int64_t* launches);
+const char* sq_profile_name(int kernel_class);   /* NULL past the last class */
+
+/* Integer-pipe micro-benchmark (roofline denominator for the DP stage):
+ * runs `iters` dependent-free instructions of `kind` per thread on a full grid and returns
+ * achieved lane-operations per second in *ops_per_s (host).
+ * kind: 0 LOP3, 1 IADD3, 2 SHF, 3 IMAD, 4 min.u32, 5 LOP3+IMAD mix, 6 POPC. */
+int  sq_int_peak(sq_ctx* ctx, int kind, int iters, double* ops_per_s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif  /* SUBQUAD_H_ */

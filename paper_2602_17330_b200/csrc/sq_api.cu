@@ -1,0 +1,205 @@
+// sq_api.cu -- context life cycle, workspace accounting, error strings and the host-buffer
+// pipeline entry point of libsubquad.so (C ABI: include/subquad.h).
+#include "sq_common.cuh"
+#include <new>
+
+extern "C" {
+
+int sq_create(sq_ctx** out, int device, void* cuda_stream) {
+  if (!out) return SQ_ERR_INVALID_ARG;
+  *out = nullptr;
+  int count = 0;
+  if (cudaGetDeviceCount(&count) != cudaSuccess || device < 0 || device >= count) return SQ_ERR_CUDA;
+  if (cudaSetDevice(device) != cudaSuccess) return SQ_ERR_CUDA;
+  sq_ctx* c = new (std::nothrow) sq_ctx();
+  if (!c) return SQ_ERR_INVALID_ARG;
+  c->device = device;
+  c->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+  cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
+  if (cudaHostAlloc(reinterpret_cast<void**>(&c->pinned), 8 * sizeof(unsigned long long),
+                    cudaHostAllocDefault) != cudaSuccess) {
+    delete c;
+    return SQ_ERR_CUDA;
+  }
+  *out = c;
+  return SQ_OK;
+}
+
+void sq_destroy(sq_ctx* c) {
+  if (!c) return;
+  if (c->prof_ev) {
+    for (int i = 0; i < 2 * kSqProfSlots; ++i) cudaEventDestroy(c->prof_ev[i]);
+    delete[] c->prof_ev;
+  }
+  if (c->pinned) cudaFreeHost(c->pinned);
+  delete c;
+}
+
+int sq_set_workspace(sq_ctx* c, void* dev_ptr, size_t bytes) {
+  if (!c || !dev_ptr || (reinterpret_cast<uintptr_t>(dev_ptr) & 255)) return SQ_ERR_INVALID_ARG;
+  if (bytes < 4096) return SQ_ERR_WORKSPACE;
+  c->ws = static_cast<uint8_t*>(dev_ptr);
+  c->ws_bytes = bytes;
+  c->dflags = reinterpret_cast<unsigned long long*>(c->ws);   // first 256 bytes: flag words
+  c->persist = 256;
+  c->scratch_top = c->persist;
+  c->n = -1;
+  c->packed = nullptr;
+  c->order = nullptr;
+  return SQ_OK;
+}
+
+int sq_profile_enable(sq_ctx* c, int on) {
+  if (!c) return SQ_ERR_INVALID_ARG;
+  if (on && !c->prof_ev) {
+    c->prof_ev = new (std::nothrow) cudaEvent_t[2 * kSqProfSlots];
+    if (!c->prof_ev) return SQ_ERR_INVALID_ARG;
+    for (int i = 0; i < 2 * kSqProfSlots; ++i) SQ_CUDA(c, cudaEventCreate(&c->prof_ev[i]));
+  }
+  if (!on && c->prof_on) sq_prof_drain(c);
+  c->prof_on = on != 0;
+  return SQ_OK;
+}
+
+int sq_profile_reset(sq_ctx* c) {
+  if (!c) return SQ_ERR_INVALID_ARG;
+  sq_prof_drain(c);
+  for (int k = 0; k < SQ_K_COUNT; ++k) { c->prof_ms[k] = 0.0; c->prof_launches[k] = 0; }
+  return SQ_OK;
+}
+
+int sq_profile_read(sq_ctx* c, int cls, double* ms, int64_t* launches) {
+  if (!c || cls < 0 || cls >= SQ_K_COUNT || !ms || !launches) return SQ_ERR_INVALID_ARG;
+  sq_prof_drain(c);
+  *ms = c->prof_ms[cls];
+  *launches = c->prof_launches[cls];
+  return SQ_OK;
+}
+
+const char* sq_profile_name(int cls) {
+  static const char* names[SQ_K_COUNT] = {"pack", "minhash", "band_key", "sort_hist", "scan",
+                                          "sort_scatter", "segment", "emit", "edit_distance",
+                                          "all_pairs", "misc"};
+  return (cls >= 0 && cls < SQ_K_COUNT) ? names[cls] : nullptr;
+}
+
+int64_t sq_packed_n(const sq_ctx* c) { return c ? c->n : -1; }
+int sq_packed_stride(const sq_ctx* c) { return c ? c->stride : 0; }
+int64_t sq_last_raw_pairs(const sq_ctx* c) { return c ? c->last_raw_pairs : 0; }
+int64_t sq_kernel_launches(const sq_ctx* c) { return c ? c->launches : 0; }
+const char* sq_last_cuda_error(const sq_ctx* c) {
+  return c ? cudaGetErrorString(c->last_err) : "no context";
+}
+
+const char* sq_strerror(int code) {
+  switch (code) {
+    case SQ_OK: return "ok";
+    case SQ_ERR_INVALID_ARG: return "invalid argument";
+    case SQ_ERR_BAD_RESIDUE: return "residue code >= alphabet, or sequence longer than max_len";
+    case SQ_ERR_NOT_PACKED: return "sq_pack has not been called on this workspace";
+    case SQ_ERR_CAPACITY: return "output capacity too small (required count returned)";
+    case SQ_ERR_WORKSPACE: return "workspace missing or too small";
+    case SQ_ERR_UNSUPPORTED: return "unsupported size (sequence length, H or bands over the compiled maximum)";
+    case SQ_ERR_CUDA: return "CUDA runtime error";
+    default: return "unknown error";
+  }
+}
+
+size_t sq_workspace_bytes(const sq_ctx*, int op, const sq_sizes* s) {
+  if (!s || s->n < 0) return 0;
+  size_t persist = 256 + sq_persist_bytes(s->n, s->max_len);
+  size_t slack = 1 << 16;
+  switch (op) {
+    case SQ_OP_PACK:
+    case SQ_OP_MINHASH:
+    case SQ_OP_EDIT_DISTANCE:
+      return persist + slack;
+    case SQ_OP_LSH:
+      return persist + sq_lsh_scratch_bytes(s->n, s->bands, s->pair_capacity) + slack;
+    case SQ_OP_ALL_PAIRS:
+      return persist + sq_allpairs_scratch_bytes(s->n, s->pair_capacity) + slack;
+    case SQ_OP_PIPELINE_HOST: {
+      size_t io = sq_align_up((size_t)s->total_len + 16) + sq_align_up((size_t)(s->n + 1) * 8 + 16) +
+                  sq_align_up((size_t)s->n * s->H * 4 + 16) +
+                  sq_align_up((size_t)s->pair_capacity * 8 + 16) +
+                  sq_align_up((size_t)s->pair_capacity * 2 + 16);
+      return persist + io + sq_lsh_scratch_bytes(s->n, s->bands, s->pair_capacity) + slack;
+    }
+    default: return 0;
+  }
+}
+
+int sq_minhash(sq_ctx* c, int k, int H, uint64_t seed, uint32_t* sig_out) {
+  if (!c) return SQ_ERR_INVALID_ARG;
+  return sq_minhash_impl(c, k, H, seed, sig_out);
+}
+
+int sq_edit_distance(sq_ctx* c, const uint32_t* pairs, int64_t n_pairs, int max_d,
+                     uint16_t* dist_out) {
+  if (!c) return SQ_ERR_INVALID_ARG;
+  return sq_edit_distance_impl(c, pairs, n_pairs, max_d, dist_out);
+}
+
+int sq_pipeline_host(sq_ctx* c, const uint8_t* seqs_host, const int64_t* offsets_host, int64_t n,
+                     int alphabet, int max_len, int k, int H, uint64_t seed, int bands, int rows,
+                     int bucket_cap, int max_d, uint32_t* pairs_out_host, uint16_t* dist_out_host,
+                     int64_t capacity, int64_t* n_pairs) {
+  if (!c || !offsets_host || !n_pairs || n < 0 || capacity < 0) return SQ_ERR_INVALID_ARG;
+  if (!c->ws) return SQ_ERR_WORKSPACE;
+  if (max_len < 0 || max_len > SQ_MAX_LEN) return SQ_ERR_UNSUPPORTED;
+  *n_pairs = 0;
+  int64_t total = offsets_host[n];
+  // Device I/O buffers sit at the END of the workspace so that sq_pack's persistent region
+  // and the per-op scratch (both allocated from the front) cannot overlap them.
+  size_t io = sq_align_up((size_t)total + 16) + sq_align_up((size_t)(n + 1) * 8 + 16) +
+              sq_align_up((size_t)n * H * 4 + 16) + sq_align_up((size_t)capacity * 8 + 16) +
+              sq_align_up((size_t)capacity * 2 + 16);
+  if (io + 4096 > c->ws_bytes) return SQ_ERR_WORKSPACE;
+  size_t full = c->ws_bytes;
+  uint8_t* p = c->ws + (full - io) / 256 * 256;
+  uint8_t* d_seqs = p;            p += sq_align_up((size_t)total + 16);
+  int64_t* d_off = (int64_t*)p;   p += sq_align_up((size_t)(n + 1) * 8 + 16);
+  uint32_t* d_sig = (uint32_t*)p; p += sq_align_up((size_t)n * H * 4 + 16);
+  uint32_t* d_pairs = (uint32_t*)p; p += sq_align_up((size_t)capacity * 8 + 16);
+  uint16_t* d_dist = (uint16_t*)p;
+  // shrink the arena seen by the ops to the part in front of the I/O buffers
+  size_t saved = c->ws_bytes;
+  c->ws_bytes = (size_t)((c->ws + (full - io) / 256 * 256) - c->ws);
+  int rc = SQ_OK;
+  do {
+    if (total > 0 && cudaMemcpyAsync(d_seqs, seqs_host, (size_t)total, cudaMemcpyHostToDevice,
+                                     c->stream) != cudaSuccess) { rc = SQ_ERR_CUDA; break; }
+    if (cudaMemcpyAsync(d_off, offsets_host, (size_t)(n + 1) * 8, cudaMemcpyHostToDevice,
+                        c->stream) != cudaSuccess) { rc = SQ_ERR_CUDA; break; }
+    if ((rc = sq_pack(c, d_seqs, d_off, n, alphabet, max_len)) != SQ_OK) break;
+    if ((rc = sq_minhash(c, k, H, seed, d_sig)) != SQ_OK) break;
+    if ((rc = sq_lsh_candidates(c, d_sig, H, bands, rows, bucket_cap, SQ_LSH_SORTED, d_pairs,
+                                capacity, n_pairs)) != SQ_OK) break;
+    if ((rc = sq_edit_distance(c, d_pairs, *n_pairs, max_d, d_dist)) != SQ_OK) break;
+    if (*n_pairs > 0) {
+      if (cudaMemcpyAsync(pairs_out_host, d_pairs, (size_t)*n_pairs * 8, cudaMemcpyDeviceToHost,
+                          c->stream) != cudaSuccess) { rc = SQ_ERR_CUDA; break; }
+      if (cudaMemcpyAsync(dist_out_host, d_dist, (size_t)*n_pairs * 2, cudaMemcpyDeviceToHost,
+                          c->stream) != cudaSuccess) { rc = SQ_ERR_CUDA; break; }
+    }
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) { rc = SQ_ERR_CUDA; break; }
+  } while (0);
+  if (rc == SQ_ERR_CUDA) c->last_err = cudaGetLastError();
+  c->ws_bytes = saved;
+  return rc;
+}
+
+}  // extern "C"
+
+void sq_prof_drain(sq_ctx* c) {
+  if (!c->prof_ev || c->prof_n == 0) return;
+  cudaEventSynchronize(c->prof_ev[2 * (c->prof_n - 1) + 1]);
+  for (int i = 0; i < c->prof_n; ++i) {
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, c->prof_ev[2 * i], c->prof_ev[2 * i + 1]) == cudaSuccess) {
+      c->prof_ms[c->prof_cls[i]] += ms;
+      c->prof_launches[c->prof_cls[i]] += 1;
+    }
+  }
+  c->prof_n = 0;
+}

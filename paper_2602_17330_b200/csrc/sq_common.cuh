@@ -1,0 +1,120 @@
+// sq_common.cuh -- context, workspace arena and small helpers shared by the kernels of
+// libsubquad.so (C ABI in include/subquad.h).  sm_100a only.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+#include "../../include/subquad.h"
+
+#define SQ_EMPTY_SIG 0xFFFFFFFFu
+#define SQ_PAD_BYTE  0xFFu
+
+// kernel classes of the built-in per-kernel timer (sq_profile_*)
+enum {
+  SQ_K_PACK = 0, SQ_K_MINHASH, SQ_K_BANDKEY, SQ_K_SORT_HIST, SQ_K_SCAN, SQ_K_SORT_SCATTER,
+  SQ_K_SEGMENT, SQ_K_EMIT, SQ_K_EDIT, SQ_K_ALLPAIRS, SQ_K_MISC, SQ_K_COUNT
+};
+constexpr int kSqProfSlots = 1024;
+
+struct sq_ctx {
+  int device = 0;
+  cudaStream_t stream = nullptr;
+  int sm_count = 148;
+  // workspace arena: [0, persist) holds the packed copy, [persist, ws_bytes) is per-call scratch
+  uint8_t* ws = nullptr;
+  size_t ws_bytes = 0;
+  size_t persist = 0;
+  size_t scratch_top = 0;
+  // state of the current pack
+  int64_t n = -1;
+  int stride = 0;
+  int max_len = 0;
+  int alphabet = 0;
+  uint8_t* packed = nullptr;    // [n][stride]
+  uint32_t* order = nullptr;    // [n] sequence ids, longest first (processing order of the sketch)
+  // bookkeeping
+  int64_t launches = 0;
+  int64_t last_raw_pairs = 0;
+  cudaError_t last_err = cudaSuccess;
+  unsigned long long* pinned = nullptr;   // 8 pinned host words for count / flag read-back
+  unsigned long long* dflags = nullptr;   // 8 device words (lives at the start of the workspace)
+  // per-kernel-class CUDA-event timer (off by default)
+  bool prof_on = false;
+  cudaEvent_t* prof_ev = nullptr;         // 2 * kSqProfSlots events, created on first enable
+  int prof_cls[kSqProfSlots];
+  int prof_n = 0;
+  double prof_ms[SQ_K_COUNT] = {0};
+  int64_t prof_launches[SQ_K_COUNT] = {0};
+};
+
+void sq_prof_drain(sq_ctx* c);           // synchronises the pending events into prof_ms
+
+// RAII: times everything enqueued on the context's stream during its lifetime as one launch
+struct SqProfScope {
+  sq_ctx* c; int slot;
+  SqProfScope(sq_ctx* ctx, int cls) : c(ctx), slot(-1) {
+    if (!c->prof_on) return;
+    if (c->prof_n == kSqProfSlots) sq_prof_drain(c);
+    slot = c->prof_n++;
+    c->prof_cls[slot] = cls;
+    cudaEventRecord(c->prof_ev[2 * slot], c->stream);
+  }
+  ~SqProfScope() { if (slot >= 0) cudaEventRecord(c->prof_ev[2 * slot + 1], c->stream); }
+};
+
+static inline size_t sq_align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+// bump allocation out of the scratch part of the workspace; nullptr when it does not fit
+template <typename T>
+static inline T* sq_scratch(sq_ctx* c, size_t count) {
+  size_t bytes = sq_align_up(count * sizeof(T) + 16);
+  if (c->scratch_top + bytes > c->ws_bytes) return nullptr;
+  T* p = reinterpret_cast<T*>(c->ws + c->scratch_top);
+  c->scratch_top += bytes;
+  return p;
+}
+static inline void sq_scratch_reset(sq_ctx* c) { c->scratch_top = c->persist; }
+
+#define SQ_CUDA(ctx, call)                                   \
+  do {                                                       \
+    cudaError_t e__ = (call);                                \
+    if (e__ != cudaSuccess) { (ctx)->last_err = e__; return SQ_ERR_CUDA; } \
+  } while (0)
+
+// SQ_TIMED(ctx, class, launch-statement): the launch, bracketed by the optional event timer
+#define SQ_TIMED(ctx, cls, ...) do { SqProfScope ps__((ctx), (cls)); __VA_ARGS__; } while (0)
+
+#define SQ_LAUNCH_CHECK(ctx)                                 \
+  do {                                                       \
+    (ctx)->launches++;                                       \
+    cudaError_t e__ = cudaGetLastError();                    \
+    if (e__ != cudaSuccess) { (ctx)->last_err = e__; return SQ_ERR_CUDA; } \
+  } while (0)
+
+static inline int sq_stride_for(int max_len) { return ((max_len + 1) + 15) / 16 * 16; }
+
+// ---- sizes of the per-op scratch (shared by sq_workspace_bytes and the ops themselves) ----
+size_t sq_persist_bytes(int64_t n, int max_len);
+size_t sq_lsh_scratch_bytes(int64_t n, int bands, int64_t pair_capacity);
+size_t sq_allpairs_scratch_bytes(int64_t n, int64_t pair_capacity);
+size_t sq_sort_scratch_bytes(int64_t n_per_batch, int nbatch);
+
+// ---- radix sort (sq_sort.cu) ----
+// Stable LSD radix sort of `nbatch` independent arrays of `n` records each (batch b occupies
+// [b*n, (b+1)*n)).  Keys are uint64; vals (uint32) may be nullptr for a keys-only sort.
+// `shifts[p]`/`widths[p]` give the digit of pass p (width <= 8).  Ping-pongs between the in
+// and alt buffers; returns (through *result_in_alt) where the result ended up.
+// `tmp` must hold sq_sort_scratch_bytes(n, nbatch) bytes.
+int sq_radix_sort(sq_ctx* c, uint64_t* keys_in, uint64_t* keys_alt, uint32_t* vals_in,
+                  uint32_t* vals_alt, int64_t n, int nbatch, const int* shifts, const int* widths,
+                  int npasses, void* tmp, int* result_in_alt);
+
+// exclusive prefix sum of uint32 -> uint64 totals are not needed: callers guarantee < 2^32.
+// In-place capable (out may equal in).  `tmp` needs (n/2048 + 2) * 4 bytes.
+int sq_exclusive_scan_u32(sq_ctx* c, const uint32_t* in, uint32_t* out, int64_t n, uint32_t* tmp,
+                          uint32_t* total_out_dev /* may be nullptr */);
+
+// ---- ops implemented in their own translation units ----
+int sq_minhash_impl(sq_ctx* c, int k, int H, uint64_t seed, uint32_t* sig_out);
+int sq_edit_distance_impl(sq_ctx* c, const uint32_t* pairs, int64_t n_pairs, int max_d,
+                          uint16_t* dist_out);

@@ -1,0 +1,266 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element.
+
+All work is integer: the bar is bit-exact signatures, identical candidate-pair sets (and
+order, which the ABI fixes to ascending (i, j)) and identical distances.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2602_17330_b200 import datagen as dg
+
+pytestmark = pytest.mark.gpu
+SEED = dg.DEFAULT_SEED64
+
+
+def _ctx():
+    from paper_2602_17330_b200 import binding
+    return binding, binding.SubQuad(0)
+
+
+def _pack(sq, binding, rep, bands=0, cap=0, pair_capacity=0, max_len=None, op=None, H=0):
+    max_len = int(rep.lengths.max()) if max_len is None and rep.n else (max_len or 0)
+    op = binding.OP_LSH if op is None else op
+    ws = sq.workspace_bytes(op, rep.n, int(rep.offsets[-1]), max_len, H, max(bands, 1), cap,
+                            pair_capacity)
+    sq.set_workspace(ws)
+    seqs = torch.from_numpy(rep.seqs if rep.seqs.size else np.zeros(1, np.uint8)).cuda()
+    offs = torch.from_numpy(rep.offsets).cuda()
+    sq.pack(seqs, offs, alphabet=20, max_len=max_len)
+    return seqs, offs
+
+
+def _u32(t):
+    return t.cpu().numpy().view(np.uint32)
+
+
+def _u16(t):
+    return t.cpu().numpy().view(np.uint16)
+
+
+# ---------------------------------------------------------------------------------------------
+# config 1: exhaustive all pairs + MinHash k=3 H=32
+# ---------------------------------------------------------------------------------------------
+def test_config1_minhash_and_all_pairs():
+    binding, sq = _ctx()
+    rep = dg.config1()
+    n = rep.n
+    npairs = n * (n - 1) // 2
+    _pack(sq, binding, rep, op=binding.OP_ALL_PAIRS, pair_capacity=npairs)
+    sig = sq.minhash(3, 32, SEED)
+    want = oracle.minhash(rep.seqs, rep.offsets, 3, 32, SEED)
+    assert np.array_equal(_u32(sig), want)
+    dist = torch.empty(npairs, dtype=torch.int16, device="cuda")
+    cnt = sq.all_pairs(-1, None, dist)
+    assert cnt == npairs
+    full = oracle.all_pairs_full(rep.seqs, rep.offsets)
+    assert np.array_equal(_u16(dist), full)
+    # thresholded tile path == filter of the full matrix (config-1 size)
+    for md in (4, 7):
+        sel = np.nonzero(full <= md)[0]
+        pairs = torch.empty((sel.size + 16, 2), dtype=torch.int32, device="cuda")
+        d2 = torch.empty(sel.size + 16, dtype=torch.int16, device="cuda")
+        cnt = sq.all_pairs(md, pairs, d2)
+        assert cnt == sel.size
+        ii, jj = np.triu_indices(n, 1)
+        got = _u32(pairs)[:cnt]
+        assert np.array_equal(got[:, 0], ii[sel]) and np.array_equal(got[:, 1], jj[sel])
+        assert np.array_equal(_u16(d2)[:cnt], full[sel])
+    # explicit pair list == all-pairs
+    ii, jj = np.triu_indices(n, 1)
+    take = np.random.default_rng(0).choice(npairs, 200000, replace=False)
+    pl = np.stack([ii[take], jj[take]], 1).astype(np.uint32)
+    d = sq.edit_distance(torch.from_numpy(pl.view(np.int32)).cuda(), pl.shape[0], -1)
+    assert np.array_equal(_u16(d)[:pl.shape[0]], full[take])
+    sq.close()
+
+
+@pytest.mark.parametrize("k,H", [(3, 32), (3, 64), (4, 128), (5, 256), (6, 96), (1, 32)])
+def test_minhash_shapes(k, H):
+    binding, sq = _ctx()
+    rep = dg.config3(20011, seed=3)          # ragged tail: not a multiple of the block size
+    _pack(sq, binding, rep, op=binding.OP_MINHASH)
+    sig = sq.minhash(k, H, SEED ^ 0xABCDEF)
+    want = oracle.minhash(rep.seqs, rep.offsets, k, H, SEED ^ 0xABCDEF)
+    assert np.array_equal(_u32(sig), want)
+    sq.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# configs 2-4 shapes: minhash -> lsh -> edit distance
+# ---------------------------------------------------------------------------------------------
+def _run_path(rep, P, capacity, flags=0):
+    binding, sq = _ctx()
+    _pack(sq, binding, rep, bands=P["bands"], cap=P["cap"], pair_capacity=capacity, H=P["H"])
+    sig = sq.minhash(P["k"], P["H"], SEED)
+    pairs = torch.empty((capacity, 2), dtype=torch.int32, device="cuda")
+    cnt = sq.lsh_candidates(sig, P["bands"], P["rows"], P["cap"], pairs, flags=flags)
+    dist = sq.edit_distance(pairs, cnt, P["max_d"])
+    torch.cuda.synchronize()
+    out = (_u32(sig), _u32(pairs)[:cnt].copy(), _u16(dist)[:cnt].copy(), sq.last_raw_pairs())
+    sq.close()
+    return out
+
+
+@pytest.mark.parametrize("cfg,n,cap_override", [
+    ("config2", 100_000, None),      # full config 2
+    ("config2", 30_011, 7),          # cap binds
+    ("config3", 60_007, None),
+    ("config4", 50_003, None),
+    ("config4", 50_003, 5),
+])
+def test_path_against_oracle(cfg, n, cap_override):
+    P = dict(dg.PARAMS[cfg])
+    if cap_override:
+        P["cap"] = cap_override
+    rep = dg.GENERATORS[cfg](n, seed=1)
+    want_sig = oracle.minhash(rep.seqs, rep.offsets, P["k"], P["H"], SEED)
+    want_pairs, want_raw, mism = oracle.lsh_sorted(want_sig, P["bands"], P["rows"], P["cap"])
+    assert mism == 0
+    sig, pairs, dist, raw = _run_path(rep, P, want_pairs.shape[0] + 1000)
+    assert np.array_equal(sig, want_sig)
+    assert pairs.shape == want_pairs.shape
+    assert np.array_equal(pairs, want_pairs)          # same set AND ascending (i, j) order
+    assert raw == want_raw
+    want_d = oracle.edit_distance_pairs(rep.seqs, rep.offsets, want_pairs, P["max_d"])
+    assert np.array_equal(dist, want_d)
+
+
+def test_lsh_unordered_is_the_same_set_and_capacity_protocol():
+    P = dict(dg.PARAMS["config2"])
+    rep = dg.config2(20_000, seed=5)
+    want_sig = oracle.minhash(rep.seqs, rep.offsets, P["k"], P["H"], SEED)
+    want_pairs, _, _ = oracle.lsh_sorted(want_sig, P["bands"], P["rows"], P["cap"])
+    from paper_2602_17330_b200 import binding
+    _, pairs, _, _ = _run_path(rep, P, want_pairs.shape[0] + 10, flags=binding.LSH_UNORDERED)
+    key = np.sort(pairs[:, 0].astype(np.int64) << 32 | pairs[:, 1])
+    wkey = want_pairs[:, 0].astype(np.int64) << 32 | want_pairs[:, 1]
+    assert np.array_equal(key, wkey)
+    # too small an output: SQ_ERR_CAPACITY and the required count comes back
+    with pytest.raises(binding.SubQuadError) as ei:
+        _run_path(rep, P, want_pairs.shape[0] // 2)
+    assert ei.value.code == binding.SQ_ERR_CAPACITY
+    assert ei.value.required == want_pairs.shape[0]
+
+
+def test_determinism_two_runs_identical():
+    # "fixed seeds and deterministic kernels"
+    P = dict(dg.PARAMS["config2"])
+    rep = dg.config2(40_000, seed=9)
+    a = _run_path(rep, P, 3_000_000)
+    b = _run_path(rep, P, 3_000_000)
+    for x, y in zip(a[:3], b[:3]):
+        assert np.array_equal(x, y)
+
+
+# ---------------------------------------------------------------------------------------------
+# edge cases
+# ---------------------------------------------------------------------------------------------
+def test_edit_distance_textbook_and_edge_cases():
+    binding, sq = _ctx()
+    enc = lambda s: [ord(c) - ord("a") for c in s]      # 26 letters < 32-symbol alphabet
+    words = ["kitten", "sitting", "", "a", "saturday", "sunday", "flaw", "lawn", "abc", "abc",
+             "intention", "execution", "a" * 31, "b" * 31, "ab" * 15, "ba" * 15]
+    rep = dg.from_list([enc(w) for w in words])
+    ws = sq.workspace_bytes(binding.OP_ALL_PAIRS, rep.n, int(rep.offsets[-1]), 31, 0, 1, 0, 1000)
+    sq.set_workspace(ws)
+    sq.pack(torch.from_numpy(rep.seqs).cuda(), torch.from_numpy(rep.offsets).cuda(),
+            alphabet=26, max_len=31)
+    n = rep.n
+    ii, jj = np.triu_indices(n, 1)
+    pl = np.stack([ii, jj], 1).astype(np.uint32)
+    pl = np.concatenate([pl, np.stack([np.arange(n), np.arange(n)], 1).astype(np.uint32)])  # i == j
+    want = oracle.edit_distance_pairs(rep.seqs, rep.offsets, pl, -1)
+    assert want[0] == 3                                   # kitten / sitting
+    for md in (-1, 0, 2, 5):
+        d = sq.edit_distance(torch.from_numpy(pl.view(np.int32)).cuda(), pl.shape[0], md)
+        w = want if md < 0 else np.minimum(want, md + 1)
+        assert np.array_equal(_u16(d)[:pl.shape[0]], w)
+    full = torch.empty(n * (n - 1) // 2, dtype=torch.int16, device="cuda")
+    sq.all_pairs(-1, None, full)
+    assert np.array_equal(_u16(full), oracle.all_pairs_full(rep.seqs, rep.offsets))
+    sq.close()
+
+
+def test_empty_inputs_and_short_sequences():
+    binding, sq = _ctx()
+    # n = 0
+    rep0 = dg.from_list([])
+    sq.set_workspace(1 << 20)
+    sq.pack(torch.zeros(1, dtype=torch.uint8, device="cuda"),
+            torch.zeros(1, dtype=torch.int64, device="cuda"), alphabet=20, max_len=0)
+    assert sq.minhash(3, 32, SEED).shape[0] == 0
+    pairs = torch.empty((4, 2), dtype=torch.int32, device="cuda")
+    assert sq.lsh_candidates(torch.empty((0, 32), dtype=torch.int32, device="cuda"), 8, 4, 10, pairs) == 0
+    assert rep0.n == 0
+    # sequences shorter than k get the sentinel and take no part in LSH
+    seqs = [[1, 2]] * 5 + [[], [3]] + [[1, 2, 3, 4, 5]] * 3 + [[7, 8, 9, 10, 11, 12]]
+    rep = dg.from_list(seqs)
+    _pack(sq, binding, rep, bands=4, cap=100, pair_capacity=100, H=32)
+    sig = sq.minhash(3, 32, SEED)
+    want = oracle.minhash(rep.seqs, rep.offsets, 3, 32, SEED)
+    assert np.array_equal(_u32(sig), want)
+    assert (want[:7] == 0xFFFFFFFF).all()
+    pairs = torch.empty((100, 2), dtype=torch.int32, device="cuda")
+    cnt = sq.lsh_candidates(sig, 8, 4, 100, pairs)
+    wp, _, _ = oracle.lsh_sorted(want, 8, 4, 100)
+    assert cnt == wp.shape[0] == 3
+    assert np.array_equal(_u32(pairs)[:cnt], wp)
+    sq.close()
+
+
+def test_closed_form_identical_sequences_and_caps():
+    binding, sq = _ctx()
+    s = [3, 7, 1, 19, 4, 4, 9, 12]
+    rep = dg.from_list([s] * 700)
+    _pack(sq, binding, rep, bands=16, cap=1024, pair_capacity=300_000, H=64)
+    sig = sq.minhash(3, 64, SEED)
+    pairs = torch.empty((300_000, 2), dtype=torch.int32, device="cuda")
+    for cap in (1024, 700, 512, 33, 2, 1):
+        m = min(700, cap)
+        cnt = sq.lsh_candidates(sig, 16, 4, cap, pairs)
+        assert cnt == m * (m - 1) // 2
+        if cnt:
+            got = _u32(pairs)[:cnt]
+            assert got.max() == m - 1                     # the cap SMALLEST indices are kept
+            ii, jj = np.triu_indices(m, 1)
+            assert np.array_equal(got[:, 0], ii) and np.array_equal(got[:, 1], jj)
+    sq.close()
+
+
+def test_error_codes():
+    binding, sq = _ctx()
+    sq.set_workspace(1 << 22)
+    seqs = torch.tensor([1, 2, 25, 3], dtype=torch.uint8, device="cuda")     # 25 >= alphabet 20
+    offs = torch.tensor([0, 2, 4], dtype=torch.int64, device="cuda")
+    with pytest.raises(binding.SubQuadError) as ei:
+        sq.pack(seqs, offs, alphabet=20, max_len=8)
+    assert ei.value.code == binding.SQ_ERR_BAD_RESIDUE
+    with pytest.raises(binding.SubQuadError) as ei:              # nothing packed after a failure
+        sq.minhash(3, 32, SEED)
+    assert ei.value.code == binding.SQ_ERR_NOT_PACKED
+    with pytest.raises(binding.SubQuadError) as ei:              # longer than the declared bound
+        sq.pack(torch.zeros(40, dtype=torch.uint8, device="cuda"),
+                torch.tensor([0, 40], dtype=torch.int64, device="cuda"), alphabet=20, max_len=8)
+    assert ei.value.code == binding.SQ_ERR_BAD_RESIDUE
+    with pytest.raises(binding.SubQuadError) as ei:
+        sq.pack(seqs, offs, alphabet=20, max_len=1000)
+    assert ei.value.code == binding.SQ_ERR_UNSUPPORTED
+    sq.pack(torch.tensor([1, 2, 5, 3], dtype=torch.uint8, device="cuda"), offs, alphabet=20, max_len=8)
+    with pytest.raises(binding.SubQuadError) as ei:
+        sq.minhash(7, 32, SEED)                                  # 5k > 32
+    assert ei.value.code == binding.SQ_ERR_INVALID_ARG
+    sig = sq.minhash(2, 32, SEED)
+    pairs = torch.empty((8, 2), dtype=torch.int32, device="cuda")
+    with pytest.raises(binding.SubQuadError) as ei:
+        sq.lsh_candidates(sig, 16, 4, 10, pairs)                 # bands*rows > H
+    assert ei.value.code == binding.SQ_ERR_INVALID_ARG
+    small = binding.SubQuad(0)
+    small.set_workspace(8192)
+    with pytest.raises(binding.SubQuadError) as ei:
+        small.pack(torch.zeros(10_000, dtype=torch.uint8, device="cuda"),
+                   torch.arange(0, 10_001, 10, dtype=torch.int64, device="cuda"), 20, 10)
+    assert ei.value.code == binding.SQ_ERR_WORKSPACE
+    small.close()
+    sq.close()
