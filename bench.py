@@ -1,0 +1,425 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the SubQuad candidate-pair affinity path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload configX] [--impl reference]
+
+A step = one pass of the whole hot path over one synthetic repertoire:
+    sq_pack -> sq_minhash -> sq_lsh_candidates (sorted) -> sq_edit_distance
+with the inputs resident in HBM (`value`), and the same through sq_pipeline_host with pinned
+HOST buffers, copies inside the timed region (`e2e`).  Prints ONE JSON line (rank 0).
+Multi-GPU: the path partitions into independent repertoires (donors), one per rank, no
+data-path collective ("scaling": "weak").  `--impl reference` times the CPU oracle.
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2602_17330_b200 import datagen as dg  # noqa: E402
+
+METRIC = "candidate_pairs_verified_per_s"
+UNIT = "pairs/s"
+INSTR_PER_COLUMN_WORD = 14          # algorithmic integer ops per unit
+# bounded oracle samples (first n_s sequences of the same workload)
+ORACLE_SAMPLE = {"config1": 2000, "config2": 100_000, "config3": 300_000, "config4": 300_000}
+CAP_PER_SEQ = {"config2": 40, "config3": 60, "config4": 200}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default=os.environ.get("SQ_BENCH_WORKLOAD", "config4"),
+                    choices=["config2", "config3", "config4"])
+    ap.add_argument("--n", type=int, default=0, help="override the number of sequences")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "200", "-i", str(self.index)],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except Exception:
+            self.proc.kill()
+            out = ""
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.strip().splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 6:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": statistics.median(sm) if sm else None,
+                "sm_max_mhz": max(mx) if mx else None, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def make_repertoire(workload, n, rank):
+    gen = dg.GENERATORS[workload]
+    rep = gen(n, seed=rank) if n else gen(seed=rank)
+    return rep
+
+
+# ---------------------------------------------------------------------------------------------
+# reference arm / cpu_baseline: the oracle as it stands, on a bounded sample
+# ---------------------------------------------------------------------------------------------
+def oracle_step(rep_sample, P):
+    import oracle
+    t0 = time.perf_counter()
+    sig = oracle.minhash(rep_sample.seqs, rep_sample.offsets, P["k"], P["H"], dg.DEFAULT_SEED64)
+    t1 = time.perf_counter()
+    pairs, raw, _ = oracle.lsh_sorted(sig, P["bands"], P["rows"], P["cap"])
+    t2 = time.perf_counter()
+    dist = oracle.edit_distance_pairs(rep_sample.seqs, rep_sample.offsets, pairs, P["max_d"])
+    t3 = time.perf_counter()
+    L = rep_sample.lengths
+    cells = float((L[pairs[:, 0]].astype(np.float64) * L[pairs[:, 1]]).sum()) if pairs.size else 0.0
+    return {"pairs": int(pairs.shape[0]), "t": t3 - t0, "t_minhash": t1 - t0, "t_lsh": t2 - t1,
+            "t_edit": t3 - t2, "cells": cells, "hits": int((dist <= P["max_d"]).sum())}
+
+
+def sample_of(rep, n_s):
+    n_s = min(n_s, rep.n)
+    end = int(rep.offsets[n_s])
+    return dg.Repertoire(rep.seqs[:end], rep.offsets[:n_s + 1].copy(), rep.family[:n_s],
+                         rep.n_edits[:n_s], rep.name)
+
+
+def cpu_baseline(rep, workload, P):
+    import oracle
+    n_s = ORACLE_SAMPLE[workload]
+    s = sample_of(rep, n_s)
+    r = oracle_step(s, P)
+    return {"value": r["pairs"] / r["t"], "unit": UNIT, "cores": oracle.num_threads(),
+            "kind": "oracle",
+            "sample": f"first {s.n} sequences of {workload} (of {rep.n}); {r['pairs']} candidate "
+                      f"pairs in {r['t']:.2f} s (minhash {r['t_minhash']:.2f} s, lsh "
+                      f"{r['t_lsh']:.2f} s single-thread qsort, edit {r['t_edit']:.2f} s)",
+            "minhash_seqs_per_s": s.n / max(r["t_minhash"], 1e-9),
+            "edit_gcups": r["cells"] / max(r["t_edit"], 1e-9) / 1e9}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    workload = args.workload
+    P = dg.PARAMS[workload]
+    n_s = min(ORACLE_SAMPLE[workload], 100_000)
+    rep = dg.GENERATORS[workload](n_s, seed=0)
+    for _ in range(args.warmup):
+        oracle_step(rep, P)
+    ts, pairs = [], 0
+    for _ in range(args.steps):
+        r = oracle_step(rep, P)
+        ts.append(r["t"]); pairs = r["pairs"]
+    t = sum(ts)
+    value = pairs * args.steps / t
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u32/u64 integer",
+        "data": "synthetic", "gpu_launches": 0,
+        "config": {"workload": f"{workload} generator at n={n_s} (bounded oracle sample)",
+                   **{k: P[k] for k in ("k", "H", "bands", "rows", "cap", "max_d")}},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(),
+                         "kind": "oracle",
+                         "sample": f"{workload} generator at n={n_s}, {pairs} pairs per step"},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line))
+
+
+# ---------------------------------------------------------------------------------------------
+# our arm
+# ---------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2602_17330_b200 import binding
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    workload = args.workload
+    P = dg.PARAMS[workload]
+    rep = make_repertoire(workload, args.n, rank)          # one independent repertoire per rank
+    n = rep.n
+    total_len = int(rep.offsets[-1])
+    max_len = int(rep.lengths.max())
+    sq = binding.SubQuad(local_rank)
+    stride = (max_len + 1 + 15) // 16 * 16
+
+    seqs_h = torch.from_numpy(rep.seqs).pin_memory()
+    offs_h = torch.from_numpy(rep.offsets).pin_memory()
+    seqs_d = seqs_h.to(dev, non_blocking=True)
+    offs_d = offs_h.to(dev, non_blocking=True)
+    sig = torch.empty((n, P["H"]), dtype=torch.int32, device=dev)
+
+    # capacity: start from an estimate, grow on SQ_ERR_CAPACITY (untimed)
+    capacity = int(CAP_PER_SEQ[workload] * n)
+    pairs = dist_out = None
+
+    def alloc(cap):
+        nonlocal pairs, dist_out
+        pairs = dist_out = None
+        torch.cuda.empty_cache()
+        ws = max(sq.workspace_bytes(binding.OP_LSH, n, total_len, max_len, P["H"], P["bands"],
+                                    P["cap"], cap),
+                 0 if args.no_e2e else sq.workspace_bytes(binding.OP_PIPELINE_HOST, n, total_len,
+                                                          max_len, P["H"], P["bands"], P["cap"], cap))
+        sq.workspace = None
+        sq.set_workspace(ws)
+        pairs = torch.empty((cap, 2), dtype=torch.int32, device=dev)
+        dist_out = torch.empty(cap, dtype=torch.int16, device=dev)
+
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+
+    def step(timed):
+        """one pass of the whole path; returns (count, [t_pack, t_minhash, t_lsh, t_edit] ms)"""
+        e = [ev() for _ in range(5)]
+        e[0].record()
+        sq.pack(seqs_d, offs_d, 20, max_len)
+        e[1].record()
+        sq.minhash(P["k"], P["H"], dg.DEFAULT_SEED64, sig)
+        e[2].record()
+        cnt = sq.lsh_candidates(sig, P["bands"], P["rows"], P["cap"], pairs)
+        e[3].record()
+        sq.edit_distance(pairs, cnt, P["max_d"], dist_out)
+        e[4].record()
+        e[4].synchronize()
+        return cnt, [e[i].elapsed_time(e[i + 1]) for i in range(4)]
+
+    alloc(capacity)
+    while True:
+        try:
+            cnt, _ = step(False)
+            break
+        except binding.SubQuadError as ex:
+            if ex.code != binding.SQ_ERR_CAPACITY:
+                raise
+            capacity = int(ex.required * 1.02) + 1024
+            alloc(capacity)
+    raw = sq.last_raw_pairs()
+
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
+
+    for _ in range(max(0, args.warmup - 1)):
+        step(False)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    sq.profile_enable(True)
+    sq.profile_reset()
+    launches0 = sq.kernel_launches()
+    t_steps, stages = [], []
+    wall0 = time.perf_counter()
+    for _ in range(args.steps):
+        flush.fill_(1)                     # L2 flush between timed iterations (outside the events)
+        torch.cuda.synchronize()
+        c2, st = step(True)
+        assert c2 == cnt
+        t_steps.append(sum(st)); stages.append(st)
+    torch.cuda.synchronize()
+    wall = time.perf_counter() - wall0
+    prof = sq.profile_read()
+    sq.profile_enable(False)
+    launches = sq.kernel_launches() - launches0
+    clocks = sampler.stop()
+    if world > 1:
+        dist.barrier()
+
+    step_ms = sum(t_steps) / args.steps
+    st_ms = [sum(s[i] for s in stages) / args.steps for i in range(4)]
+    # work units of this rank
+    lens = torch.from_numpy(rep.lengths.astype(np.int32)).to(dev)
+    pi = pairs[:cnt, 0].long(); pj = pairs[:cnt, 1].long()
+    cells = float((lens[pi].double() * lens[pj].double()).sum().item())
+    text_cols = float(lens[pj].double().sum().item())
+    hits = int((dist_out[:cnt] <= P["max_d"]).sum().item())
+    del pi, pj
+
+    # aggregate over ranks: units summed, time = max over ranks
+    agg = torch.tensor([step_ms, float(cnt), float(n), cells], dtype=torch.float64, device=dev)
+    if world > 1:
+        tmax = agg[:1].clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        tot = agg[1:].clone(); dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+        step_ms_all, cnt_all, n_all, cells_all = tmax.item(), tot[0].item(), tot[1].item(), tot[2].item()
+    else:
+        step_ms_all, cnt_all, n_all, cells_all = step_ms, float(cnt), float(n), cells
+
+    # ---- e2e: through the C ABI with HOST buffers -------------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        try:
+            pairs_h = torch.empty((capacity, 2), dtype=torch.int32).pin_memory()
+            dist_h = torch.empty(capacity, dtype=torch.int16).pin_memory()
+            e2e_steps = max(1, min(args.steps, 3))
+            sq.pipeline_host(seqs_h, offs_h, 20, max_len, P["k"], P["H"], dg.DEFAULT_SEED64,
+                             P["bands"], P["rows"], P["cap"], P["max_d"], pairs_h, dist_h)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            for _ in range(e2e_steps):
+                c3 = sq.pipeline_host(seqs_h, offs_h, 20, max_len, P["k"], P["H"],
+                                      dg.DEFAULT_SEED64, P["bands"], P["rows"], P["cap"],
+                                      P["max_d"], pairs_h, dist_h)
+            torch.cuda.synchronize()
+            t_e2e = (time.perf_counter() - t0) / e2e_steps
+            assert c3 == cnt
+            te = torch.tensor([t_e2e], dtype=torch.float64, device=dev)
+            if world > 1:
+                dist.all_reduce(te, op=dist.ReduceOp.MAX)
+            e2e = {"value": cnt_all / te.item(), "unit": UNIT,
+                   "h2d_bytes_per_step": total_len + 8 * (n + 1),
+                   "d2h_bytes_per_step": 10 * cnt, "ms_per_step": 1e3 * te.item(),
+                   "steps": e2e_steps, "api": "sq_pipeline_host (pinned host buffers)"}
+            del pairs_h, dist_h
+        except Exception as ex:               # e.g. not enough pinned host memory
+            e2e = {"value": None, "unit": UNIT, "error": repr(ex)[:200]}
+
+    if rank != 0:
+        return
+    # ---- rooflines ---------------------------------------------------------------------------
+    hbm_peak, peak_src = measured_peaks()
+    int_peak = {name: sq.int_peak(kind, 2048) for kind, name in
+                ((0, "lop3"), (1, "iadd"), (3, "imad"), (4, "umin"), (5, "lop3+imad"))}
+    B = P["bands"]
+    nb_bits = max(1, int(np.ceil(np.log2(max(n, 2)))))
+    pair_passes = 2 * ((nb_bits + 7) // 8)
+    K = args.steps
+    alg_bytes = {   # algorithmic bytes per STEP of each kernel class
+        "pack": total_len + 8 * (n + 1) + n * stride + 12 * n,
+        "minhash": n * (stride + 4 + 4 * P["H"]),
+        "band_key": n * (4 * P["H"] + 12 * B + 4),
+        "sort_hist": 8 * (8 * n * B + pair_passes * cnt + n),
+        "sort_scatter": 24 * (8 * n * B + n) + 16 * pair_passes * cnt,
+        "segment": n * B * (8 + 4 + 4 + 4 + 4 + 4 + 4 + 4),
+        "emit": 8 * cnt + 12 * n * B,
+    }
+    kernels = {}
+    tot_prof = sum(ms for ms, _ in prof.values()) or 1.0
+    for name, (ms, ln) in prof.items():
+        if ln == 0:
+            continue
+        k = {"ms_per_step": ms / K, "launches_per_step": ln / K, "share": ms / tot_prof}
+        if name in alg_bytes:
+            k["bound"] = "hbm"
+            k["achieved_GBs"] = alg_bytes[name] / (ms / K * 1e-3) / 1e9
+            k["frac"] = k["achieved_GBs"] / hbm_peak
+        if name == "edit_distance":
+            ops = INSTR_PER_COLUMN_WORD * text_cols * ((max_len + 31) // 32)
+            k["bound"] = "alu"
+            k["achieved_Gops"] = ops / (ms / K * 1e-3) / 1e9
+            k["frac"] = k["achieved_Gops"] * 1e9 / int_peak["lop3"]
+        if name == "minhash":
+            L = rep.lengths
+            upd = float(np.maximum(L - P["k"] + 1, 0).sum()) * P["H"]
+            k["alu_Gupdates_per_s"] = upd / (ms / K * 1e-3) / 1e9
+            k["alu_frac_of_imad_peak"] = upd / (ms / K * 1e-3) / int_peak["imad"]
+        kernels[name] = k
+    dom = max(kernels, key=lambda q: kernels[q]["ms_per_step"])
+    kd = kernels[dom]
+    if kd.get("bound") == "alu":
+        roof = {"kernel": dom, "bound": "alu", "achieved": kd["achieved_Gops"],
+                "peak": int_peak["lop3"] / 1e9, "unit": "Gop/s", "frac": kd["frac"], "traffic": None,
+                "peak_source": "sq_int_peak LOP3 stream measured in this run"}
+    else:
+        roof = {"kernel": dom, "bound": "hbm", "achieved": kd.get("achieved_GBs"), "peak": hbm_peak,
+                "unit": "GB/s", "frac": kd.get("frac"), "traffic": None, "peak_source": peak_src}
+    roof["avg_launch_ms"] = kd["ms_per_step"] / max(kd["launches_per_step"], 1)
+
+    cpu = None if args.no_cpu_baseline else cpu_baseline(rep, workload, P)
+    line = {
+        "metric": METRIC, "value": cnt_all / (step_ms_all * 1e-3), "unit": UNIT,
+        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": step_ms_all,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "u32/u64 integer", "data": "synthetic",
+        "config": {"workload": f"{workload}: N={n} CDR3-like sequences per GPU "
+                               f"(BASELINE.json configs[{int(workload[-1]) - 1}])",
+                   **{k: P[k] for k in ("k", "H", "bands", "rows", "cap", "max_d")},
+                   "candidate_pairs": cnt, "raw_pairs_before_dedupe": raw, "hits": hits,
+                   "timing": "CUDA events per step on the library's stream; 256 MB L2 flush "
+                             "between timed steps (outside the events); parallelism: one "
+                             "independent repertoire per GPU, no collective"},
+        "stages": {"pack_ms": st_ms[0], "minhash_ms": st_ms[1], "lsh_ms": st_ms[2],
+                   "edit_ms": st_ms[3],
+                   "minhash_seqs_per_s": n / (st_ms[1] * 1e-3),
+                   "lsh_candidate_pairs_per_s": cnt / (st_ms[2] * 1e-3),
+                   "lsh_raw_pairs_per_s": raw / (st_ms[2] * 1e-3),
+                   "edit_pairs_per_s": cnt / (st_ms[3] * 1e-3),
+                   "edit_gcups": cells / (st_ms[3] * 1e-3) / 1e9,
+                   "wall_s_timed_region": wall},
+        "roofline": roof, "kernels": kernels, "int_peak_ops_per_s": int_peak,
+        "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+    }
+    print(json.dumps(line))
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

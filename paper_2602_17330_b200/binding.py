@@ -25,7 +25,8 @@ LSH_SORTED, LSH_UNORDERED = 0, 1
 EXPORTS = ["sq_create", "sq_destroy", "sq_workspace_bytes", "sq_set_workspace", "sq_pack",
            "sq_minhash", "sq_lsh_candidates", "sq_edit_distance", "sq_all_pairs",
            "sq_pipeline_host", "sq_packed_n", "sq_packed_stride", "sq_last_raw_pairs",
-           "sq_kernel_launches", "sq_last_cuda_error", "sq_strerror", "sq_int_peak"]
+           "sq_kernel_launches", "sq_last_cuda_error", "sq_strerror", "sq_int_peak",
+           "sq_profile_enable", "sq_profile_reset", "sq_profile_read", "sq_profile_name"]
 
 
 class SqSizes(C.Structure):
@@ -90,6 +91,14 @@ def load_library():
     L.sq_strerror.argtypes = [i32]
     L.sq_int_peak.restype = i32
     L.sq_int_peak.argtypes = [vp, i32, i32, C.POINTER(C.c_double)]
+    L.sq_profile_enable.restype = i32
+    L.sq_profile_enable.argtypes = [vp, i32]
+    L.sq_profile_reset.restype = i32
+    L.sq_profile_reset.argtypes = [vp]
+    L.sq_profile_read.restype = i32
+    L.sq_profile_read.argtypes = [vp, i32, C.POINTER(C.c_double), C.POINTER(i64)]
+    L.sq_profile_name.restype = C.c_char_p
+    L.sq_profile_name.argtypes = [i32]
     _lib = L
     return L
 
@@ -231,6 +240,26 @@ class SubQuad:
 
     def kernel_launches(self) -> int:
         return int(self.lib.sq_kernel_launches(self.h))
+
+    def profile_enable(self, on: bool = True):
+        self._check(self.lib.sq_profile_enable(self.h, 1 if on else 0))
+
+    def profile_reset(self):
+        self._check(self.lib.sq_profile_reset(self.h))
+
+    def profile_read(self) -> dict:
+        """{kernel class: (milliseconds, launches)} accumulated since the last reset."""
+        out = {}
+        k = 0
+        while True:
+            name = self.lib.sq_profile_name(k)
+            if not name:
+                break
+            ms, ln = C.c_double(0.0), C.c_int64(0)
+            self._check(self.lib.sq_profile_read(self.h, k, C.byref(ms), C.byref(ln)))
+            out[name.decode()] = (ms.value, ln.value)
+            k += 1
+        return out
 
     def int_peak(self, kind: int, iters: int = 4096) -> float:
         out = C.c_double(0.0)
