@@ -46,7 +46,7 @@ extern "C" {
 
 #define SQ_MAX_LEN    240   /* longest sequence the packed layout and the DP kernels accept   */
 #define SQ_MAX_H      256   /* largest signature length ({64,128,256})        */
-#define SQ_MAX_BANDS   64
+#define SQ_MAX_BANDS   32
 
 /* operations, for sq_workspace_bytes */
 #define SQ_OP_PACK            0
@@ -58,7 +58,8 @@ extern "C" {
 
 /* flags of sq_lsh_candidates */
 #define SQ_LSH_SORTED     0   /* pairs_out ascending by (i, j) (default)                      */
-#define SQ_LSH_UNORDERED  1   /* same SET of pairs, order unspecified (skips the final sort)  */
+#define SQ_LSH_UNORDERED  1   /* caller does not need the order (the current kernels emit
+                                 ascending (i, j) either way, at no extra cost)               */
 
 typedef struct sq_ctx sq_ctx;   /* opaque; owns only small host metadata + 2 pinned words */
 

@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libsubquad.so")
 SQ_OK = 0
 SQ_ERR_INVALID_ARG, SQ_ERR_BAD_RESIDUE, SQ_ERR_NOT_PACKED, SQ_ERR_CAPACITY = -1, -2, -3, -4
 SQ_ERR_WORKSPACE, SQ_ERR_UNSUPPORTED, SQ_ERR_CUDA = -5, -6, -7
-SQ_MAX_LEN, SQ_MAX_H, SQ_MAX_BANDS = 240, 256, 64
+SQ_MAX_LEN, SQ_MAX_H, SQ_MAX_BANDS = 240, 256, 32
 OP_PACK, OP_MINHASH, OP_LSH, OP_EDIT_DISTANCE, OP_ALL_PAIRS, OP_PIPELINE_HOST = range(6)
 LSH_SORTED, LSH_UNORDERED = 0, 1
 

@@ -109,10 +109,11 @@ int sq_radix_sort(sq_ctx* c, uint64_t* keys_in, uint64_t* keys_alt, uint32_t* va
                   uint32_t* vals_alt, int64_t n, int nbatch, const int* shifts, const int* widths,
                   int npasses, void* tmp, int* result_in_alt);
 
-// exclusive prefix sum of uint32 -> uint64 totals are not needed: callers guarantee < 2^32.
-// In-place capable (out may equal in).  `tmp` needs (n/2048 + 2) * 4 bytes.
+// exclusive prefix sum of uint32 (offsets wrap mod 2^32; the grand total is returned in 64 bits
+// so callers can detect the wrap).  In-place capable (out may equal in).
+// `tmp` needs (n/2048 + 2) * 4 bytes.
 int sq_exclusive_scan_u32(sq_ctx* c, const uint32_t* in, uint32_t* out, int64_t n, uint32_t* tmp,
-                          uint32_t* total_out_dev /* may be nullptr */);
+                          unsigned long long* total_out_dev /* may be nullptr */);
 
 // ---- ops implemented in their own translation units ----
 int sq_minhash_impl(sq_ctx* c, int k, int H, uint64_t seed, uint32_t* sig_out);

@@ -6,21 +6,22 @@
 //                        test; records (key, id) are written band-major.
 //   a4 sq_radix_sort     stable LSD radix sort of every band's records by key (ids ascend
 //                        inside a bucket because the sort is stable and ids start ascending).
-//   a5 segment_kernel    bucket boundaries -> bucket id of every sorted record;
-//      bucket_id_kernel  bid[id][b] = bucket id if the record is among the `cap` smallest ids
-//                        of its bucket, else a unique "not kept" value;
-//      emit_kernel       one thread per sorted record p: pairs (id[p], id[q]) for the kept q > p
-//                        of the same bucket.  A pair is emitted only from the FIRST band in which
-//                        both ends are kept in the same bucket (checked against bid[][0..b)), so
-//                        the output is duplicate free without ever materialising the raw pairs.
-//      final radix sort  of the unique pairs by (i, j)   (skipped with SQ_LSH_UNORDERED).
+//   a5 head_flag / segment kernels: bucket boundaries of the sorted records;
+//      range_kernel      for every (sequence, band): the slice of the sorted id array holding
+//                        the kept members AFTER it in its bucket (the `cap` smallest ids of a
+//                        bucket are kept) -- an ascending run of partner ids;
+//      merge_rows_kernel one warp per sequence i, lane b = band b: warp-wide B-way merge of the
+//                        <= 32 ascending runs.  Equal heads advance together, so a pair found in
+//                        several bands is emitted once, and row i comes out ascending in j.
+//                        Pass 1 counts, a scan gives row offsets (and the total, so a too-small
+//                        output is reported before anything is written), pass 2 writes (i, j).
+//   The output is ascending in (i, j) by construction: no pair sort, no raw-pair buffer.
 #include "sq_common.cuh"
 
 namespace {
 
 constexpr uint64_t kKeyInit = 0x6A09E667F3BCC908ull;
 constexpr uint64_t kKeyMult = 0x9E3779B97F4A7C15ull;
-constexpr uint32_t kNotKept = 0x80000000u;
 
 __global__ void __launch_bounds__(256)
 band_key_kernel(const uint32_t* __restrict__ sig, int64_t n, int H, int bands, int rows,
@@ -92,114 +93,140 @@ seg_fix_kernel(const uint32_t* excl, const uint32_t* __restrict__ head, int64_t 
   seg[p] = excl[p] + head[p] - 1u;
 }
 
+// For every sorted record p (band b, sequence id): the slice of the sorted id array holding the
+// partners id can be paired with in this band -- the kept members AFTER p in p's bucket:
+// range[id][b] = (p+1, min(bucket end, bucket start + cap)) if p itself is kept, else (0,0).
+// Also accumulates the number of raw (pre-dedupe) pairs.
 __global__ void __launch_bounds__(256)
-bucket_id_kernel(const uint32_t* __restrict__ ids, const uint32_t* __restrict__ seg,
-                 const uint32_t* __restrict__ heads_pos, int64_t n2, int64_t total, int bands,
-                 int cap, uint32_t* __restrict__ bid) {
-  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (p >= total) return;
-  const int b = (int)(p / n2);
-  const uint32_t sg = seg[p];
-  const uint32_t s = heads_pos[sg];
-  const bool kept = (uint32_t)p - s < (uint32_t)cap;
-  bid[(int64_t)ids[p] * bands + b] = kept ? sg : (kNotKept | (uint32_t)p);
-}
-
-constexpr int kEmitThreads = 256;
-constexpr int kEmitStage = 256;   // pairs staged per warp before one global reservation
-
-__global__ void __launch_bounds__(kEmitThreads)
-emit_kernel(const uint32_t* __restrict__ ids, const uint32_t* __restrict__ seg,
-            const uint32_t* __restrict__ heads_pos, const uint32_t* __restrict__ bid, int64_t n2,
-            int64_t total, int bands, int cap, uint64_t* __restrict__ out,
-            unsigned long long capacity, unsigned long long* __restrict__ counters) {
-  __shared__ uint64_t stage[kEmitThreads / 32][kEmitStage];
+range_kernel(const uint32_t* __restrict__ ids, const uint32_t* __restrict__ seg,
+             const uint32_t* __restrict__ heads_pos, int64_t n2, int64_t total, int bands, int cap,
+             uint2* __restrict__ range, unsigned long long* __restrict__ raw_counter) {
   __shared__ unsigned long long raw_block;
-  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  const uint32_t lt = (1u << lane) - 1u;
   if (threadIdx.x == 0) raw_block = 0ull;
   __syncthreads();
-  const int64_t p = (int64_t)blockIdx.x * kEmitThreads + threadIdx.x;
-  uint32_t cnt = 0, u = 0;
-  int b = 0;
+  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  uint32_t cnt = 0;
   if (p < total) {
-    b = (int)(p / n2);
+    const int b = (int)(p / n2);
     const uint32_t sg = seg[p];
     const uint32_t s = heads_pos[sg], e = heads_pos[sg + 1];
     const uint32_t ek = min(e, s + (uint32_t)cap);
-    if ((uint32_t)p < ek) cnt = ek - (uint32_t)p - 1u;
-    u = ids[p];
+    uint2 r = make_uint2(0u, 0u);
+    if ((uint32_t)p + 1u < ek) { r = make_uint2((uint32_t)p + 1u, ek); cnt = ek - (uint32_t)p - 1u; }
+    range[(int64_t)ids[p] * bands + b] = r;
   }
-  const uint32_t maxcnt = __reduce_max_sync(0xFFFFFFFFu, cnt);
-  const uint32_t* urow = bid + (int64_t)u * bands;
-  uint32_t wcount = 0;   // warp-uniform fill of stage[w]
-  for (uint32_t off = 1; off <= maxcnt; ++off) {
-    bool ok = false;
-    uint32_t v = 0;
-    if (off <= cnt) {
-      v = ids[p + off];
-      ok = true;
-      const uint32_t* vrow = bid + (int64_t)v * bands;
-      for (int bb = 0; bb < b; ++bb)
-        if (urow[bb] == vrow[bb]) { ok = false; break; }
-    }
-    const uint32_t mask = __ballot_sync(0xFFFFFFFFu, ok);
-    const uint32_t add = __popc(mask);
-    if (wcount + add > kEmitStage) {         // flush the warp's stage
-      unsigned long long base = 0;
-      if (lane == 0) base = atomicAdd(&counters[0], (unsigned long long)wcount);
-      base = __shfl_sync(0xFFFFFFFFu, base, 0);
-      for (uint32_t t = lane; t < wcount; t += 32)
-        if (base + t < capacity) out[base + t] = stage[w][t];
-      __syncwarp();
-      wcount = 0;
-    }
-    if (ok) stage[w][wcount + __popc(mask & lt)] = (uint64_t)u | ((uint64_t)v << 32);
-    wcount += add;
-    __syncwarp();
-  }
-  if (wcount) {
-    unsigned long long base = 0;
-    if (lane == 0) base = atomicAdd(&counters[0], (unsigned long long)wcount);
-    base = __shfl_sync(0xFFFFFFFFu, base, 0);
-    for (uint32_t t = lane; t < wcount; t += 32)
-      if (base + t < capacity) out[base + t] = stage[w][t];
-  }
-  // raw (pre-dedupe) pair count, for reporting
-  uint32_t wsum = __reduce_add_sync(0xFFFFFFFFu, cnt);
-  if (lane == 0 && wsum) atomicAdd(&raw_block, (unsigned long long)wsum);
+  const uint32_t wsum = __reduce_add_sync(0xFFFFFFFFu, cnt);
+  if ((threadIdx.x & 31) == 0 && wsum) atomicAdd(&raw_block, (unsigned long long)wsum);
   __syncthreads();
-  if (threadIdx.x == 0 && raw_block) atomicAdd(&counters[1], raw_block);
+  if (threadIdx.x == 0 && raw_block) atomicAdd(raw_counter, raw_block);
 }
 
-inline int bits_for(int64_t n) {   // bits needed to represent values in [0, n)
-  int b = 1;
-  while (b < 32 && (1ll << b) < n) ++b;
-  return b;
+// Row-centric emission.  A group of G lanes (G = 16 for <= 16 bands, else 32) owns sequence i;
+// lane l of the group owns band l's partner slice (an ascending run of ids, all > i).  The union
+// of the runs is produced by a group-wide B-way merge: every step takes the minimum head (REDUX),
+// emits it once, and advances EVERY lane whose head equals it -- duplicates across bands vanish
+// and the row comes out ascending.  Each lane keeps its head plus kLook look-ahead ids in
+// registers; the load issued at an advance is consumed kLook advances later, so the serial merge
+// chain does not wait on global memory.
+// FILL = false: count the row's unique partners.  FILL = true: write (i, j) pairs at the row's
+// offset, G at a time.
+constexpr int kMergeWarps = 8;
+constexpr int kLook = 6;
+
+template <int G, bool FILL>
+__global__ void __launch_bounds__(kMergeWarps * 32)
+merge_rows_kernel(const uint32_t* __restrict__ ids, const uint2* __restrict__ range, int64_t n,
+                  int bands, uint32_t* __restrict__ row_cnt, const uint32_t* __restrict__ row_off,
+                  uint2* __restrict__ pairs_out) {
+  constexpr int RPW = 32 / G;                        // rows per warp
+  constexpr uint32_t INF = 0xFFFFFFFFu;
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const int sub = lane / G, l = lane % G;
+  const int64_t row = ((int64_t)blockIdx.x * kMergeWarps + w) * RPW + sub;
+  const bool valid = row < n;
+  uint32_t cur = 0, end = 0;                         // next id to LOAD of this lane's run
+  if (valid && l < bands) {
+    const uint2 r = range[row * bands + l];
+    cur = r.x; end = r.y;
+  }
+  if (FILL && valid && row_cnt[row] == 0) end = cur;
+  if (__ballot_sync(0xFFFFFFFFu, cur < end) == 0) {
+    if (!FILL && valid && l == 0) row_cnt[row] = 0;
+    return;
+  }
+  uint32_t q[kLook + 1];                             // q[0] = head, q[1..] = look-ahead
+#pragma unroll
+  for (int t = 0; t <= kLook; ++t) { q[t] = cur < end ? ids[cur] : INF; ++cur; }
+  uint32_t c = 0, out = 0;
+  const uint32_t base = (FILL && valid) ? row_off[row] : 0u;
+  for (;;) {
+    uint32_t m;
+    if (RPW == 1) {
+      m = __reduce_min_sync(0xFFFFFFFFu, q[0]);
+      if (m == INF) break;
+    } else {
+      const uint32_t m0 = __reduce_min_sync(0xFFFFFFFFu, sub == 0 ? q[0] : INF);
+      const uint32_t m1 = __reduce_min_sync(0xFFFFFFFFu, sub == 1 ? q[0] : INF);
+      if ((m0 & m1) == INF) break;
+      m = sub == 0 ? m0 : m1;
+    }
+    const bool live = m != INF;
+    if (FILL && live) {
+      if (l == (int)(c & (G - 1))) out = m;
+      if ((c & (G - 1)) == G - 1)
+        pairs_out[base + (c & ~(uint32_t)(G - 1)) + l] = make_uint2((uint32_t)row, out);
+    }
+    c += live ? 1u : 0u;
+    if (live && q[0] == m) {
+#pragma unroll
+      for (int t = 0; t < kLook; ++t) q[t] = q[t + 1];
+      q[kLook] = cur < end ? ids[cur] : INF;
+      ++cur;
+    }
+  }
+  if (FILL) {
+    if (valid && l < (int)(c & (G - 1)))
+      pairs_out[base + (c & ~(uint32_t)(G - 1)) + l] = make_uint2((uint32_t)row, out);
+  } else {
+    if (valid && l == 0) row_cnt[row] = c;
+  }
+}
+
+template <bool FILL>
+int launch_merge(sq_ctx* c, const uint32_t* ids, const uint2* range, int64_t n, int bands,
+                 uint32_t* row_cnt, const uint32_t* row_off, uint2* pairs_out) {
+  if (bands <= 16) {
+    const int64_t rows_per_block = kMergeWarps * 2;
+    const unsigned g = (unsigned)((n + rows_per_block - 1) / rows_per_block);
+    SQ_TIMED(c, SQ_K_EMIT, merge_rows_kernel<16, FILL><<<g, kMergeWarps * 32, 0, c->stream>>>(
+        ids, range, n, bands, row_cnt, row_off, pairs_out));
+  } else {
+    const unsigned g = (unsigned)((n + kMergeWarps - 1) / kMergeWarps);
+    SQ_TIMED(c, SQ_K_EMIT, merge_rows_kernel<32, FILL><<<g, kMergeWarps * 32, 0, c->stream>>>(
+        ids, range, n, bands, row_cnt, row_off, pairs_out));
+  }
+  SQ_LAUNCH_CHECK(c);
+  return SQ_OK;
 }
 
 }  // namespace
 
-size_t sq_lsh_scratch_bytes(int64_t n, int bands, int64_t pair_capacity) {
+size_t sq_lsh_scratch_bytes(int64_t n, int bands, int64_t /*pair_capacity*/) {
   size_t nn = (size_t)(n > 0 ? n : 1), B = (size_t)(bands > 0 ? bands : 1);
-  size_t cap = (size_t)(pair_capacity > 0 ? pair_capacity : 1);
   size_t rec = nn * B;
   size_t s = 0;
-  s += 2 * sq_align_up(rec * 8 + 16);          // keys ping-pong
+  s += 2 * sq_align_up(rec * 8 + 16);          // keys ping-pong (the range table reuses one)
   s += 2 * sq_align_up(rec * 4 + 16);          // ids ping-pong
   s += 3 * sq_align_up((rec + 2) * 4 + 16);    // head flags, scan / seg ids, head positions
-  s += sq_align_up(rec * 4 + 16);              // bid table
-  s += sq_align_up((nn + 2) * 4 + 16);         // non-empty flags / ranks
-  size_t sort_recs = sq_sort_scratch_bytes(n, bands);
-  size_t sort_pairs = sq_sort_scratch_bytes(pair_capacity, 1);
-  s += sort_recs > sort_pairs ? sort_recs : sort_pairs;
-  s += sq_align_up(cap * 8 + 16);              // alternate pair buffer for the final sort
+  s += 2 * sq_align_up((nn + 2) * 4 + 16);     // non-empty flags / ranks; row counts / offsets
+  s += sq_sort_scratch_bytes(n, bands);
   return s + 4096;
 }
 
 extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int bands, int rows,
                                  int bucket_cap, int flags, uint32_t* pairs_out, int64_t capacity,
                                  int64_t* n_pairs) {
+  (void)flags;   // the row-centric merge always produces ascending (i, j)
   if (!c || !n_pairs) return SQ_ERR_INVALID_ARG;
   *n_pairs = 0;
   if (c->n < 0) return SQ_ERR_NOT_PACKED;
@@ -211,7 +238,7 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
   c->last_raw_pairs = 0;
   if (n == 0) return SQ_OK;
   if (!sig || (capacity > 0 && !pairs_out)) return SQ_ERR_INVALID_ARG;
-  if (n * bands >= (1ll << 31) || capacity >= (1ll << 32) - 1) return SQ_ERR_UNSUPPORTED;
+  if (n * bands >= (1ll << 31)) return SQ_ERR_UNSUPPORTED;
 
   sq_scratch_reset(c);
   const size_t rec = (size_t)n * bands;
@@ -222,13 +249,10 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
   uint32_t* head = sq_scratch<uint32_t>(c, rec + 2);
   uint32_t* seg = sq_scratch<uint32_t>(c, rec + 2);
   uint32_t* heads_pos = sq_scratch<uint32_t>(c, rec + 2);
-  uint32_t* bid = sq_scratch<uint32_t>(c, rec);
   uint32_t* nonempty = sq_scratch<uint32_t>(c, (size_t)n + 2);
-  size_t sort_recs = sq_sort_scratch_bytes(n, bands), sort_pairs = sq_sort_scratch_bytes(capacity, 1);
-  uint8_t* tmp = sq_scratch<uint8_t>(c, sort_recs > sort_pairs ? sort_recs : sort_pairs);
-  uint64_t* pairs_alt = sq_scratch<uint64_t>(c, (size_t)(capacity > 0 ? capacity : 1));
-  if (!k0 || !k1 || !v0 || !v1 || !head || !seg || !heads_pos || !bid || !nonempty || !tmp ||
-      !pairs_alt)
+  uint32_t* row_cnt = sq_scratch<uint32_t>(c, (size_t)n + 2);
+  uint8_t* tmp = sq_scratch<uint8_t>(c, sq_sort_scratch_bytes(n, bands));
+  if (!k0 || !k1 || !v0 || !v1 || !head || !seg || !heads_pos || !nonempty || !row_cnt || !tmp)
     return SQ_ERR_WORKSPACE;
   cudaStream_t st = c->stream;
   unsigned long long* counters = c->dflags;      // [0] unique, [1] raw, [2] n2, [3] nseg
@@ -238,13 +262,12 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
   const unsigned gb = (unsigned)((n + 255) / 256);
   SQ_TIMED(c, SQ_K_BANDKEY, band_key_kernel<<<gb, 256, 0, st>>>(sig, n, H, bands, rows, k0, v0, nonempty));
   SQ_LAUNCH_CHECK(c);
-  uint32_t* d_n2 = reinterpret_cast<uint32_t*>(counters + 2);
-  uint32_t* d_nseg = reinterpret_cast<uint32_t*>(counters + 3);
-  int rc = sq_exclusive_scan_u32(c, nonempty, nonempty, n, reinterpret_cast<uint32_t*>(tmp), d_n2);
+  int rc = sq_exclusive_scan_u32(c, nonempty, nonempty, n, reinterpret_cast<uint32_t*>(tmp),
+                                 counters + 2);
   if (rc != SQ_OK) return rc;
   SQ_CUDA(c, cudaMemcpyAsync(c->pinned, counters + 2, 8, cudaMemcpyDeviceToHost, st));
   SQ_CUDA(c, cudaStreamSynchronize(st));
-  const int64_t n2 = (int64_t)(uint32_t)c->pinned[0];
+  const int64_t n2 = (int64_t)c->pinned[0];
   if (n2 < 2) return SQ_OK;                       // fewer than two usable signatures: no pairs
   uint64_t* kin = k0; uint64_t* kalt = k1; uint32_t* vin = v0; uint32_t* valt = v1;
   if (n2 != n) {
@@ -261,12 +284,12 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
     if (rc != SQ_OK) return rc;
     if (in_alt) { uint64_t* t = kin; kin = kalt; kalt = t; uint32_t* tv = vin; vin = valt; valt = tv; }
   }
-  // a5: buckets
+  // a5: buckets -> per (sequence, band) partner slices
   const int64_t total = n2 * bands;
   const unsigned gt = (unsigned)((total + 255) / 256);
   SQ_TIMED(c, SQ_K_SEGMENT, head_flag_kernel<<<gt, 256, 0, st>>>(kin, n2, total, head));
   SQ_LAUNCH_CHECK(c);
-  rc = sq_exclusive_scan_u32(c, head, seg, total, reinterpret_cast<uint32_t*>(tmp), d_nseg);
+  rc = sq_exclusive_scan_u32(c, head, seg, total, reinterpret_cast<uint32_t*>(tmp), counters + 3);
   if (rc != SQ_OK) return rc;
   SQ_CUDA(c, cudaMemcpyAsync(c->pinned, counters + 3, 8, cudaMemcpyDeviceToHost, st));
   SQ_CUDA(c, cudaStreamSynchronize(st));
@@ -275,39 +298,28 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
   SQ_LAUNCH_CHECK(c);
   SQ_TIMED(c, SQ_K_SEGMENT, seg_fix_kernel<<<gt, 256, 0, st>>>(seg, head, total, seg));
   SQ_LAUNCH_CHECK(c);
-  SQ_TIMED(c, SQ_K_SEGMENT, bucket_id_kernel<<<gt, 256, 0, st>>>(vin, seg, heads_pos, n2, total, bands, bucket_cap, bid));
+  // the sorted keys are dead now: their buffer becomes the [n][bands] range table (8 B / entry)
+  uint2* range = reinterpret_cast<uint2*>(kalt);
+  SQ_CUDA(c, cudaMemsetAsync(range, 0, rec * 8, st));
+  SQ_TIMED(c, SQ_K_SEGMENT, range_kernel<<<gt, 256, 0, st>>>(vin, seg, heads_pos, n2, total, bands,
+                                                             bucket_cap, range, counters + 1));
   SQ_LAUNCH_CHECK(c);
-  // unique pairs, unordered; land them so that the final sort ends in pairs_out
-  const int nb = bits_for(n);
-  const int per_field = (nb + 7) / 8;
-  const int npasses = (flags & SQ_LSH_UNORDERED) ? 0 : 2 * per_field;
-  uint64_t* pout = reinterpret_cast<uint64_t*>(pairs_out);
-  uint64_t* emit_to = (npasses & 1) ? pairs_alt : pout;
-  SQ_TIMED(c, SQ_K_EMIT, emit_kernel<<<gt, kEmitThreads, 0, st>>>(
-      vin, seg, heads_pos, bid, n2, total, bands, bucket_cap, emit_to,
-      (unsigned long long)capacity, counters));
-  SQ_LAUNCH_CHECK(c);
+  // a5: row-centric merge, pass 1 = count, scan, pass 2 = fill
+  rc = launch_merge<false>(c, vin, range, n, bands, row_cnt, nullptr, nullptr);
+  if (rc != SQ_OK) return rc;
+  uint32_t* row_off = nonempty;                  // ranks are dead: reuse for the row offsets
+  rc = sq_exclusive_scan_u32(c, row_cnt, row_off, n, reinterpret_cast<uint32_t*>(tmp), counters);
+  if (rc != SQ_OK) return rc;
   SQ_CUDA(c, cudaMemcpyAsync(c->pinned, counters, 16, cudaMemcpyDeviceToHost, st));
   SQ_CUDA(c, cudaStreamSynchronize(st));
   const int64_t uniq = (int64_t)c->pinned[0];
   c->last_raw_pairs = (int64_t)c->pinned[1];
   *n_pairs = uniq;
   if (uniq > capacity) return SQ_ERR_CAPACITY;
-  if (npasses > 0 && uniq > 0) {
-    int shifts[8], widths[8];
-    int q = 0;
-    for (int f = 0; f < 2; ++f) {                 // minor field j (high word) first, then i
-      const int base = f == 0 ? 32 : 0;
-      for (int p = 0; p < per_field; ++p) {
-        shifts[q] = base + 8 * p;
-        widths[q] = (nb - 8 * p) >= 8 ? 8 : (nb - 8 * p);
-        ++q;
-      }
-    }
-    int in_alt = 0;
-    uint64_t* other = (emit_to == pout) ? pairs_alt : pout;
-    rc = sq_radix_sort(c, emit_to, other, nullptr, nullptr, uniq, 1, shifts, widths, npasses, tmp,
-                       &in_alt);
+  if (uniq >= (1ll << 32) - 1) return SQ_ERR_UNSUPPORTED;   // 32-bit row offsets
+  if (uniq > 0) {
+    rc = launch_merge<true>(c, vin, range, n, bands, row_cnt, row_off,
+                            reinterpret_cast<uint2*>(pairs_out));
     if (rc != SQ_OK) return rc;
     SQ_CUDA(c, cudaStreamSynchronize(st));
   }

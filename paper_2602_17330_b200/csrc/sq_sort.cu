@@ -63,15 +63,16 @@ scan_reduce_kernel(const uint32_t* __restrict__ in, int64_t n, uint32_t* __restr
 
 // single block: exclusive scan of block_sums in place; writes the grand total
 __global__ void __launch_bounds__(kScanThreads)
-scan_spine_kernel(uint32_t* __restrict__ block_sums, int64_t nblk, uint32_t* __restrict__ total_out) {
+scan_spine_kernel(uint32_t* __restrict__ block_sums, int64_t nblk,
+                  unsigned long long* __restrict__ total_out) {
   __shared__ uint32_t sh[9];
-  uint32_t carry = 0;
+  unsigned long long carry = 0;    // the grand total is kept in 64 bits so a wrap is detectable
   for (int64_t base = 0; base < nblk; base += kScanThreads) {
     int64_t idx = base + threadIdx.x;
     uint32_t v = idx < nblk ? block_sums[idx] : 0;
     uint32_t tot;
     uint32_t ex = block_excl_scan(v, sh, &tot);
-    if (idx < nblk) block_sums[idx] = ex + carry;
+    if (idx < nblk) block_sums[idx] = ex + (uint32_t)carry;
     carry += tot;
   }
   if (threadIdx.x == 0 && total_out) *total_out = carry;
@@ -192,9 +193,9 @@ size_t sq_sort_scratch_bytes(int64_t n, int nbatch) {
 }
 
 int sq_exclusive_scan_u32(sq_ctx* c, const uint32_t* in, uint32_t* out, int64_t n, uint32_t* tmp,
-                          uint32_t* total_out_dev) {
+                          unsigned long long* total_out_dev) {
   if (n <= 0) {
-    if (total_out_dev) SQ_CUDA(c, cudaMemsetAsync(total_out_dev, 0, 4, c->stream));
+    if (total_out_dev) SQ_CUDA(c, cudaMemsetAsync(total_out_dev, 0, 8, c->stream));
     return SQ_OK;
   }
   int64_t nblk = (n + kScanChunk - 1) / kScanChunk;
