@@ -58,20 +58,27 @@ def measured_peaks():
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region."""
-    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,"
+    """nvidia-smi clocks / throttle reasons sampled every 100 ms.  The process is started BEFORE
+    the warm-up (its start-up stalls the GPU for a while) and only the samples stamped inside
+    the timed region [mark(), stop()] are kept."""
+    Q = ("timestamp,clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
 
     def __init__(self, index):
         self.index = index
         self.proc = None
+        self.t_mark = None
+
+    def mark(self):
+        import datetime
+        self.t_mark = datetime.datetime.now()
 
     def start(self):
         try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                 "-lms", "200", "-i", str(self.index)],
+                 "-lms", "100", "-i", str(self.index)],
                 stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
         except Exception:
             self.proc = None
@@ -79,7 +86,9 @@ class ClockSampler:
     def stop(self):
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.25)
+        import datetime
+        t_end = datetime.datetime.now()
+        time.sleep(0.15)
         self.proc.terminate()
         try:
             out, _ = self.proc.communicate(timeout=5)
@@ -88,11 +97,16 @@ class ClockSampler:
             out = ""
         sm, mx, reasons = [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        margin = datetime.timedelta(milliseconds=120)
         for line in out.strip().splitlines():
             f = [x.strip() for x in line.split(",")]
-            if len(f) < 6:
+            if len(f) < 7:
                 continue
             try:
+                ts = datetime.datetime.strptime(f[0], "%Y/%m/%d %H:%M:%S.%f")
+                if self.t_mark is not None and not (self.t_mark - margin <= ts <= t_end + margin):
+                    continue
+                f = f[1:]
                 sm.append(float(f[0])); mx.append(float(f[1]))
             except ValueError:
                 continue
@@ -260,13 +274,15 @@ def run_ours(args):
 
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
 
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    time.sleep(1.0)                        # let nvidia-smi finish its start-up outside the timing
     for _ in range(max(0, args.warmup - 1)):
         step(False)
     if world > 1:
         dist.barrier()
     torch.cuda.synchronize()
-    sampler = ClockSampler(local_rank)
-    sampler.start()
+    sampler.mark()
     sq.profile_enable(True)
     sq.profile_reset()
     launches0 = sq.kernel_launches()
@@ -342,17 +358,19 @@ def run_ours(args):
     int_peak = {name: sq.int_peak(kind, 2048) for kind, name in
                 ((0, "lop3"), (1, "iadd"), (3, "imad"), (4, "umin"), (5, "lop3+imad"))}
     B = P["bands"]
-    nb_bits = max(1, int(np.ceil(np.log2(max(n, 2)))))
-    pair_passes = 2 * ((nb_bits + 7) // 8)
     K = args.steps
+    rec = n * B                                    # (sequence, band) records
+    sw = 4 * (1 if B <= 4 else 2 if B <= 8 else 4 if B <= 16 else 8)   # S row width (words)
     alg_bytes = {   # algorithmic bytes per STEP of each kernel class
         "pack": total_len + 8 * (n + 1) + n * stride + 12 * n,
         "minhash": n * (stride + 4 + 4 * P["H"]),
         "band_key": n * (4 * P["H"] + 12 * B + 4),
-        "sort_hist": 8 * (8 * n * B + pair_passes * cnt + n),
-        "sort_scatter": 24 * (8 * n * B + n) + 16 * pair_passes * cnt,
-        "segment": n * B * (8 + 4 + 4 + 4 + 4 + 4 + 4 + 4),
-        "emit": 8 * cnt + 12 * n * B,
+        "sort_hist": 8 * (8 * rec + n),            # 8 key passes of the LSH sort + pack's 1 pass
+        "sort_scatter": 24 * (8 * rec + n),        # read + write (key 8 B, id 4 B) per pass
+        "scan": 12 * (rec + 2 * n),                # counts -> offsets; flag scans (read 2x, write 1x)
+        "bucket_scan": rec * (8 + 4 + 4),          # keys + ids in, S out
+        "emit": 2 * rec * (4 + 4 * sw) + 4 * rec + 4 * rec + 4 * cnt,   # 2 passes: ids + S rows; counts; offsets; partners
+        "row_sort": 4 * cnt + 4 * rec + 8 * cnt,   # partners + offsets in, pairs out
     }
     kernels = {}
     tot_prof = sum(ms for ms, _ in prof.values()) or 1.0

@@ -58,8 +58,10 @@ extern "C" {
 
 /* flags of sq_lsh_candidates */
 #define SQ_LSH_SORTED     0   /* pairs_out ascending by (i, j) (default)                      */
-#define SQ_LSH_UNORDERED  1   /* caller does not need the order (the current kernels emit
-                                 ascending (i, j) either way, at no extra cost)               */
+#define SQ_LSH_UNORDERED  1   /* caller does not need ascending j inside a row: pairs_out is
+                                 ascending in i; row i's partners come grouped by the first
+                                 band b in which the pair shares a bucket (b ascending), j
+                                 ascending inside a group.  Deterministic; skips the row merge */
 
 typedef struct sq_ctx sq_ctx;   /* opaque; owns only small host metadata + 2 pinned words */
 
@@ -160,8 +162,8 @@ const char* sq_strerror(int code);
 
 /* Built-in per-kernel timer: when enabled, every kernel launch of the context is bracketed by
  * CUDA events on the context's stream and its duration is accumulated per kernel class
- * (0 pack, 1 minhash, 2 band_key, 3 sort_hist, 4 scan, 5 sort_scatter, 6 segment, 7 emit,
- * 8 edit_distance, 9 all_pairs, 10 misc).  sq_profile_read synchronises the pending events and
+ * (0 pack, 1 minhash, 2 band_key, 3 sort_hist, 4 scan, 5 sort_scatter, 6 bucket_scan, 7 emit,
+ * 8 edit_distance, 9 all_pairs, 10 misc, 11 row_sort).  sq_profile_read synchronises the pending events and
  * returns the accumulated milliseconds and launch count of one class (host values). */
 int  sq_profile_enable(sq_ctx* ctx, int on);
 int  sq_profile_reset(sq_ctx* ctx);

@@ -78,8 +78,8 @@ int sq_profile_read(sq_ctx* c, int cls, double* ms, int64_t* launches) {
 
 const char* sq_profile_name(int cls) {
   static const char* names[SQ_K_COUNT] = {"pack", "minhash", "band_key", "sort_hist", "scan",
-                                          "sort_scatter", "segment", "emit", "edit_distance",
-                                          "all_pairs", "misc"};
+                                          "sort_scatter", "bucket_scan", "emit", "edit_distance",
+                                          "all_pairs", "misc", "row_sort"};
   return (cls >= 0 && cls < SQ_K_COUNT) ? names[cls] : nullptr;
 }
 

@@ -12,7 +12,7 @@
 // kernel classes of the built-in per-kernel timer (sq_profile_*)
 enum {
   SQ_K_PACK = 0, SQ_K_MINHASH, SQ_K_BANDKEY, SQ_K_SORT_HIST, SQ_K_SCAN, SQ_K_SORT_SCATTER,
-  SQ_K_SEGMENT, SQ_K_EMIT, SQ_K_EDIT, SQ_K_ALLPAIRS, SQ_K_MISC, SQ_K_COUNT
+  SQ_K_SEGMENT, SQ_K_EMIT, SQ_K_EDIT, SQ_K_ALLPAIRS, SQ_K_MISC, SQ_K_ROWSORT, SQ_K_COUNT
 };
 constexpr int kSqProfSlots = 1024;
 

@@ -2,26 +2,36 @@
 // de-duplicated candidate pairs (Alg. 1 step 2 "build MinHash index; generate
 // candidate list CAND"; L273 "MinHash LSH index with block-aligned storage"; spec C3).
 //
-//   a3 band_key_kernel   one thread per sequence: B 64-bit band keys + the "empty signature"
-//                        test; records (key, id) are written band-major.
-//   a4 sq_radix_sort     stable LSD radix sort of every band's records by key (ids ascend
-//                        inside a bucket because the sort is stable and ids start ascending).
-//   a5 head_flag / segment kernels: bucket boundaries of the sorted records;
-//      range_kernel      for every (sequence, band): the slice of the sorted id array holding
-//                        the kept members AFTER it in its bucket (the `cap` smallest ids of a
-//                        bucket are kept) -- an ascending run of partner ids;
-//      merge_rows_kernel one warp per sequence i, lane b = band b: warp-wide B-way merge of the
-//                        <= 32 ascending runs.  Equal heads advance together, so a pair found in
-//                        several bands is emitted once, and row i comes out ascending in j.
-//                        Pass 1 counts, a scan gives row offsets (and the total, so a too-small
-//                        output is reported before anything is written), pass 2 writes (i, j).
-//   The output is ascending in (i, j) by construction: no pair sort, no raw-pair buffer.
+//   a3 band_key_kernel     one thread per sequence: B 64-bit band keys + the "empty signature"
+//                          test; records (key, id) are written band-major.
+//   a4 sq_radix_sort       stable LSD radix sort of every band's records by key (ids ascend
+//                          inside a bucket because the sort is stable and ids start ascending).
+//   a5 bucket_scan_kernel  one pass over the sorted keys: every record learns its bucket
+//                          [head, end) (block max-/min-scans, galloping search across tile
+//                          borders), hence its rank r and whether it is KEPT (r < cap).  Writes
+//                          the bucket-id table S[id][b] (= head position if kept, else a value
+//                          unique to the sequence) and the work list: one UNIT per 32 kept rows
+//                          of a bucket that still have partners after them.
+//      emit_kernel         one warp per unit, lane = row (a kept member), sweeping the later kept
+//                          members of the bucket (columns) 32 at a time through shared memory.
+//                          Pair (row, column) of band b is NEW iff no earlier band b' < b has
+//                          S[row][b'] == S[col][b'] -- i.e. b is the first band in which both
+//                          are kept in the same bucket -- so every candidate is produced exactly
+//                          once, by one compare per earlier band (broadcast LDS.128 + 4 ISETP).
+//                          Pass 1 counts per (sequence, band); an exclusive scan turns the
+//                          counts into output offsets (and the total, so a too-small output is
+//                          reported before anything is written); pass 2 writes.
+//      row_sort_kernel     SQ_LSH_SORTED only: row i's partners arrive as <= B ascending,
+//                          pairwise-disjoint groups (one per band); every element's final rank
+//                          is the sum of its lower bounds in the groups.
+//   No raw-pair buffer and no atomics on the data path: results are deterministic.
 #include "sq_common.cuh"
 
 namespace {
 
 constexpr uint64_t kKeyInit = 0x6A09E667F3BCC908ull;
 constexpr uint64_t kKeyMult = 0x9E3779B97F4A7C15ull;
+constexpr uint32_t kFull = 0xFFFFFFFFu;
 
 __global__ void __launch_bounds__(256)
 band_key_kernel(const uint32_t* __restrict__ sig, int64_t n, int H, int bands, int rows,
@@ -49,7 +59,7 @@ band_key_kernel(const uint32_t* __restrict__ sig, int64_t n, int H, int bands, i
 // drop the records of empty signatures: record of sequence i moves to slot rank[i]
 __global__ void __launch_bounds__(256)
 compact_kernel(const uint64_t* __restrict__ keys_in, const uint32_t* __restrict__ rank,
-               const uint32_t* __restrict__ sig, int H, int64_t n, int64_t n2, int bands,
+               int64_t n, int64_t n2, int bands,
                uint64_t* __restrict__ keys_out, uint32_t* __restrict__ ids_out) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
@@ -62,176 +72,492 @@ compact_kernel(const uint64_t* __restrict__ keys_in, const uint32_t* __restrict_
   }
 }
 
-__global__ void __launch_bounds__(256)
-head_flag_kernel(const uint64_t* __restrict__ keys, int64_t n2, int64_t total,
-                 uint32_t* __restrict__ head) {
-  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (p >= total) return;
-  const bool h = (p % n2 == 0) || (keys[p] != keys[p - 1]);
-  head[p] = h ? 1u : 0u;
-}
+// ---------------------------------------------------------------------------------------------
+// a5.1  bucket scan
+// ---------------------------------------------------------------------------------------------
+constexpr int kBsThreads = 256;
+constexpr int kBsItems = 4;
+constexpr int kBsTile = kBsThreads * kBsItems;
 
-// in: excl = exclusive scan of the head flags (segment id of p = excl[p] + head - 1, and a
-// record is a head iff excl[p+1] != excl[p]).  Writes seg id in place and the head positions.
-__global__ void __launch_bounds__(256)
-segment_kernel(const uint32_t* __restrict__ excl_to_seg, int64_t total, uint32_t nseg,
-               uint32_t* __restrict__ heads_pos) {
-  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (p > total) return;
-  if (p == total) { heads_pos[nseg] = (uint32_t)total; return; }
-  const uint32_t ex = excl_to_seg[p];
-  const uint32_t nx = (p + 1 < total) ? excl_to_seg[p + 1] : nseg;
-  const bool is_head = nx != ex;
-  if (is_head) heads_pos[ex] = (uint32_t)p;
-}
-
-__global__ void __launch_bounds__(256)
-seg_fix_kernel(const uint32_t* excl, const uint32_t* __restrict__ head, int64_t total,
-               uint32_t* seg) {   // in place: excl == seg
-  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (p >= total) return;
-  seg[p] = excl[p] + head[p] - 1u;
-}
-
-// For every sorted record p (band b, sequence id): the slice of the sorted id array holding the
-// partners id can be paired with in this band -- the kept members AFTER p in p's bucket:
-// range[id][b] = (p+1, min(bucket end, bucket start + cap)) if p itself is kept, else (0,0).
-// Also accumulates the number of raw (pre-dedupe) pairs.
-__global__ void __launch_bounds__(256)
-range_kernel(const uint32_t* __restrict__ ids, const uint32_t* __restrict__ seg,
-             const uint32_t* __restrict__ heads_pos, int64_t n2, int64_t total, int bands, int cap,
-             uint2* __restrict__ range, unsigned long long* __restrict__ raw_counter) {
-  __shared__ unsigned long long raw_block;
-  if (threadIdx.x == 0) raw_block = 0ull;
-  __syncthreads();
-  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  uint32_t cnt = 0;
-  if (p < total) {
-    const int b = (int)(p / n2);
-    const uint32_t sg = seg[p];
-    const uint32_t s = heads_pos[sg], e = heads_pos[sg + 1];
-    const uint32_t ek = min(e, s + (uint32_t)cap);
-    uint2 r = make_uint2(0u, 0u);
-    if ((uint32_t)p + 1u < ek) { r = make_uint2((uint32_t)p + 1u, ek); cnt = ek - (uint32_t)p - 1u; }
-    range[(int64_t)ids[p] * bands + b] = r;
+// first position of the run of `key` that contains position `at` (keys sorted, k[at] == key)
+__device__ int64_t run_begin(const uint64_t* __restrict__ k, int64_t at, uint64_t key) {
+  int64_t hi = at, lo = -1, step = 1;
+  for (;;) {
+    const int64_t p = hi - step;
+    if (p < 0) break;
+    if (k[p] == key) { hi = p; step <<= 1; } else { lo = p; break; }
   }
-  const uint32_t wsum = __reduce_add_sync(0xFFFFFFFFu, cnt);
-  if ((threadIdx.x & 31) == 0 && wsum) atomicAdd(&raw_block, (unsigned long long)wsum);
-  __syncthreads();
-  if (threadIdx.x == 0 && raw_block) atomicAdd(raw_counter, raw_block);
+  while (hi - lo > 1) {
+    const int64_t mid = lo + (hi - lo) / 2;
+    if (k[mid] == key) hi = mid; else lo = mid;
+  }
+  return hi;
 }
 
-// Row-centric emission.  A group of G lanes (G = 16 for <= 16 bands, else 32) owns sequence i;
-// lane l of the group owns band l's partner slice (an ascending run of ids, all > i).  The union
-// of the runs is produced by a group-wide B-way merge: every step takes the minimum head (REDUX),
-// emits it once, and advances EVERY lane whose head equals it -- duplicates across bands vanish
-// and the row comes out ascending.  Each lane keeps its head plus kLook look-ahead ids in
-// registers; the load issued at an advance is consumed kLook advances later, so the serial merge
-// chain does not wait on global memory.
-// FILL = false: count the row's unique partners.  FILL = true: write (i, j) pairs at the row's
-// offset, G at a time.
-constexpr int kMergeWarps = 8;
-constexpr int kLook = 6;
+// one past the last position of the run of `key` that contains position `at`
+__device__ int64_t run_end(const uint64_t* __restrict__ k, int64_t at, uint64_t key, int64_t n) {
+  int64_t lo = at, hi = n, step = 1;
+  for (;;) {
+    const int64_t p = lo + step;
+    if (p >= n) break;
+    if (k[p] == key) { lo = p; step <<= 1; } else { hi = p; break; }
+  }
+  while (hi - lo > 1) {
+    const int64_t mid = lo + (hi - lo) / 2;
+    if (k[mid] == key) lo = mid; else hi = mid;
+  }
+  return hi;
+}
 
-template <int G, bool FILL>
-__global__ void __launch_bounds__(kMergeWarps * 32)
-merge_rows_kernel(const uint32_t* __restrict__ ids, const uint2* __restrict__ range, int64_t n,
-                  int bands, uint32_t* __restrict__ row_cnt, const uint32_t* __restrict__ row_off,
-                  uint2* __restrict__ pairs_out) {
-  constexpr int RPW = 32 / G;                        // rows per warp
-  constexpr uint32_t INF = 0xFFFFFFFFu;
+// S layout: [n][SW] uint32, SW = 4 * BW (rows are 16-byte aligned for vector loads).
+// units: (global sorted position of the unit's first row, kept members from there to the end
+// of the bucket); band 0's units go to their own list units0 (they need no compares).
+// counters: [1] raw pairs, [4] number of units of bands >= 1, [5] number of units of band 0.
+__global__ void __launch_bounds__(kBsThreads)
+bucket_scan_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict__ ids, int64_t n2,
+                   int cap, int SW, uint32_t* __restrict__ S, uint2* __restrict__ units,
+                   uint2* __restrict__ units0, unsigned long long* __restrict__ counters) {
+  __shared__ int sh_w[kBsThreads / 32];
+  __shared__ int sh_carry_head, sh_carry_end;
+  __shared__ unsigned long long sh_raw;
+  __shared__ uint32_t sh_unit_base, sh_unit_cnt;
+  const int band = blockIdx.y;
+  const uint64_t* __restrict__ k = keys + (int64_t)band * n2;
+  const uint32_t* __restrict__ idb = ids + (int64_t)band * n2;
+  const int64_t tile0 = (int64_t)blockIdx.x * kBsTile;
+  const int64_t tile_end = min(n2, tile0 + kBsTile);             // exclusive
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  const int sub = lane / G, l = lane % G;
-  const int64_t row = ((int64_t)blockIdx.x * kMergeWarps + w) * RPW + sub;
-  const bool valid = row < n;
-  uint32_t cur = 0, end = 0;                         // next id to LOAD of this lane's run
-  if (valid && l < bands) {
-    const uint2 r = range[row * bands + l];
-    cur = r.x; end = r.y;
+  const int64_t p0 = tile0 + (int64_t)threadIdx.x * kBsItems;
+  if (threadIdx.x == 0) { sh_raw = 0ull; sh_unit_cnt = 0u; }
+
+  uint64_t kk[kBsItems];
+  bool valid[kBsItems], head[kBsItems], tail[kBsItems];
+  uint64_t prev = 0, next = 0;
+  bool has_prev = p0 > 0 && p0 < n2, has_next = false;
+  if (has_prev) prev = k[p0 - 1];
+#pragma unroll
+  for (int t = 0; t < kBsItems; ++t) {
+    valid[t] = p0 + t < n2;
+    kk[t] = valid[t] ? k[p0 + t] : 0ull;
   }
-  if (FILL && valid && row_cnt[row] == 0) end = cur;
-  if (__ballot_sync(0xFFFFFFFFu, cur < end) == 0) {
-    if (!FILL && valid && l == 0) row_cnt[row] = 0;
+  if (p0 + kBsItems < n2) { has_next = true; next = k[p0 + kBsItems]; }
+#pragma unroll
+  for (int t = 0; t < kBsItems; ++t) {
+    const bool hp = t == 0 ? (!has_prev || kk[0] != prev) : (kk[t] != kk[t - 1]);
+    bool tl;
+    if (t == kBsItems - 1) tl = !has_next || kk[t] != next;
+    else tl = !valid[t + 1] || kk[t] != kk[t + 1];
+    head[t] = valid[t] && hp;
+    tail[t] = valid[t] && tl;
+  }
+  // the two tile-border searches (done by one thread each, overlapped with the scans below)
+  if (threadIdx.x == 0)
+    sh_carry_head = head[0] ? (int)tile0 : (int)run_begin(k, tile0, kk[0]);
+#pragma unroll
+  for (int t = 0; t < kBsItems; ++t)
+    if (p0 + t == tile_end - 1)                                  // thread owning the last record
+      sh_carry_end = tail[t] ? (int)tile_end : (int)run_end(k, tile_end - 1, kk[t], n2);
+  // forward max-scan of head positions
+  int hpos[kBsItems];
+  int run = -1;
+#pragma unroll
+  for (int t = 0; t < kBsItems; ++t) { if (head[t]) run = (int)(p0 + t); hpos[t] = run; }
+  int inc = run;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const int o = __shfl_up_sync(kFull, inc, d);
+    if (lane >= d) inc = max(inc, o);
+  }
+  if (lane == 31) sh_w[w] = inc;
+  __syncthreads();
+  int ex = __shfl_up_sync(kFull, inc, 1);
+  if (lane == 0) ex = -1;
+  for (int q = 0; q < w; ++q) ex = max(ex, sh_w[q]);
+  if (ex < 0) ex = sh_carry_head;
+#pragma unroll
+  for (int t = 0; t < kBsItems; ++t) if (hpos[t] < 0) hpos[t] = ex;
+  __syncthreads();
+  // backward min-scan of end positions
+  int epos[kBsItems];
+  constexpr int kInf = 0x7FFFFFFF;
+  run = kInf;
+#pragma unroll
+  for (int t = kBsItems - 1; t >= 0; --t) { if (tail[t]) run = (int)(p0 + t + 1); epos[t] = run; }
+  inc = run;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const int o = __shfl_down_sync(kFull, inc, d);
+    if (lane + d < 32) inc = min(inc, o);
+  }
+  if (lane == 0) sh_w[w] = inc;
+  __syncthreads();
+  int ee = __shfl_down_sync(kFull, inc, 1);
+  if (lane == 31) ee = kInf;
+  for (int q = w + 1; q < kBsThreads / 32; ++q) ee = min(ee, sh_w[q]);
+  if (ee == kInf) ee = sh_carry_end;
+#pragma unroll
+  for (int t = 0; t < kBsItems; ++t) if (epos[t] == kInf) epos[t] = ee;
+
+  // per record: rank, kept, S entry, unit, raw pairs
+  unsigned long long raw = 0;
+  uint32_t nunit = 0;
+  uint2 unit[kBsItems];
+  bool has_unit[kBsItems];
+#pragma unroll
+  for (int t = 0; t < kBsItems; ++t) {
+    has_unit[t] = false;
+    if (!valid[t]) continue;
+    const uint32_t id = idb[p0 + t];
+    const int r = (int)(p0 + t) - hpos[t];
+    const int size = epos[t] - hpos[t];
+    const int m = min(size, cap);
+    const bool kept = r < m;
+    S[(int64_t)id * SW + band] = kept ? (uint32_t)hpos[t] : (0x80000000u | id);
+    if (kept) {
+      raw += (unsigned long long)(m - 1 - r);
+      if ((r & 31) == 0 && r + 1 < m) {
+        has_unit[t] = true;
+        ++nunit;
+        unit[t] = make_uint2((uint32_t)((int64_t)band * n2 + p0 + t), (uint32_t)(m - r));
+      }
+    }
+  }
+  // append the units (order across blocks is irrelevant: output positions never depend on it)
+  uint32_t my = 0;
+  if (nunit) my = atomicAdd(&sh_unit_cnt, nunit);
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) raw += __shfl_xor_sync(kFull, raw, d);
+  if (lane == 0 && raw) atomicAdd(&sh_raw, raw);
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    if (sh_unit_cnt)
+      sh_unit_base = (uint32_t)atomicAdd(counters + (band == 0 ? 5 : 4), (unsigned long long)sh_unit_cnt);
+    if (sh_raw) atomicAdd(counters + 1, sh_raw);
+  }
+  __syncthreads();
+  uint2* __restrict__ ulist = band == 0 ? units0 : units;
+  uint32_t q = sh_unit_base + my;
+#pragma unroll
+  for (int t = 0; t < kBsItems; ++t) if (has_unit[t]) ulist[q++] = unit[t];
+}
+
+// ---------------------------------------------------------------------------------------------
+// a5.2  emission: lane = row, columns swept through shared memory
+// ---------------------------------------------------------------------------------------------
+constexpr int kEmWarps = 4;
+enum { EM_COUNT = 0, EM_FILL_J = 1, EM_FILL_PAIRS = 2 };
+
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
+  const uint32_t s = (uint32_t)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
+
+// Band 0: every pair of kept members is new.  One warp per unit.
+template <int MODE>
+__global__ void __launch_bounds__(kEmWarps * 32)
+emit_band0_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint32_t* __restrict__ ids,
+                  int bands, uint32_t* __restrict__ cnt_off, uint32_t* __restrict__ outJ,
+                  uint2* __restrict__ outP) {
+  const int lane = threadIdx.x & 31;
+  const uint32_t u = blockIdx.x * kEmWarps + (threadIdx.x >> 5);
+  if (u >= nunits) return;
+  const uint2 unit = units[u];
+  const uint32_t mrem = unit.y;
+  const uint32_t* __restrict__ idp = ids + unit.x;
+  const uint32_t nrows = min(32u, mrem - 1u);
+  const bool rowok = (uint32_t)lane < nrows;
+  const uint32_t myid = rowok ? idp[lane] : 0u;
+  if (MODE == EM_COUNT) {
+    if (rowok) cnt_off[(int64_t)myid * bands] = mrem - 1u - (uint32_t)lane;
     return;
   }
-  uint32_t q[kLook + 1];                             // q[0] = head, q[1..] = look-ahead
-#pragma unroll
-  for (int t = 0; t <= kLook; ++t) { q[t] = cur < end ? ids[cur] : INF; ++cur; }
-  uint32_t c = 0, out = 0;
-  const uint32_t base = (FILL && valid) ? row_off[row] : 0u;
-  for (;;) {
-    uint32_t m;
-    if (RPW == 1) {
-      m = __reduce_min_sync(0xFFFFFFFFu, q[0]);
-      if (m == INF) break;
-    } else {
-      const uint32_t m0 = __reduce_min_sync(0xFFFFFFFFu, sub == 0 ? q[0] : INF);
-      const uint32_t m1 = __reduce_min_sync(0xFFFFFFFFu, sub == 1 ? q[0] : INF);
-      if ((m0 & m1) == INF) break;
-      m = sub == 0 ? m0 : m1;
+  const uint32_t off = rowok ? cnt_off[(int64_t)myid * bands] : 0u;
+  for (uint32_t l = 0; l < nrows; ++l) {     // coalesced: the warp writes row l's partners
+    const uint32_t o = __shfl_sync(kFull, off, l), i = __shfl_sync(kFull, myid, l);
+    for (uint32_t cc = l + 1 + lane; cc < mrem; cc += 32) {
+      const uint32_t j = idp[cc];
+      if (MODE == EM_FILL_J) outJ[o + cc - l - 1] = j;
+      else outP[o + cc - l - 1] = make_uint2(i, j);
     }
-    const bool live = m != INF;
-    if (FILL && live) {
-      if (l == (int)(c & (G - 1))) out = m;
-      if ((c & (G - 1)) == G - 1)
-        pairs_out[base + (c & ~(uint32_t)(G - 1)) + l] = make_uint2((uint32_t)row, out);
-    }
-    c += live ? 1u : 0u;
-    if (live && q[0] == m) {
-#pragma unroll
-      for (int t = 0; t < kLook; ++t) q[t] = q[t + 1];
-      q[kLook] = cur < end ? ids[cur] : INF;
-      ++cur;
-    }
-  }
-  if (FILL) {
-    if (valid && l < (int)(c & (G - 1)))
-      pairs_out[base + (c & ~(uint32_t)(G - 1)) + l] = make_uint2((uint32_t)row, out);
-  } else {
-    if (valid && l == 0) row_cnt[row] = c;
   }
 }
 
-template <bool FILL>
-int launch_merge(sq_ctx* c, const uint32_t* ids, const uint2* range, int64_t n, int bands,
-                 uint32_t* row_cnt, const uint32_t* row_off, uint2* pairs_out) {
-  if (bands <= 16) {
-    const int64_t rows_per_block = kMergeWarps * 2;
-    const unsigned g = (unsigned)((n + rows_per_block - 1) / rows_per_block);
-    SQ_TIMED(c, SQ_K_EMIT, merge_rows_kernel<16, FILL><<<g, kMergeWarps * 32, 0, c->stream>>>(
-        ids, range, n, bands, row_cnt, row_off, pairs_out));
-  } else {
-    const unsigned g = (unsigned)((n + kMergeWarps - 1) / kMergeWarps);
-    SQ_TIMED(c, SQ_K_EMIT, merge_rows_kernel<32, FILL><<<g, kMergeWarps * 32, 0, c->stream>>>(
-        ids, range, n, bands, row_cnt, row_off, pairs_out));
+// One column tile against the warp's 32 rows: NCH chunks of 4 earlier bands are compared.
+template <int BW, int NCH, int MODE>
+__device__ __forceinline__ void sweep_tile(const uint32_t* __restrict__ sm,
+                                           const uint32_t* __restrict__ idt, const uint4 (&R)[BW],
+                                           uint32_t cbeg, uint32_t ncol, uint32_t c0, uint32_t lane,
+                                           bool rowok, uint32_t myid, uint32_t& acc,
+                                           uint32_t* __restrict__ outJ, uint2* __restrict__ outP) {
+  constexpr int RS = 4 * BW + 4;
+  if constexpr (NCH <= BW) {
+#pragma unroll 4
+    for (uint32_t c = cbeg; c < ncol; ++c) {
+      bool dup = false;
+#pragma unroll
+      for (int ch = 0; ch < NCH; ++ch) {
+        const uint4 v = *reinterpret_cast<const uint4*>(sm + c * RS + 4 * ch);   // broadcast
+        dup |= (v.x == R[ch].x) | (v.y == R[ch].y) | (v.z == R[ch].z) | (v.w == R[ch].w);
+      }
+      const bool isnew = !dup && rowok && (c0 + c > lane);
+      if (MODE == EM_COUNT) {
+        acc += isnew ? 1u : 0u;
+      } else if (isnew) {
+        const uint32_t j = idt[c];
+        if (MODE == EM_FILL_J) outJ[acc] = j; else outP[acc] = make_uint2(myid, j);
+        ++acc;
+      }
+    }
   }
+}
+
+struct EmDesc { uint32_t u, g0, mrem, c0; int b; bool ok; };
+
+// Bands >= 1.  Persistent warps stride over the unit list; the stream of (unit, column tile)
+// items is software-pipelined: ids two tiles ahead (registers), S rows one tile ahead
+// (cp.async into the other shared-memory buffer), compares on the current tile.
+// BW = 16-byte chunks per S row (S row width SW = 4*BW >= bands).
+// MODE EM_COUNT:      cnt[id*bands + b] = number of NEW partners of row id in band b.
+// MODE EM_FILL_J:     outJ[off[id*bands + b] + t] = t-th new partner (ascending).
+// MODE EM_FILL_PAIRS: outP[...] = (id, partner).
+template <int BW, int MODE>
+__global__ void __launch_bounds__(kEmWarps * 32)
+emit_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint32_t* __restrict__ ids,
+            uint32_t n2, int bands, const uint32_t* __restrict__ S, uint32_t* __restrict__ cnt_off,
+            uint32_t* __restrict__ outJ, uint2* __restrict__ outP) {
+  constexpr int SW = 4 * BW;
+  constexpr int RS = SW + 4;                 // shared row stride in words (16-byte aligned)
+  constexpr int RPR = 32 / BW;               // S rows fetched per load round
+  __shared__ __align__(16) uint32_t Sm[kEmWarps][2][32 * RS];
+  __shared__ uint32_t idsm[kEmWarps][2][32];
+  const uint32_t lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const uint32_t nw = gridDim.x * kEmWarps;
+  const uint32_t wg = blockIdx.x * kEmWarps + w;
+  if (wg >= nunits) return;
+  uint2 unit_pref = units[wg];               // always the next unit this warp will open
+
+  auto next_desc = [&](EmDesc d) -> EmDesc {
+    if (d.ok && d.c0 + 32 < d.mrem) { d.c0 += 32; return d; }
+    EmDesc r;
+    r.u = d.u + nw;
+    r.ok = d.ok && r.u < nunits;
+    r.g0 = unit_pref.x; r.mrem = unit_pref.y; r.c0 = 0;
+    r.b = (int)(r.g0 / n2);
+    if (r.ok && r.u + nw < nunits) unit_pref = units[r.u + nw];
+    return r;
+  };
+  auto load_ids = [&](const EmDesc& d) -> uint32_t {
+    return (d.ok && d.c0 + lane < d.mrem) ? ids[(int64_t)d.g0 + d.c0 + lane] : 0u;
+  };
+  auto issue_rows = [&](const EmDesc& d, uint32_t idc, uint32_t* sm) {
+    const uint32_t ncol = min(32u, d.mrem - d.c0);
+    const int nch = (d.b + 3) >> 2;
+#pragma unroll
+    for (int it = 0; it < BW; ++it) {
+      const uint32_t rr = it * RPR + lane / BW;
+      const int ch = lane % BW;
+      const uint32_t rid = __shfl_sync(kFull, idc, rr);
+      if (ch < nch && rr < ncol) cp_async16(sm + rr * RS + 4 * ch, S + (int64_t)rid * SW + 4 * ch);
+    }
+  };
+
+  EmDesc dc;                                  // current tile
+  dc.u = wg - nw; dc.ok = true; dc.mrem = 0; dc.c0 = 0; dc.g0 = 0; dc.b = 0;
+  dc = next_desc(dc);
+  uint32_t idc_c = load_ids(dc);
+  EmDesc dn = next_desc(dc);                  // next tile
+  uint32_t idc_n = load_ids(dn);
+  issue_rows(dc, idc_c, Sm[w][0]);
+  cp_async_commit();
+
+  uint4 R[BW];
+  uint32_t acc = 0, myid = 0;
+  bool rowok = false;
+  int k = 0;
+  while (dc.ok) {
+    if (dn.ok) issue_rows(dn, idc_n, Sm[w][(k + 1) & 1]);
+    cp_async_commit();
+    const EmDesc d2 = next_desc(dn);
+    const uint32_t id2 = load_ids(d2);
+    cp_async_wait<1>();
+    __syncwarp();
+    const uint32_t* sm = Sm[w][k & 1];
+    const int b = dc.b;
+    if (dc.c0 == 0) {                         // a unit starts: its rows are the first 32 columns
+      myid = idc_c;
+      rowok = lane < min(32u, dc.mrem - 1u);
+      acc = 0;
+      if (MODE != EM_COUNT && rowok) acc = cnt_off[(int64_t)myid * bands + b];
+#pragma unroll
+      for (int ch = 0; ch < BW; ++ch) {
+        if (4 * ch < b) {
+          uint4 v = *reinterpret_cast<const uint4*>(sm + lane * RS + 4 * ch);
+          if (4 * ch + 1 >= b) v.y = kFull;   // bands >= b never match (no S value is 0xFFFFFFFF)
+          if (4 * ch + 2 >= b) v.z = kFull;
+          if (4 * ch + 3 >= b) v.w = kFull;
+          R[ch] = v;
+        }
+      }
+    }
+    if (MODE != EM_COUNT) { idsm[w][k & 1][lane] = idc_c; __syncwarp(); }
+    const uint32_t ncol = min(32u, dc.mrem - dc.c0);
+    const uint32_t cbeg = dc.c0 == 0 ? 1u : 0u;
+    const uint32_t* idt = idsm[w][k & 1];
+    switch ((b + 3) >> 2) {
+      case 1: sweep_tile<BW, 1, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, outJ, outP); break;
+      case 2: sweep_tile<BW, 2, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, outJ, outP); break;
+      case 3: sweep_tile<BW, 3, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, outJ, outP); break;
+      case 4: sweep_tile<BW, 4, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, outJ, outP); break;
+      case 5: sweep_tile<BW, 5, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, outJ, outP); break;
+      case 6: sweep_tile<BW, 6, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, outJ, outP); break;
+      case 7: sweep_tile<BW, 7, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, outJ, outP); break;
+      default: sweep_tile<BW, 8, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, outJ, outP); break;
+    }
+    if (MODE == EM_COUNT && rowok && dc.c0 + 32 >= dc.mrem)
+      cnt_off[(int64_t)myid * bands + b] = acc;
+    __syncwarp();
+    dc = dn; idc_c = idc_n; dn = d2; idc_n = id2; ++k;
+  }
+  cp_async_wait<0>();
+}
+
+// ---------------------------------------------------------------------------------------------
+// a5.3  SQ_LSH_SORTED: merge the <= B ascending, disjoint groups of every row
+// ---------------------------------------------------------------------------------------------
+constexpr int kRsWarps = 8;
+
+__global__ void __launch_bounds__(kRsWarps * 32)
+row_sort_kernel(const uint32_t* __restrict__ off, int64_t n, int bands, uint32_t total,
+                const uint32_t* __restrict__ inJ, uint2* __restrict__ out) {
+  const int lane = threadIdx.x & 31;
+  const int64_t i = (int64_t)blockIdx.x * kRsWarps + (threadIdx.x >> 5);
+  if (i >= n) return;
+  // lane b holds the start of group b; lane `bands` (or the shuffle below) gives the row end
+  const uint32_t row_end = (i + 1 < n) ? off[(i + 1) * bands] : total;
+  const uint32_t gs = lane < bands ? off[i * bands + lane] : row_end;
+  uint32_t ge = __shfl_down_sync(kFull, gs, 1);
+  if (lane == 31 || lane + 1 >= bands) ge = row_end;
+  const uint32_t base = __shfl_sync(kFull, gs, 0);
+  const uint32_t T = row_end - base;
+  if (T == 0) return;
+  const uint32_t nonempty = __ballot_sync(kFull, lane < bands && ge > gs);
+  if (__popc(nonempty) == 1) {               // already ascending
+    for (uint32_t t = lane; t < T; t += 32) out[base + t] = make_uint2((uint32_t)i, inJ[base + t]);
+    return;
+  }
+  for (uint32_t t0 = 0; t0 < T; t0 += 32) {
+    const uint32_t t = t0 + lane;
+    const uint32_t x = t < T ? inJ[base + t] : 0u;
+    uint32_t rank = 0;
+    for (uint32_t gm = nonempty; gm; gm &= gm - 1) {
+      const int g = __ffs(gm) - 1;
+      uint32_t lo = __shfl_sync(kFull, gs, g);
+      uint32_t len = __shfl_sync(kFull, ge, g) - lo;
+      const uint32_t first = lo;
+      while (len > 0) {                      // lower bound of x in group g (uniform trip count)
+        const uint32_t half = len >> 1;
+        const bool less = inJ[lo + half] < x;
+        lo = less ? lo + half + 1 : lo;
+        len = less ? len - half - 1 : half;
+      }
+      rank += lo - first;
+    }
+    if (t < T) out[base + rank] = make_uint2((uint32_t)i, x);
+  }
+}
+
+template <int BW>
+int launch_emit(sq_ctx* c, int mode, const uint2* units, uint32_t nunits, const uint32_t* ids,
+                uint32_t n2, int bands, const uint32_t* S, uint32_t* cnt_off, uint32_t* outJ,
+                uint2* outP) {
+  // persistent warps: exactly the resident blocks of every SM, never more warps than units
+  int per_sm = 0;
+  cudaError_t e;
+  if (mode == EM_COUNT)
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, emit_kernel<BW, EM_COUNT>, kEmWarps * 32, 0);
+  else if (mode == EM_FILL_J)
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, emit_kernel<BW, EM_FILL_J>, kEmWarps * 32, 0);
+  else
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, emit_kernel<BW, EM_FILL_PAIRS>, kEmWarps * 32, 0);
+  if (e != cudaSuccess || per_sm < 1) per_sm = 4;
+  unsigned g = (unsigned)(c->sm_count * per_sm);
+  const unsigned need = (nunits + kEmWarps - 1) / kEmWarps;
+  if (g > need) g = need;
+  if (mode == EM_COUNT)
+    SQ_TIMED(c, SQ_K_EMIT, emit_kernel<BW, EM_COUNT><<<g, kEmWarps * 32, 0, c->stream>>>(
+        units, nunits, ids, n2, bands, S, cnt_off, outJ, outP));
+  else if (mode == EM_FILL_J)
+    SQ_TIMED(c, SQ_K_EMIT, emit_kernel<BW, EM_FILL_J><<<g, kEmWarps * 32, 0, c->stream>>>(
+        units, nunits, ids, n2, bands, S, cnt_off, outJ, outP));
+  else
+    SQ_TIMED(c, SQ_K_EMIT, emit_kernel<BW, EM_FILL_PAIRS><<<g, kEmWarps * 32, 0, c->stream>>>(
+        units, nunits, ids, n2, bands, S, cnt_off, outJ, outP));
   SQ_LAUNCH_CHECK(c);
   return SQ_OK;
 }
 
+int launch_emit_band0(sq_ctx* c, int mode, const uint2* units0, uint32_t nunits0,
+                      const uint32_t* ids, int bands, uint32_t* cnt_off, uint32_t* outJ,
+                      uint2* outP) {
+  const unsigned g = (nunits0 + kEmWarps - 1) / kEmWarps;
+  if (mode == EM_COUNT)
+    SQ_TIMED(c, SQ_K_EMIT, emit_band0_kernel<EM_COUNT><<<g, kEmWarps * 32, 0, c->stream>>>(
+        units0, nunits0, ids, bands, cnt_off, outJ, outP));
+  else if (mode == EM_FILL_J)
+    SQ_TIMED(c, SQ_K_EMIT, emit_band0_kernel<EM_FILL_J><<<g, kEmWarps * 32, 0, c->stream>>>(
+        units0, nunits0, ids, bands, cnt_off, outJ, outP));
+  else
+    SQ_TIMED(c, SQ_K_EMIT, emit_band0_kernel<EM_FILL_PAIRS><<<g, kEmWarps * 32, 0, c->stream>>>(
+        units0, nunits0, ids, bands, cnt_off, outJ, outP));
+  SQ_LAUNCH_CHECK(c);
+  return SQ_OK;
+}
+
+// both unit lists, one mode
+int dispatch_emit(sq_ctx* c, int bw, int mode, const uint2* units, uint32_t nunits,
+                  const uint2* units0, uint32_t nunits0, const uint32_t* ids, uint32_t n2, int bands,
+                  const uint32_t* S, uint32_t* cnt_off, uint32_t* outJ, uint2* outP) {
+  int rc = SQ_OK;
+  if (nunits0) rc = launch_emit_band0(c, mode, units0, nunits0, ids, bands, cnt_off, outJ, outP);
+  if (rc != SQ_OK || nunits == 0) return rc;
+  switch (bw) {
+    case 1: return launch_emit<1>(c, mode, units, nunits, ids, n2, bands, S, cnt_off, outJ, outP);
+    case 2: return launch_emit<2>(c, mode, units, nunits, ids, n2, bands, S, cnt_off, outJ, outP);
+    case 4: return launch_emit<4>(c, mode, units, nunits, ids, n2, bands, S, cnt_off, outJ, outP);
+    default: return launch_emit<8>(c, mode, units, nunits, ids, n2, bands, S, cnt_off, outJ, outP);
+  }
+}
+
+inline int chunks_for(int bands) { return bands <= 4 ? 1 : bands <= 8 ? 2 : bands <= 16 ? 4 : 8; }
+
 }  // namespace
 
-size_t sq_lsh_scratch_bytes(int64_t n, int bands, int64_t /*pair_capacity*/) {
-  size_t nn = (size_t)(n > 0 ? n : 1), B = (size_t)(bands > 0 ? bands : 1);
-  size_t rec = nn * B;
+size_t sq_lsh_scratch_bytes(int64_t n, int bands, int64_t pair_capacity) {
+  const size_t nn = (size_t)(n > 0 ? n : 1), B = (size_t)(bands > 0 ? bands : 1);
+  const size_t rec = nn * B;
+  const size_t sw = 4 * (size_t)chunks_for((int)B);
   size_t s = 0;
-  s += 2 * sq_align_up(rec * 8 + 16);          // keys ping-pong (the range table reuses one)
+  s += 2 * sq_align_up(rec * 8 + 16);          // keys ping-pong (the unit list reuses one)
   s += 2 * sq_align_up(rec * 4 + 16);          // ids ping-pong
-  s += 3 * sq_align_up((rec + 2) * 4 + 16);    // head flags, scan / seg ids, head positions
-  s += 2 * sq_align_up((nn + 2) * 4 + 16);     // non-empty flags / ranks; row counts / offsets
+  s += sq_align_up(nn * sw * 4 + 16);          // bucket-id table S
+  s += sq_align_up((rec + 2) * 4 + 16);        // per (sequence, band) counts -> offsets
+  s += sq_align_up((nn + 2) * 4 + 16);         // non-empty flags / ranks
   s += sq_sort_scratch_bytes(n, bands);
+  s += sq_align_up((size_t)(pair_capacity > 0 ? pair_capacity : 0) * 4 + 16);   // SORTED: partners
   return s + 4096;
 }
 
 extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int bands, int rows,
                                  int bucket_cap, int flags, uint32_t* pairs_out, int64_t capacity,
                                  int64_t* n_pairs) {
-  (void)flags;   // the row-centric merge always produces ascending (i, j)
   if (!c || !n_pairs) return SQ_ERR_INVALID_ARG;
   *n_pairs = 0;
   if (c->n < 0) return SQ_ERR_NOT_PACKED;
   if (H < 1 || bands < 1 || rows < 1 || bucket_cap < 1 || capacity < 0 ||
-      (int64_t)bands * rows > H)
+      (int64_t)bands * rows > H || (flags != SQ_LSH_SORTED && flags != SQ_LSH_UNORDERED))
     return SQ_ERR_INVALID_ARG;
   if (bands > SQ_MAX_BANDS || H > SQ_MAX_H) return SQ_ERR_UNSUPPORTED;
   const int64_t n = c->n;
@@ -242,20 +568,18 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
 
   sq_scratch_reset(c);
   const size_t rec = (size_t)n * bands;
+  const int bw = chunks_for(bands), sw = 4 * bw;
   uint64_t* k0 = sq_scratch<uint64_t>(c, rec);
   uint64_t* k1 = sq_scratch<uint64_t>(c, rec);
   uint32_t* v0 = sq_scratch<uint32_t>(c, rec);
   uint32_t* v1 = sq_scratch<uint32_t>(c, rec);
-  uint32_t* head = sq_scratch<uint32_t>(c, rec + 2);
-  uint32_t* seg = sq_scratch<uint32_t>(c, rec + 2);
-  uint32_t* heads_pos = sq_scratch<uint32_t>(c, rec + 2);
+  uint32_t* S = sq_scratch<uint32_t>(c, (size_t)n * sw);
+  uint32_t* cnt = sq_scratch<uint32_t>(c, rec + 2);
   uint32_t* nonempty = sq_scratch<uint32_t>(c, (size_t)n + 2);
-  uint32_t* row_cnt = sq_scratch<uint32_t>(c, (size_t)n + 2);
   uint8_t* tmp = sq_scratch<uint8_t>(c, sq_sort_scratch_bytes(n, bands));
-  if (!k0 || !k1 || !v0 || !v1 || !head || !seg || !heads_pos || !nonempty || !row_cnt || !tmp)
-    return SQ_ERR_WORKSPACE;
+  if (!k0 || !k1 || !v0 || !v1 || !S || !cnt || !nonempty || !tmp) return SQ_ERR_WORKSPACE;
   cudaStream_t st = c->stream;
-  unsigned long long* counters = c->dflags;      // [0] unique, [1] raw, [2] n2, [3] nseg
+  unsigned long long* counters = c->dflags;      // [0] unique, [1] raw, [2] n2, [4] units
   SQ_CUDA(c, cudaMemsetAsync(counters, 0, 64, st));
 
   // a3: band keys + non-empty flags
@@ -271,7 +595,7 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
   if (n2 < 2) return SQ_OK;                       // fewer than two usable signatures: no pairs
   uint64_t* kin = k0; uint64_t* kalt = k1; uint32_t* vin = v0; uint32_t* valt = v1;
   if (n2 != n) {
-    SQ_TIMED(c, SQ_K_BANDKEY, compact_kernel<<<gb, 256, 0, st>>>(k0, nonempty, sig, H, n, n2, bands, k1, v1));
+    SQ_TIMED(c, SQ_K_BANDKEY, compact_kernel<<<gb, 256, 0, st>>>(k0, nonempty, n, n2, bands, k1, v1));
     SQ_LAUNCH_CHECK(c);
     kin = k1; kalt = k0; vin = v1; valt = v0;
   }
@@ -284,44 +608,47 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
     if (rc != SQ_OK) return rc;
     if (in_alt) { uint64_t* t = kin; kin = kalt; kalt = t; uint32_t* tv = vin; vin = valt; valt = tv; }
   }
-  // a5: buckets -> per (sequence, band) partner slices
-  const int64_t total = n2 * bands;
-  const unsigned gt = (unsigned)((total + 255) / 256);
-  SQ_TIMED(c, SQ_K_SEGMENT, head_flag_kernel<<<gt, 256, 0, st>>>(kin, n2, total, head));
-  SQ_LAUNCH_CHECK(c);
-  rc = sq_exclusive_scan_u32(c, head, seg, total, reinterpret_cast<uint32_t*>(tmp), counters + 3);
-  if (rc != SQ_OK) return rc;
-  SQ_CUDA(c, cudaMemcpyAsync(c->pinned, counters + 3, 8, cudaMemcpyDeviceToHost, st));
+  // a5.1: buckets -> S table + unit list (the unit list lives in the dead key buffer)
+  uint2* units = reinterpret_cast<uint2*>(kalt);
+  uint2* units0 = units + rec / 2 + 1;           // <= n2/2 units of band 0, <= rec/2 in all
+  SQ_CUDA(c, cudaMemsetAsync(cnt, 0, (rec + 2) * 4, st));
+  {
+    dim3 grid((unsigned)((n2 + kBsTile - 1) / kBsTile), (unsigned)bands);
+    SQ_TIMED(c, SQ_K_SEGMENT, bucket_scan_kernel<<<grid, kBsThreads, 0, st>>>(
+        kin, vin, n2, bucket_cap, sw, S, units, units0, counters));
+    SQ_LAUNCH_CHECK(c);
+  }
+  SQ_CUDA(c, cudaMemcpyAsync(c->pinned, counters, 48, cudaMemcpyDeviceToHost, st));
   SQ_CUDA(c, cudaStreamSynchronize(st));
-  const uint32_t nseg = (uint32_t)c->pinned[0];
-  SQ_TIMED(c, SQ_K_SEGMENT, segment_kernel<<<(unsigned)((total + 256) / 256), 256, 0, st>>>(seg, total, nseg, heads_pos));
-  SQ_LAUNCH_CHECK(c);
-  SQ_TIMED(c, SQ_K_SEGMENT, seg_fix_kernel<<<gt, 256, 0, st>>>(seg, head, total, seg));
-  SQ_LAUNCH_CHECK(c);
-  // the sorted keys are dead now: their buffer becomes the [n][bands] range table (8 B / entry)
-  uint2* range = reinterpret_cast<uint2*>(kalt);
-  SQ_CUDA(c, cudaMemsetAsync(range, 0, rec * 8, st));
-  SQ_TIMED(c, SQ_K_SEGMENT, range_kernel<<<gt, 256, 0, st>>>(vin, seg, heads_pos, n2, total, bands,
-                                                             bucket_cap, range, counters + 1));
-  SQ_LAUNCH_CHECK(c);
-  // a5: row-centric merge, pass 1 = count, scan, pass 2 = fill
-  rc = launch_merge<false>(c, vin, range, n, bands, row_cnt, nullptr, nullptr);
+  c->last_raw_pairs = (int64_t)c->pinned[1];
+  const uint32_t nunits = (uint32_t)c->pinned[4], nunits0 = (uint32_t)c->pinned[5];
+  if (nunits + nunits0 == 0) return SQ_OK;
+  // a5.2 pass 1: counts per (sequence, band) -> offsets
+  rc = dispatch_emit(c, bw, EM_COUNT, units, nunits, units0, nunits0, vin, (uint32_t)n2, bands, S, cnt, nullptr, nullptr);
   if (rc != SQ_OK) return rc;
-  uint32_t* row_off = nonempty;                  // ranks are dead: reuse for the row offsets
-  rc = sq_exclusive_scan_u32(c, row_cnt, row_off, n, reinterpret_cast<uint32_t*>(tmp), counters);
+  rc = sq_exclusive_scan_u32(c, cnt, cnt, (int64_t)rec, reinterpret_cast<uint32_t*>(tmp), counters);
   if (rc != SQ_OK) return rc;
-  SQ_CUDA(c, cudaMemcpyAsync(c->pinned, counters, 16, cudaMemcpyDeviceToHost, st));
+  SQ_CUDA(c, cudaMemcpyAsync(c->pinned, counters, 8, cudaMemcpyDeviceToHost, st));
   SQ_CUDA(c, cudaStreamSynchronize(st));
   const int64_t uniq = (int64_t)c->pinned[0];
-  c->last_raw_pairs = (int64_t)c->pinned[1];
   *n_pairs = uniq;
   if (uniq > capacity) return SQ_ERR_CAPACITY;
-  if (uniq >= (1ll << 32) - 1) return SQ_ERR_UNSUPPORTED;   // 32-bit row offsets
-  if (uniq > 0) {
-    rc = launch_merge<true>(c, vin, range, n, bands, row_cnt, row_off,
-                            reinterpret_cast<uint2*>(pairs_out));
+  if (uniq >= (1ll << 32) - 1) return SQ_ERR_UNSUPPORTED;   // 32-bit output offsets
+  if (uniq == 0) return SQ_OK;
+  // a5.2 pass 2 (+ a5.3)
+  uint2* out = reinterpret_cast<uint2*>(pairs_out);
+  if (flags == SQ_LSH_UNORDERED) {
+    rc = dispatch_emit(c, bw, EM_FILL_PAIRS, units, nunits, units0, nunits0, vin, (uint32_t)n2, bands, S, cnt, nullptr, out);
     if (rc != SQ_OK) return rc;
-    SQ_CUDA(c, cudaStreamSynchronize(st));
+  } else {
+    uint32_t* tmpJ = sq_scratch<uint32_t>(c, (size_t)uniq);
+    if (!tmpJ) return SQ_ERR_WORKSPACE;
+    rc = dispatch_emit(c, bw, EM_FILL_J, units, nunits, units0, nunits0, vin, (uint32_t)n2, bands, S, cnt, tmpJ, nullptr);
+    if (rc != SQ_OK) return rc;
+    SQ_TIMED(c, SQ_K_ROWSORT, row_sort_kernel<<<(unsigned)((n + kRsWarps - 1) / kRsWarps), kRsWarps * 32, 0, st>>>(
+        cnt, n, bands, (uint32_t)uniq, tmpJ, out));
+    SQ_LAUNCH_CHECK(c);
   }
+  SQ_CUDA(c, cudaStreamSynchronize(st));
   return SQ_OK;
 }

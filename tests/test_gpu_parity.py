@@ -137,6 +137,16 @@ def test_lsh_unordered_is_the_same_set_and_capacity_protocol():
     key = np.sort(pairs[:, 0].astype(np.int64) << 32 | pairs[:, 1])
     wkey = want_pairs[:, 0].astype(np.int64) << 32 | want_pairs[:, 1]
     assert np.array_equal(key, wkey)
+    # the documented order of SQ_LSH_UNORDERED: i ascending; inside a row, grouped by the first
+    # band in which the pair shares a bucket, j ascending inside a group.  The cap (512) does not
+    # bind here (largest bucket of this input < 512), so "shares a bucket" == equal band tuples.
+    B, r = P["bands"], P["rows"]
+    tup = want_sig[:, :B * r].reshape(rep.n, B, r)
+    eq = (tup[pairs[:, 0]] == tup[pairs[:, 1]]).all(axis=2)          # [P, B]
+    assert eq.any(axis=1).all()
+    first = eq.argmax(axis=1).astype(np.int64)
+    order = (pairs[:, 0].astype(np.int64) << 40) | (first << 32) | pairs[:, 1]
+    assert (np.diff(order) > 0).all()
     # too small an output: SQ_ERR_CAPACITY and the required count comes back
     with pytest.raises(binding.SubQuadError) as ei:
         _run_path(rep, P, want_pairs.shape[0] // 2)
