@@ -22,8 +22,9 @@
 //                          counts into output offsets (and the total, so a too-small output is
 //                          reported before anything is written); pass 2 writes.
 //      row_sort_kernel     SQ_LSH_SORTED only: row i's partners arrive as <= B ascending,
-//                          pairwise-disjoint groups (one per band); every element's final rank
-//                          is the sum of its lower bounds in the groups.
+//                          pairwise-disjoint groups (one per band); they are merged pairwise in
+//                          a binary tree, an element's place being its own index plus its
+//                          lower bound in the sibling run.
 //   No raw-pair buffer and no atomics on the data path: results are deterministic.
 #include "sq_common.cuh"
 
@@ -427,15 +428,131 @@ emit_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint32_t* __
 // ---------------------------------------------------------------------------------------------
 // a5.3  SQ_LSH_SORTED: merge the <= B ascending, disjoint groups of every row
 // ---------------------------------------------------------------------------------------------
+// One warp per row.  The row's partners sit in inJ[base, base+T) as G non-empty ascending groups
+// that are pairwise disjoint.  They are merged pairwise, level by level (a binary tree over the
+// groups): an element's place in the merged pair is its index in its own run plus its lower
+// bound in the sibling run.  Levels ping-pong between inJ and the row's own slice of `out`
+// (viewed as uint32 scratch); the parity is arranged so that the last level reads inJ and
+// writes the final (i, j) pairs.
 constexpr int kRsWarps = 8;
+
+__device__ __forceinline__ uint32_t lower_bound_u32(const uint32_t* a, uint32_t len, uint32_t x) {
+  uint32_t lo = 0;
+  while (len > 0) {
+    const uint32_t half = len >> 1;
+    const bool less = a[lo + half] < x;
+    lo = less ? lo + half + 1 : lo;
+    len = less ? len - half - 1 : half;
+  }
+  return lo;
+}
+
+// Merge-path merge of the adjacent ascending runs src[a0,a1) and src[a1,b1) (all elements
+// distinct) into dst[a0,b1), or into outp[a0,b1) as (row, j) pairs when outp != nullptr.
+// Output tiles of kRsTile elements: the tile borders' splits are found 31 at a time (one binary
+// search per lane over the two runs), a tile's two input slices are staged in shared memory,
+// every lane merges 8 consecutive outputs, and the tile is written back coalesced.
+constexpr int kRsTile = 256;
+
+__device__ __forceinline__ void merge_pair_tiled(const uint32_t* src, uint32_t a0, uint32_t a1,
+                                                 uint32_t b1, uint32_t* dst, uint2* outp,
+                                                 uint32_t row, uint32_t* buf, int lane) {
+  const uint32_t* A = src + a0;
+  const uint32_t* B = src + a1;
+  const uint32_t lenA = a1 - a0, lenB = b1 - a1, nab = lenA + lenB;
+  const uint32_t ntile = (nab + kRsTile - 1) / kRsTile;
+  for (uint32_t tb = 0; tb < ntile; tb += 31) {
+    uint32_t my_ia;
+    {
+      const uint32_t d = min((tb + lane) * kRsTile, nab);
+      uint32_t lo = d > lenB ? d - lenB : 0u, hi = min(d, lenA);
+      while (lo < hi) {
+        const uint32_t mid = (lo + hi) >> 1;
+        if (A[mid] < B[d - 1 - mid]) lo = mid + 1; else hi = mid;
+      }
+      my_ia = lo;
+    }
+    const uint32_t ntb = min(31u, ntile - tb);
+    for (uint32_t tt = 0; tt < ntb; ++tt) {
+      const uint32_t ia0 = __shfl_sync(kFull, my_ia, tt), ia1 = __shfl_sync(kFull, my_ia, tt + 1);
+      const uint32_t d0 = (tb + tt) * kRsTile, d1 = min(d0 + kRsTile, nab);
+      const uint32_t ib0 = d0 - ia0, la = ia1 - ia0, nout = d1 - d0, lb = nout - la;
+      for (uint32_t e = lane; e < nout; e += 32) buf[e] = e < la ? A[ia0 + e] : B[ib0 + e - la];
+      __syncwarp();
+      const uint32_t dl = min((uint32_t)lane * 8u, nout);
+      uint32_t lo = dl > lb ? dl - lb : 0u, hi = min(dl, la);
+      while (lo < hi) {
+        const uint32_t mid = (lo + hi) >> 1;
+        if (buf[mid] < buf[la + dl - 1 - mid]) lo = mid + 1; else hi = mid;
+      }
+      uint32_t ii = lo, jj = dl - lo;
+      uint32_t x = ii < la ? buf[ii] : kFull, y = jj < lb ? buf[la + jj] : kFull;
+      uint32_t r[8];
+#pragma unroll
+      for (int k = 0; k < 8; ++k) {
+        const bool take = x < y;
+        r[k] = take ? x : y;
+        if (take) { ++ii; x = ii < la ? buf[ii] : kFull; }
+        else { ++jj; y = jj < lb ? buf[la + jj] : kFull; }
+      }
+      __syncwarp();
+      *reinterpret_cast<uint4*>(buf + lane * 8) = make_uint4(r[0], r[1], r[2], r[3]);
+      *reinterpret_cast<uint4*>(buf + lane * 8 + 4) = make_uint4(r[4], r[5], r[6], r[7]);
+      __syncwarp();
+      for (uint32_t e = lane; e < nout; e += 32) {
+        const uint32_t v = buf[e];
+        if (outp) outp[a0 + d0 + e] = make_uint2(row, v); else dst[a0 + d0 + e] = v;
+      }
+      __syncwarp();
+    }
+  }
+}
+
+// Merge of a SHORT ascending run (s <= kRsSmall elements) into a long one, both in src, adjacent
+// ([a0,a1) and [a1,b1), either may be the short one), all elements distinct.  Every short
+// element finds its lower bound in the long run (one binary search per lane); a long element
+// then moves up by the number of short elements placed before it, counted while the warp
+// streams over the long run 32 at a time.
+constexpr int kRsSmall = 64;
+
+__device__ __forceinline__ void merge_small_into_big(const uint32_t* src, uint32_t a0, uint32_t a1,
+                                                     uint32_t b1, uint32_t* dst, uint2* outp,
+                                                     uint32_t row, uint32_t* posbuf, int lane) {
+  const bool small_first = (a1 - a0) <= (b1 - a1);
+  const uint32_t* sm = src + (small_first ? a0 : a1);
+  const uint32_t* bg = src + (small_first ? a1 : a0);
+  const uint32_t s = small_first ? a1 - a0 : b1 - a1;
+  const uint32_t nb = (b1 - a0) - s;
+  for (uint32_t k = lane; k < s; k += 32) {
+    const uint32_t u = sm[k];
+    const uint32_t pos = lower_bound_u32(bg, nb, u);
+    posbuf[k] = pos;
+    if (outp) outp[a0 + pos + k] = make_uint2(row, u); else dst[a0 + pos + k] = u;
+  }
+  __syncwarp();
+  uint32_t kk = 0;                                   // short elements with pos <= e0 (uniform)
+  for (uint32_t e0 = 0; e0 < nb; e0 += 32) {
+    while (kk < s && posbuf[kk] <= e0) ++kk;
+    const uint32_t idx = e0 + lane;
+    uint32_t shift = kk;
+    for (uint32_t k2 = kk; k2 < s && posbuf[k2] <= e0 + 31; ++k2) shift += posbuf[k2] <= idx ? 1u : 0u;
+    if (idx < nb) {
+      const uint32_t v = bg[idx];
+      if (outp) outp[a0 + idx + shift] = make_uint2(row, v); else dst[a0 + idx + shift] = v;
+    }
+  }
+  __syncwarp();
+}
 
 __global__ void __launch_bounds__(kRsWarps * 32)
 row_sort_kernel(const uint32_t* __restrict__ off, int64_t n, int bands, uint32_t total,
-                const uint32_t* __restrict__ inJ, uint2* __restrict__ out) {
-  const int lane = threadIdx.x & 31;
-  const int64_t i = (int64_t)blockIdx.x * kRsWarps + (threadIdx.x >> 5);
+                uint32_t* inJ, uint2* out) {
+  __shared__ uint32_t bnd_sh[kRsWarps][34];
+  __shared__ __align__(16) uint32_t tile_sh[kRsWarps][kRsTile];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const int64_t i = (int64_t)blockIdx.x * kRsWarps + w;
   if (i >= n) return;
-  // lane b holds the start of group b; lane `bands` (or the shuffle below) gives the row end
+  // lane b holds the start of group b; the lanes past `bands` hold the row end
   const uint32_t row_end = (i + 1 < n) ? off[(i + 1) * bands] : total;
   const uint32_t gs = lane < bands ? off[i * bands + lane] : row_end;
   uint32_t ge = __shfl_down_sync(kFull, gs, 1);
@@ -444,28 +561,59 @@ row_sort_kernel(const uint32_t* __restrict__ off, int64_t n, int bands, uint32_t
   const uint32_t T = row_end - base;
   if (T == 0) return;
   const uint32_t nonempty = __ballot_sync(kFull, lane < bands && ge > gs);
-  if (__popc(nonempty) == 1) {               // already ascending
-    for (uint32_t t = lane; t < T; t += 32) out[base + t] = make_uint2((uint32_t)i, inJ[base + t]);
+  const int G = __popc(nonempty);
+  const uint32_t row = (uint32_t)i;
+  if (G == 1) {                              // already ascending
+    for (uint32_t t = lane; t < T; t += 32) out[base + t] = make_uint2(row, inJ[base + t]);
     return;
   }
-  for (uint32_t t0 = 0; t0 < T; t0 += 32) {
-    const uint32_t t = t0 + lane;
-    const uint32_t x = t < T ? inJ[base + t] : 0u;
+  if (T <= 32) {                             // rank by counting inside the warp
+    const uint32_t x = (uint32_t)lane < T ? inJ[base + lane] : kFull;
     uint32_t rank = 0;
-    for (uint32_t gm = nonempty; gm; gm &= gm - 1) {
-      const int g = __ffs(gm) - 1;
-      uint32_t lo = __shfl_sync(kFull, gs, g);
-      uint32_t len = __shfl_sync(kFull, ge, g) - lo;
-      const uint32_t first = lo;
-      while (len > 0) {                      // lower bound of x in group g (uniform trip count)
-        const uint32_t half = len >> 1;
-        const bool less = inJ[lo + half] < x;
-        lo = less ? lo + half + 1 : lo;
-        len = less ? len - half - 1 : half;
+    for (uint32_t s = 0; s < T; ++s) rank += __shfl_sync(kFull, x, s) < x ? 1u : 0u;
+    if ((uint32_t)lane < T) out[base + rank] = make_uint2(row, x);
+    return;
+  }
+  // compacted run boundaries, relative to base: bnd[q] = start of the q-th non-empty group
+  uint32_t* bnd = bnd_sh[w];
+  if (lane < bands && ge > gs) bnd[__popc(nonempty & ((1u << lane) - 1u))] = gs - base;
+  if (lane == 0) bnd[G] = T;
+  __syncwarp();
+  const int L = 32 - __clz(G - 1);           // ceil(log2 G), G >= 2
+  uint32_t* bufJ = inJ + base;
+  uint32_t* bufX = reinterpret_cast<uint32_t*>(out + base);
+  if ((L & 1) == 0) {                        // even number of levels: start from the scratch side
+    for (uint32_t t = lane; t < T; t += 32) bufX[t] = bufJ[t];
+    __syncwarp();
+  }
+  for (int k = 1; k <= L; ++k) {
+    const bool from_j = ((k + ((L & 1) ? 0 : 1)) & 1) != 0;
+    const uint32_t* src = from_j ? bufJ : bufX;
+    uint32_t* dst = from_j ? bufX : bufJ;
+    const bool last = k == L;
+    const int step = 1 << (k - 1);
+    for (int q = 0; q * 2 * step < G; ++q) {
+      const uint32_t a0 = bnd[min(2 * q * step, G)];
+      const uint32_t a1 = bnd[min((2 * q + 1) * step, G)];
+      const uint32_t b1 = bnd[min((2 * q + 2) * step, G)];
+      const uint32_t smaller = min(a1 - a0, b1 - a1);
+      if (smaller > 0 && smaller <= kRsSmall && smaller * 8 <= b1 - a0) {
+        merge_small_into_big(src, a0, a1, b1, dst, last ? out + base : nullptr, row, tile_sh[w], lane);
+        continue;
       }
-      rank += lo - first;
+      if (b1 - a0 >= 2 * kRsTile && smaller > 0) {
+        merge_pair_tiled(src, a0, a1, b1, dst, last ? out + base : nullptr, row, tile_sh[w], lane);
+        continue;
+      }
+      for (uint32_t e = a0 + lane; e < b1; e += 32) {
+        const uint32_t x = src[e];
+        uint32_t pos;
+        if (e < a1) pos = e + lower_bound_u32(src + a1, b1 - a1, x);
+        else pos = a0 + (e - a1) + lower_bound_u32(src + a0, a1 - a0, x);
+        if (last) out[base + pos] = make_uint2(row, x); else dst[pos] = x;
+      }
     }
-    if (t < T) out[base + rank] = make_uint2((uint32_t)i, x);
+    __syncwarp();
   }
 }
 
