@@ -24,10 +24,11 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 from paper_2602_17330_b200 import datagen as dg  # noqa: E402
+from paper_2602_17330_b200 import shard  # noqa: E402
 
 METRIC = "candidate_pairs_verified_per_s"
 UNIT = "pairs/s"
-INSTR_PER_COLUMN_WORD = 14          # algorithmic integer ops per unit
+ALU_OPS_PER_COLUMN_WORD = 7         # ALU-pipe logic ops of one Myers/Hyyro column step
 # bounded oracle samples (first n_s sequences of the same workload)
 ORACLE_SAMPLE = {"config1": 2000, "config2": 100_000, "config3": 300_000, "config4": 300_000}
 CAP_PER_SEQ = {"config2": 40, "config3": 60, "config4": 200}
@@ -213,7 +214,7 @@ def run_ours(args):
     dev = torch.device("cuda", local_rank)
     workload = args.workload
     P = dg.PARAMS[workload]
-    rep = make_repertoire(workload, args.n, rank)          # one independent repertoire per rank
+    rep = make_repertoire(workload, args.n, shard.rank_seed(rank))   # one independent repertoire per rank
     n = rep.n
     total_len = int(rep.offsets[-1])
     max_len = int(rep.lengths.max())
@@ -313,14 +314,9 @@ def run_ours(args):
     hits = int((dist_out[:cnt] <= P["max_d"]).sum().item())
     del pi, pj
 
-    # aggregate over ranks: units summed, time = max over ranks
-    agg = torch.tensor([step_ms, float(cnt), float(n), cells], dtype=torch.float64, device=dev)
-    if world > 1:
-        tmax = agg[:1].clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        tot = agg[1:].clone(); dist.all_reduce(tot, op=dist.ReduceOp.SUM)
-        step_ms_all, cnt_all, n_all, cells_all = tmax.item(), tot[0].item(), tot[1].item(), tot[2].item()
-    else:
-        step_ms_all, cnt_all, n_all, cells_all = step_ms, float(cnt), float(n), cells
+    # aggregate over ranks: units summed, time = max over ranks (paper_2602_17330_b200/shard.py)
+    step_ms_all, tot = shard.aggregate(step_ms, {"pairs": cnt, "seqs": n, "cells": cells}, dev)
+    cnt_all, n_all, cells_all = tot["pairs"], tot["seqs"], tot["cells"]
 
     # ---- e2e: through the C ABI with HOST buffers -------------------------------------------
     e2e = None
@@ -340,9 +336,8 @@ def run_ours(args):
             torch.cuda.synchronize()
             t_e2e = (time.perf_counter() - t0) / e2e_steps
             assert c3 == cnt
-            te = torch.tensor([t_e2e], dtype=torch.float64, device=dev)
-            if world > 1:
-                dist.all_reduce(te, op=dist.ReduceOp.MAX)
+            t_e2e_ms, _ = shard.aggregate(1e3 * t_e2e, {}, dev)
+            te = torch.tensor([t_e2e_ms * 1e-3], dtype=torch.float64)
             e2e = {"value": cnt_all / te.item(), "unit": UNIT,
                    "h2d_bytes_per_step": total_len + 8 * (n + 1),
                    "d2h_bytes_per_step": 10 * cnt, "ms_per_step": 1e3 * te.item(),
@@ -383,7 +378,7 @@ def run_ours(args):
             k["achieved_GBs"] = alg_bytes[name] / (ms / K * 1e-3) / 1e9
             k["frac"] = k["achieved_GBs"] / hbm_peak
         if name == "edit_distance":
-            ops = INSTR_PER_COLUMN_WORD * text_cols * ((max_len + 31) // 32)
+            ops = ALU_OPS_PER_COLUMN_WORD * text_cols * ((max_len + 31) // 32)
             k["bound"] = "alu"
             k["achieved_Gops"] = ops / (ms / K * 1e-3) / 1e9
             k["frac"] = k["achieved_Gops"] * 1e9 / int_peak["lop3"]
