@@ -21,6 +21,114 @@ __global__ void edit_pairs_kernel(const uint8_t* __restrict__ packed, int stride
   dist[p] = (uint16_t)d;
 }
 
+
+// ---- single-word fast path: every sequence fits one 32-bit word (max_len <= 31) ---------------
+// A warp takes 32 consecutive pairs.  sq_lsh_candidates emits pairs grouped by i, so the lanes
+// of a warp share a few distinct patterns i ("runs"): the Peq table of every run is built ONCE,
+// cooperatively (lane x holds residue x of the pattern; match.any gives the bit mask of every
+// residue in one instruction), and kept in shared memory [run][33] (odd stride: lanes of
+// different runs hit different banks, lanes of one run reading one residue are a broadcast).
+// Each lane then streams its own text j (one or two 16-byte loads, held in registers) through
+// the Myers/Hyyro column step; the distance is read off the final vertical deltas:
+// D[m][n] = n + popc(Pv) - popc(Mv) over the m pattern bits, so no score is tracked per column.
+constexpr int kEdWarps = 8;
+
+template <int STRIDE>
+__global__ void __launch_bounds__(kEdWarps * 32)
+edit_pairs_w1_kernel(const uint8_t* __restrict__ packed, int64_t n, const uint2* __restrict__ pairs,
+                     int64_t n_pairs, int max_d, uint16_t* __restrict__ dist) {
+  constexpr int WORDS = STRIDE / 4;
+  __shared__ uint32_t peq_sm[kEdWarps][32 * 33];
+  __shared__ uint32_t mlen_sm[kEdWarps][32];
+  const uint32_t lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const int64_t p = ((int64_t)blockIdx.x * kEdWarps + w) * 32 + lane;
+  const bool valid = p < n_pairs;
+  uint2 pr = make_uint2(0xFFFFFFFFu, 0xFFFFFFFFu);
+  if (valid) pr = pairs[p];
+  const bool inrange = valid && pr.x < (uint64_t)n && pr.y < (uint64_t)n;
+  const uint32_t i = inrange ? pr.x : 0xFFFFFFFFu;
+  // the text is independent of the runs: issue its load first
+  uint32_t tw[WORDS];
+  {
+    const uint4* rowB = reinterpret_cast<const uint4*>(packed + (int64_t)(inrange ? pr.y : 0u) * STRIDE);
+#pragma unroll
+    for (int q = 0; q < WORDS / 4; ++q) {
+      const uint4 v = inrange ? rowB[q] : make_uint4(0, 0, 0, 0);
+      tw[4 * q] = v.x; tw[4 * q + 1] = v.y; tw[4 * q + 2] = v.z; tw[4 * q + 3] = v.w;
+    }
+  }
+  // runs of equal i
+  const uint32_t prev = __shfl_up_sync(0xFFFFFFFFu, i, 1);
+  const bool head = lane == 0 || i != prev;
+  const uint32_t hm = __ballot_sync(0xFFFFFFFFu, head);
+  const uint32_t run = __popc(hm & (0xFFFFFFFFu >> (31 - lane))) - 1;
+  const int nruns = __popc(hm);
+  uint32_t* peq = peq_sm[w];
+  uint32_t rem = hm;
+#pragma unroll 1
+  for (int r = 0; r < nruns; ++r) {
+    const int hl = __ffs(rem) - 1;
+    rem &= rem - 1;
+    const uint32_t ir = __shfl_sync(0xFFFFFFFFu, i, hl);
+    uint32_t ch = 0xFFu;
+    if (ir != 0xFFFFFFFFu && lane < (uint32_t)STRIDE) ch = packed[(int64_t)ir * STRIDE + lane];
+    const uint32_t m = ir != 0xFFFFFFFFu ? __shfl_sync(0xFFFFFFFFu, ch, STRIDE - 1) : 0u;
+    peq[r * 33 + lane] = 0u;
+    __syncwarp();
+    const uint32_t mm = __match_any_sync(0xFFFFFFFFu, ch);
+    if (lane < m) peq[r * 33 + ch] = mm & ((1u << m) - 1u);       // m <= 31
+    if (lane == 0) mlen_sm[w][r] = m;
+  }
+  __syncwarp();
+  if (!valid) return;
+  if (!inrange) { dist[p] = 0xFFFFu; return; }
+  const int m = (int)mlen_sm[w][run];
+  const int nlen = (int)(tw[WORDS - 1] >> 24);
+  const int diff = m > nlen ? m - nlen : nlen - m;
+  int d;
+  if (max_d >= 0 && diff > max_d) d = max_d + 1;
+  else if (m == 0) d = nlen;
+  else if (nlen == 0) d = m;
+  else {
+    const uint32_t* pq = peq + run * 33;
+    uint32_t Pv = 0xFFFFFFFFu, Mv = 0u;
+#pragma unroll
+    for (int wi = 0; wi < WORDS; ++wi) {
+      if (4 * wi < nlen) {
+        const uint32_t word = tw[wi];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          if (4 * wi + q < nlen) {
+            const uint32_t Eq = pq[(word >> (8 * q)) & 0xFFu];
+            const uint32_t Xv = Eq | Mv;
+            const uint32_t Xh = (((Eq & Pv) + Pv) ^ Pv) | Eq;
+            uint32_t Ph = Mv | ~(Xh | Pv);
+            uint32_t Mh = Pv & Xh;
+            Ph = (Ph << 1) | 1u;
+            Mh <<= 1;
+            Pv = Mh | ~(Xv | Ph);
+            Mv = Ph & Xv;
+          }
+        }
+      }
+    }
+    const uint32_t mask = (1u << m) - 1u;                          // m <= 31
+    d = nlen + __popc(Pv & mask) - __popc(Mv & mask);
+  }
+  if (max_d >= 0 && d > max_d) d = max_d + 1;
+  dist[p] = (uint16_t)d;
+}
+
+template <int STRIDE>
+int launch_edit_w1(sq_ctx* c, const uint32_t* pairs, int64_t n_pairs, int max_d, uint16_t* dist_out) {
+  const int64_t per_block = kEdWarps * 32;
+  const int64_t blocks = (n_pairs + per_block - 1) / per_block;
+  SQ_TIMED(c, SQ_K_EDIT, edit_pairs_w1_kernel<STRIDE><<<(unsigned)blocks, kEdWarps * 32, 0, c->stream>>>(
+      c->packed, c->n, reinterpret_cast<const uint2*>(pairs), n_pairs, max_d, dist_out));
+  SQ_LAUNCH_CHECK(c);
+  return SQ_OK;
+}
+
 template <int W>
 int launch_edit(sq_ctx* c, const uint32_t* pairs, int64_t n_pairs, int max_d, uint16_t* dist_out) {
   const int threads = W <= 2 ? 256 : 128;
@@ -46,6 +154,8 @@ int sq_edit_distance_impl(sq_ctx* c, const uint32_t* pairs, int64_t n_pairs, int
   if (!pairs || !dist_out) return SQ_ERR_INVALID_ARG;
   if (n_pairs >= (1ll << 31) * 128) return SQ_ERR_UNSUPPORTED;
   if (max_d > 65534) max_d = -1;
+  if (c->stride == 16) return launch_edit_w1<16>(c, pairs, n_pairs, max_d, dist_out);
+  if (c->stride == 32) return launch_edit_w1<32>(c, pairs, n_pairs, max_d, dist_out);
   const int words = (c->max_len + 31) / 32;
   if (words <= 1) return launch_edit<1>(c, pairs, n_pairs, max_d, dist_out);
   if (words <= 2) return launch_edit<2>(c, pairs, n_pairs, max_d, dist_out);

@@ -21,10 +21,10 @@
 //                          Pass 1 counts per (sequence, band); an exclusive scan turns the
 //                          counts into output offsets (and the total, so a too-small output is
 //                          reported before anything is written); pass 2 writes.
-//      row_sort_kernel     SQ_LSH_SORTED only: row i's partners arrive as <= B ascending,
-//                          pairwise-disjoint groups (one per band); they are merged pairwise in
-//                          a binary tree, an element's place being its own index plus its
-//                          lower bound in the sibling run.
+//      row_sort_kernel     SQ_LSH_SORTED only: row i's partners arrive as <= B ascending
+//                          groups (one per band); one warp per row orders them with a single
+//                          most-significant-digit pass over 1,024 value bins (shared-memory
+//                          counters) plus a rank inside the bin.
 //   No raw-pair buffer and no atomics on the data path: results are deterministic.
 #include "sq_common.cuh"
 
@@ -426,132 +426,21 @@ emit_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint32_t* __
 }
 
 // ---------------------------------------------------------------------------------------------
-// a5.3  SQ_LSH_SORTED: merge the <= B ascending, disjoint groups of every row
+// a5.3  SQ_LSH_SORTED: put every row's partners in ascending order
 // ---------------------------------------------------------------------------------------------
-// One warp per row.  The row's partners sit in inJ[base, base+T) as G non-empty ascending groups
-// that are pairwise disjoint.  They are merged pairwise, level by level (a binary tree over the
-// groups): an element's place in the merged pair is its index in its own run plus its lower
-// bound in the sibling run.  Levels ping-pong between inJ and the row's own slice of `out`
-// (viewed as uint32 scratch); the parity is arranged so that the last level reads inJ and
-// writes the final (i, j) pairs.
+// One warp per row.  The row's partners sit in inJ[base, base+T) as <= B ascending groups.  The
+// ids of a repertoire carry no structure, so the partners of a row are spread evenly between the
+// row's smallest and largest partner: ONE most-significant-digit pass over kRsBins equal-width
+// value bins (shared-memory counters) groups them, and an element's final place is its bin's
+// start plus the number of smaller elements in its own bin (1-2 on average, any number is
+// correct).  Passes: count per bin -> scan -> group into the row's slice of `out` (as uint32
+// scratch) -> rank inside the bin, back into inJ (now sorted) -> write (i, j) pairs.
 constexpr int kRsWarps = 8;
+constexpr int kRsBins = 1024;
 
-__device__ __forceinline__ uint32_t lower_bound_u32(const uint32_t* a, uint32_t len, uint32_t x) {
-  uint32_t lo = 0;
-  while (len > 0) {
-    const uint32_t half = len >> 1;
-    const bool less = a[lo + half] < x;
-    lo = less ? lo + half + 1 : lo;
-    len = less ? len - half - 1 : half;
-  }
-  return lo;
-}
-
-// Merge-path merge of the adjacent ascending runs src[a0,a1) and src[a1,b1) (all elements
-// distinct) into dst[a0,b1), or into outp[a0,b1) as (row, j) pairs when outp != nullptr.
-// Output tiles of kRsTile elements: the tile borders' splits are found 31 at a time (one binary
-// search per lane over the two runs), a tile's two input slices are staged in shared memory,
-// every lane merges 8 consecutive outputs, and the tile is written back coalesced.
-constexpr int kRsTile = 256;
-
-__device__ __forceinline__ void merge_pair_tiled(const uint32_t* src, uint32_t a0, uint32_t a1,
-                                                 uint32_t b1, uint32_t* dst, uint2* outp,
-                                                 uint32_t row, uint32_t* buf, int lane) {
-  const uint32_t* A = src + a0;
-  const uint32_t* B = src + a1;
-  const uint32_t lenA = a1 - a0, lenB = b1 - a1, nab = lenA + lenB;
-  const uint32_t ntile = (nab + kRsTile - 1) / kRsTile;
-  for (uint32_t tb = 0; tb < ntile; tb += 31) {
-    uint32_t my_ia;
-    {
-      const uint32_t d = min((tb + lane) * kRsTile, nab);
-      uint32_t lo = d > lenB ? d - lenB : 0u, hi = min(d, lenA);
-      while (lo < hi) {
-        const uint32_t mid = (lo + hi) >> 1;
-        if (A[mid] < B[d - 1 - mid]) lo = mid + 1; else hi = mid;
-      }
-      my_ia = lo;
-    }
-    const uint32_t ntb = min(31u, ntile - tb);
-    for (uint32_t tt = 0; tt < ntb; ++tt) {
-      const uint32_t ia0 = __shfl_sync(kFull, my_ia, tt), ia1 = __shfl_sync(kFull, my_ia, tt + 1);
-      const uint32_t d0 = (tb + tt) * kRsTile, d1 = min(d0 + kRsTile, nab);
-      const uint32_t ib0 = d0 - ia0, la = ia1 - ia0, nout = d1 - d0, lb = nout - la;
-      for (uint32_t e = lane; e < nout; e += 32) buf[e] = e < la ? A[ia0 + e] : B[ib0 + e - la];
-      __syncwarp();
-      const uint32_t dl = min((uint32_t)lane * 8u, nout);
-      uint32_t lo = dl > lb ? dl - lb : 0u, hi = min(dl, la);
-      while (lo < hi) {
-        const uint32_t mid = (lo + hi) >> 1;
-        if (buf[mid] < buf[la + dl - 1 - mid]) lo = mid + 1; else hi = mid;
-      }
-      uint32_t ii = lo, jj = dl - lo;
-      uint32_t x = ii < la ? buf[ii] : kFull, y = jj < lb ? buf[la + jj] : kFull;
-      uint32_t r[8];
-#pragma unroll
-      for (int k = 0; k < 8; ++k) {
-        const bool take = x < y;
-        r[k] = take ? x : y;
-        if (take) { ++ii; x = ii < la ? buf[ii] : kFull; }
-        else { ++jj; y = jj < lb ? buf[la + jj] : kFull; }
-      }
-      __syncwarp();
-      *reinterpret_cast<uint4*>(buf + lane * 8) = make_uint4(r[0], r[1], r[2], r[3]);
-      *reinterpret_cast<uint4*>(buf + lane * 8 + 4) = make_uint4(r[4], r[5], r[6], r[7]);
-      __syncwarp();
-      for (uint32_t e = lane; e < nout; e += 32) {
-        const uint32_t v = buf[e];
-        if (outp) outp[a0 + d0 + e] = make_uint2(row, v); else dst[a0 + d0 + e] = v;
-      }
-      __syncwarp();
-    }
-  }
-}
-
-// Merge of a SHORT ascending run (s <= kRsSmall elements) into a long one, both in src, adjacent
-// ([a0,a1) and [a1,b1), either may be the short one), all elements distinct.  Every short
-// element finds its lower bound in the long run (one binary search per lane); a long element
-// then moves up by the number of short elements placed before it, counted while the warp
-// streams over the long run 32 at a time.
-constexpr int kRsSmall = 64;
-
-__device__ __forceinline__ void merge_small_into_big(const uint32_t* src, uint32_t a0, uint32_t a1,
-                                                     uint32_t b1, uint32_t* dst, uint2* outp,
-                                                     uint32_t row, uint32_t* posbuf, int lane) {
-  const bool small_first = (a1 - a0) <= (b1 - a1);
-  const uint32_t* sm = src + (small_first ? a0 : a1);
-  const uint32_t* bg = src + (small_first ? a1 : a0);
-  const uint32_t s = small_first ? a1 - a0 : b1 - a1;
-  const uint32_t nb = (b1 - a0) - s;
-  for (uint32_t k = lane; k < s; k += 32) {
-    const uint32_t u = sm[k];
-    const uint32_t pos = lower_bound_u32(bg, nb, u);
-    posbuf[k] = pos;
-    if (outp) outp[a0 + pos + k] = make_uint2(row, u); else dst[a0 + pos + k] = u;
-  }
-  __syncwarp();
-  uint32_t kk = 0;                                   // short elements with pos <= e0 (uniform)
-  for (uint32_t e0 = 0; e0 < nb; e0 += 32) {
-    while (kk < s && posbuf[kk] <= e0) ++kk;
-    const uint32_t idx = e0 + lane;
-    uint32_t shift = kk;
-    for (uint32_t k2 = kk; k2 < s && posbuf[k2] <= e0 + 31; ++k2) shift += posbuf[k2] <= idx ? 1u : 0u;
-    if (idx < nb) {
-      const uint32_t v = bg[idx];
-      if (outp) outp[a0 + idx + shift] = make_uint2(row, v); else dst[a0 + idx + shift] = v;
-    }
-  }
-  __syncwarp();
-}
-
-__global__ void __launch_bounds__(kRsWarps * 32)
-row_sort_kernel(const uint32_t* __restrict__ off, int64_t n, int bands, uint32_t total,
-                uint32_t* inJ, uint2* out) {
-  __shared__ uint32_t bnd_sh[kRsWarps][34];
-  __shared__ __align__(16) uint32_t tile_sh[kRsWarps][kRsTile];
-  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  const int64_t i = (int64_t)blockIdx.x * kRsWarps + w;
-  if (i >= n) return;
+__device__ __forceinline__ void
+sort_one_row(const uint32_t* __restrict__ off, int64_t n, int bands, uint32_t total,
+             uint32_t* inJ, uint2* out, int64_t i, uint32_t* bins, int lane) {
   // lane b holds the start of group b; the lanes past `bands` hold the row end
   const uint32_t row_end = (i + 1 < n) ? off[(i + 1) * bands] : total;
   const uint32_t gs = lane < bands ? off[i * bands + lane] : row_end;
@@ -560,60 +449,86 @@ row_sort_kernel(const uint32_t* __restrict__ off, int64_t n, int bands, uint32_t
   const uint32_t base = __shfl_sync(kFull, gs, 0);
   const uint32_t T = row_end - base;
   if (T == 0) return;
-  const uint32_t nonempty = __ballot_sync(kFull, lane < bands && ge > gs);
-  const int G = __popc(nonempty);
+  const bool has = lane < bands && ge > gs;
+  const uint32_t nonempty = __ballot_sync(kFull, has);
   const uint32_t row = (uint32_t)i;
-  if (G == 1) {                              // already ascending
-    for (uint32_t t = lane; t < T; t += 32) out[base + t] = make_uint2(row, inJ[base + t]);
+  uint32_t* J = inJ + base;
+  if (__popc(nonempty) == 1) {               // already ascending
+    for (uint32_t t = lane; t < T; t += 32) out[base + t] = make_uint2(row, J[t]);
     return;
   }
   if (T <= 32) {                             // rank by counting inside the warp
-    const uint32_t x = (uint32_t)lane < T ? inJ[base + lane] : kFull;
+    const uint32_t x = (uint32_t)lane < T ? J[lane] : kFull;
     uint32_t rank = 0;
     for (uint32_t s = 0; s < T; ++s) rank += __shfl_sync(kFull, x, s) < x ? 1u : 0u;
     if ((uint32_t)lane < T) out[base + rank] = make_uint2(row, x);
     return;
   }
-  // compacted run boundaries, relative to base: bnd[q] = start of the q-th non-empty group
-  uint32_t* bnd = bnd_sh[w];
-  if (lane < bands && ge > gs) bnd[__popc(nonempty & ((1u << lane) - 1u))] = gs - base;
-  if (lane == 0) bnd[G] = T;
+  // value range of the row: every group is ascending, so its ends are its extremes
+  uint32_t lo = has ? inJ[gs] : kFull, hi = has ? inJ[ge - 1] : 0u;
+  lo = __reduce_min_sync(kFull, lo);
+  hi = __reduce_max_sync(kFull, hi);
+  const float scale = (float)kRsBins / ((float)(hi - lo) + 1.0f);
+  auto bin_of = [&](uint32_t x) -> uint32_t {     // monotone in x, < kRsBins
+    return min((uint32_t)kRsBins - 1u, (uint32_t)((float)(x - lo) * scale));
+  };
+  uint32_t* X = reinterpret_cast<uint32_t*>(out + base);     // scratch: first T words of the slice
+#pragma unroll
+  for (int q = 0; q < kRsBins / 128; ++q)
+    *reinterpret_cast<uint4*>(bins + q * 128 + lane * 4) = make_uint4(0, 0, 0, 0);
   __syncwarp();
-  const int L = 32 - __clz(G - 1);           // ceil(log2 G), G >= 2
-  uint32_t* bufJ = inJ + base;
-  uint32_t* bufX = reinterpret_cast<uint32_t*>(out + base);
-  if ((L & 1) == 0) {                        // even number of levels: start from the scratch side
-    for (uint32_t t = lane; t < T; t += 32) bufX[t] = bufJ[t];
-    __syncwarp();
-  }
-  for (int k = 1; k <= L; ++k) {
-    const bool from_j = ((k + ((L & 1) ? 0 : 1)) & 1) != 0;
-    const uint32_t* src = from_j ? bufJ : bufX;
-    uint32_t* dst = from_j ? bufX : bufJ;
-    const bool last = k == L;
-    const int step = 1 << (k - 1);
-    for (int q = 0; q * 2 * step < G; ++q) {
-      const uint32_t a0 = bnd[min(2 * q * step, G)];
-      const uint32_t a1 = bnd[min((2 * q + 1) * step, G)];
-      const uint32_t b1 = bnd[min((2 * q + 2) * step, G)];
-      const uint32_t smaller = min(a1 - a0, b1 - a1);
-      if (smaller > 0 && smaller <= kRsSmall && smaller * 8 <= b1 - a0) {
-        merge_small_into_big(src, a0, a1, b1, dst, last ? out + base : nullptr, row, tile_sh[w], lane);
-        continue;
-      }
-      if (b1 - a0 >= 2 * kRsTile && smaller > 0) {
-        merge_pair_tiled(src, a0, a1, b1, dst, last ? out + base : nullptr, row, tile_sh[w], lane);
-        continue;
-      }
-      for (uint32_t e = a0 + lane; e < b1; e += 32) {
-        const uint32_t x = src[e];
-        uint32_t pos;
-        if (e < a1) pos = e + lower_bound_u32(src + a1, b1 - a1, x);
-        else pos = a0 + (e - a1) + lower_bound_u32(src + a0, a1 - a0, x);
-        if (last) out[base + pos] = make_uint2(row, x); else dst[pos] = x;
-      }
+  for (uint32_t t = lane; t < T; t += 32) atomicAdd(&bins[bin_of(J[t])], 1u);
+  __syncwarp();
+  {                                          // exclusive scan of the bin counts
+    constexpr int PER = kRsBins / 32;
+    uint32_t v[PER], s = 0;
+#pragma unroll
+    for (int q = 0; q < PER; ++q) { v[q] = bins[lane * PER + q]; s += v[q]; }
+    uint32_t inc = s;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const uint32_t o = __shfl_up_sync(kFull, inc, d);
+      if (lane >= d) inc += o;
     }
-    __syncwarp();
+    uint32_t run = inc - s;
+#pragma unroll
+    for (int q = 0; q < PER; ++q) { bins[lane * PER + q] = run; run += v[q]; }
+  }
+  __syncwarp();
+  for (uint32_t t = lane; t < T; t += 32) {  // group by bin (arrival order inside a bin)
+    const uint32_t x = J[t];
+    X[atomicAdd(&bins[bin_of(x)], 1u)] = x;
+  }
+  __syncwarp();                              // now bins[b] = end of bin b = start of bin b+1
+  for (uint32_t t = lane; t < T; t += 32) {  // rank inside the bin -> sorted, back into J
+    const uint32_t x = X[t];
+    const uint32_t b = bin_of(x);
+    const uint32_t s = b ? bins[b - 1] : 0u, e = bins[b];
+    uint32_t r = s;
+    for (uint32_t q = s; q < e; ++q) r += X[q] < x ? 1u : 0u;
+    J[r] = x;
+  }
+  __syncwarp();
+  for (uint32_t t = lane; t < T; t += 32) out[base + t] = make_uint2(row, J[t]);
+}
+
+constexpr int kRsChunk = 8;
+
+__global__ void __launch_bounds__(kRsWarps * 32)
+row_sort_kernel(const uint32_t* __restrict__ off, int64_t n, int bands, uint32_t total,
+                uint32_t* inJ, uint2* out, unsigned long long* __restrict__ next_row) {
+  __shared__ uint32_t bins_sh[kRsWarps][kRsBins];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  // Rows differ by four orders of magnitude in size: persistent warps fetch rows kRsChunk at a
+  // time from a global counter, so no warp idles behind a heavy row of its block.
+  for (;;) {
+    unsigned long long first = 0;
+    if (lane == 0) first = atomicAdd(next_row, (unsigned long long)kRsChunk);
+    first = __shfl_sync(kFull, first, 0);
+    if ((int64_t)first >= n) return;
+    const int64_t last = min(n, (int64_t)first + kRsChunk);
+    for (int64_t i = (int64_t)first; i < last; ++i)
+      sort_one_row(off, n, bands, total, inJ, out, i, bins_sh[w], lane);
   }
 }
 
@@ -793,8 +708,16 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
     if (!tmpJ) return SQ_ERR_WORKSPACE;
     rc = dispatch_emit(c, bw, EM_FILL_J, units, nunits, units0, nunits0, vin, (uint32_t)n2, bands, S, cnt, tmpJ, nullptr);
     if (rc != SQ_OK) return rc;
-    SQ_TIMED(c, SQ_K_ROWSORT, row_sort_kernel<<<(unsigned)((n + kRsWarps - 1) / kRsWarps), kRsWarps * 32, 0, st>>>(
-        cnt, n, bands, (uint32_t)uniq, tmpJ, out));
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, row_sort_kernel, kRsWarps * 32, 0) != cudaSuccess ||
+        per_sm < 1)
+      per_sm = 2;
+    unsigned g = (unsigned)(c->sm_count * per_sm);
+    const unsigned need = (unsigned)((n + kRsWarps * kRsChunk - 1) / (kRsWarps * kRsChunk));
+    if (g > need) g = need;
+    SQ_CUDA(c, cudaMemsetAsync(counters + 6, 0, 8, st));
+    SQ_TIMED(c, SQ_K_ROWSORT, row_sort_kernel<<<g, kRsWarps * 32, 0, st>>>(
+        cnt, n, bands, (uint32_t)uniq, tmpJ, out, counters + 6));
     SQ_LAUNCH_CHECK(c);
   }
   SQ_CUDA(c, cudaStreamSynchronize(st));
