@@ -113,15 +113,18 @@ __device__ int64_t run_end(const uint64_t* __restrict__ k, int64_t at, uint64_t 
 // S layout: [n][SW] uint32, SW = 4 * BW (rows are 16-byte aligned for vector loads).
 // units: (global sorted position of the unit's first row, kept members from there to the end
 // of the bucket); band 0's units go to their own list units0 (they need no compares).
-// counters: [1] raw pairs, [4] number of units of bands >= 1, [5] number of units of band 0.
+// ubase[u] = index of unit u's first 32-word tile in the mask cache (bands >= 1).
+// counters: [1] raw pairs, [4] units of bands >= 1, [5] units of band 0, [7] mask tiles.
 __global__ void __launch_bounds__(kBsThreads)
 bucket_scan_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict__ ids, int64_t n2,
                    int cap, int SW, uint32_t* __restrict__ S, uint2* __restrict__ units,
-                   uint2* __restrict__ units0, unsigned long long* __restrict__ counters) {
+                   uint2* __restrict__ units0, uint32_t* __restrict__ ubase,
+                   unsigned long long* __restrict__ counters) {
   __shared__ int sh_w[kBsThreads / 32];
   __shared__ int sh_carry_head, sh_carry_end;
   __shared__ unsigned long long sh_raw;
-  __shared__ uint32_t sh_unit_base, sh_unit_cnt;
+  __shared__ uint32_t sh_unit_base, sh_unit_cnt, sh_tile_cnt;
+  __shared__ unsigned long long sh_tile_base;
   const int band = blockIdx.y;
   const uint64_t* __restrict__ k = keys + (int64_t)band * n2;
   const uint32_t* __restrict__ idb = ids + (int64_t)band * n2;
@@ -129,7 +132,7 @@ bucket_scan_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict
   const int64_t tile_end = min(n2, tile0 + kBsTile);             // exclusive
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int64_t p0 = tile0 + (int64_t)threadIdx.x * kBsItems;
-  if (threadIdx.x == 0) { sh_raw = 0ull; sh_unit_cnt = 0u; }
+  if (threadIdx.x == 0) { sh_raw = 0ull; sh_unit_cnt = 0u; sh_tile_cnt = 0u; }
 
   uint64_t kk[kBsItems];
   bool valid[kBsItems], head[kBsItems], tail[kBsItems];
@@ -224,8 +227,10 @@ bucket_scan_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict
     }
   }
   // append the units (order across blocks is irrelevant: output positions never depend on it)
-  uint32_t my = 0;
-  if (nunit) my = atomicAdd(&sh_unit_cnt, nunit);
+  uint32_t my = 0, my_tiles = 0, ntiles = 0;
+#pragma unroll
+  for (int t = 0; t < kBsItems; ++t) if (has_unit[t]) ntiles += (unit[t].y + 31u) >> 5;
+  if (nunit) { my = atomicAdd(&sh_unit_cnt, nunit); my_tiles = atomicAdd(&sh_tile_cnt, ntiles); }
 #pragma unroll
   for (int d = 16; d > 0; d >>= 1) raw += __shfl_xor_sync(kFull, raw, d);
   if (lane == 0 && raw) atomicAdd(&sh_raw, raw);
@@ -234,12 +239,19 @@ bucket_scan_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict
     if (sh_unit_cnt)
       sh_unit_base = (uint32_t)atomicAdd(counters + (band == 0 ? 5 : 4), (unsigned long long)sh_unit_cnt);
     if (sh_raw) atomicAdd(counters + 1, sh_raw);
+    if (band != 0 && sh_tile_cnt) sh_tile_base = atomicAdd(counters + 7, (unsigned long long)sh_tile_cnt);
   }
   __syncthreads();
   uint2* __restrict__ ulist = band == 0 ? units0 : units;
   uint32_t q = sh_unit_base + my;
+  unsigned long long tb = sh_tile_base + my_tiles;   // (band >= 1) first tile of the unit's masks
 #pragma unroll
-  for (int t = 0; t < kBsItems; ++t) if (has_unit[t]) ulist[q++] = unit[t];
+  for (int t = 0; t < kBsItems; ++t) {
+    if (has_unit[t]) {
+      if (band != 0) { ubase[q] = (uint32_t)tb; tb += (unit[t].y + 31u) >> 5; }
+      ulist[q++] = unit[t];
+    }
+  }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -292,7 +304,8 @@ __device__ __forceinline__ void sweep_tile(const uint32_t* __restrict__ sm,
                                            const uint32_t* __restrict__ idt, const uint4 (&R)[BW],
                                            uint32_t cbeg, uint32_t ncol, uint32_t c0, uint32_t lane,
                                            bool rowok, uint32_t myid, uint32_t& acc,
-                                           uint32_t* __restrict__ outJ, uint2* __restrict__ outP) {
+                                           uint32_t& tmask, uint32_t* __restrict__ outJ,
+                                           uint2* __restrict__ outP) {
   constexpr int RS = 4 * BW + 4;
   if constexpr (NCH <= BW) {
 #pragma unroll 4
@@ -305,7 +318,7 @@ __device__ __forceinline__ void sweep_tile(const uint32_t* __restrict__ sm,
       }
       const bool isnew = !dup && rowok && (c0 + c > lane);
       if (MODE == EM_COUNT) {
-        acc += isnew ? 1u : 0u;
+        tmask |= isnew ? (1u << c) : 0u;
       } else if (isnew) {
         const uint32_t j = idt[c];
         if (MODE == EM_FILL_J) outJ[acc] = j; else outP[acc] = make_uint2(myid, j);
@@ -328,7 +341,8 @@ template <int BW, int MODE>
 __global__ void __launch_bounds__(kEmWarps * 32)
 emit_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint32_t* __restrict__ ids,
             uint32_t n2, int bands, const uint32_t* __restrict__ S, uint32_t* __restrict__ cnt_off,
-            uint32_t* __restrict__ outJ, uint2* __restrict__ outP) {
+            uint32_t* __restrict__ outJ, uint2* __restrict__ outP,
+            const uint32_t* __restrict__ ubase, uint32_t* __restrict__ masks) {
   constexpr int SW = 4 * BW;
   constexpr int RS = SW + 4;                 // shared row stride in words (16-byte aligned)
   constexpr int RPR = 32 / BW;               // S rows fetched per load round
@@ -375,7 +389,7 @@ emit_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint32_t* __
   cp_async_commit();
 
   uint4 R[BW];
-  uint32_t acc = 0, myid = 0;
+  uint32_t acc = 0, myid = 0, ub = 0;
   bool rowok = false;
   int k = 0;
   while (dc.ok) {
@@ -392,6 +406,7 @@ emit_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint32_t* __
       rowok = lane < min(32u, dc.mrem - 1u);
       acc = 0;
       if (MODE != EM_COUNT && rowok) acc = cnt_off[(int64_t)myid * bands + b];
+      if (MODE == EM_COUNT && masks) ub = ubase[dc.u];
 #pragma unroll
       for (int ch = 0; ch < BW; ++ch) {
         if (4 * ch < b) {
@@ -407,22 +422,68 @@ emit_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint32_t* __
     const uint32_t ncol = min(32u, dc.mrem - dc.c0);
     const uint32_t cbeg = dc.c0 == 0 ? 1u : 0u;
     const uint32_t* idt = idsm[w][k & 1];
+    uint32_t tmask = 0;                       // EM_COUNT: bit c = pair (my row, column c) is new
     switch ((b + 3) >> 2) {
-      case 1: sweep_tile<BW, 1, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, outJ, outP); break;
-      case 2: sweep_tile<BW, 2, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, outJ, outP); break;
-      case 3: sweep_tile<BW, 3, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, outJ, outP); break;
-      case 4: sweep_tile<BW, 4, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, outJ, outP); break;
-      case 5: sweep_tile<BW, 5, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, outJ, outP); break;
-      case 6: sweep_tile<BW, 6, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, outJ, outP); break;
-      case 7: sweep_tile<BW, 7, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, outJ, outP); break;
-      default: sweep_tile<BW, 8, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, outJ, outP); break;
+      case 1: sweep_tile<BW, 1, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, tmask, outJ, outP); break;
+      case 2: sweep_tile<BW, 2, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, tmask, outJ, outP); break;
+      case 3: sweep_tile<BW, 3, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, tmask, outJ, outP); break;
+      case 4: sweep_tile<BW, 4, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, tmask, outJ, outP); break;
+      case 5: sweep_tile<BW, 5, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, tmask, outJ, outP); break;
+      case 6: sweep_tile<BW, 6, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, tmask, outJ, outP); break;
+      case 7: sweep_tile<BW, 7, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, tmask, outJ, outP); break;
+      default: sweep_tile<BW, 8, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, tmask, outJ, outP); break;
     }
-    if (MODE == EM_COUNT && rowok && dc.c0 + 32 >= dc.mrem)
-      cnt_off[(int64_t)myid * bands + b] = acc;
+    if (MODE == EM_COUNT) {
+      acc += __popc(tmask);
+      if (masks) masks[((size_t)ub + (dc.c0 >> 5)) * 32 + lane] = tmask;   // kept for the fill pass
+      if (rowok && dc.c0 + 32 >= dc.mrem) cnt_off[(int64_t)myid * bands + b] = acc;
+    }
     __syncwarp();
     dc = dn; idc_c = idc_n; dn = d2; idc_n = id2; ++k;
   }
   cp_async_wait<0>();
+}
+
+// Pass 2 when the count pass could keep its per-tile masks: no S rows, no compares.  One
+// (persistent) warp per unit walks the unit's tiles; lane = row holds the mask of its new columns
+// of the tile and the id of column `lane`; every round each lane with a bit left takes its next
+// column's id from the owning lane (SHFL) and appends it to its row's output.
+template <bool PAIRS>
+__global__ void __launch_bounds__(kEmWarps * 32)
+emit_fill_masks_kernel(const uint2* __restrict__ units, uint32_t nunits,
+                       const uint32_t* __restrict__ ubase, const uint32_t* __restrict__ masks,
+                       const uint32_t* __restrict__ ids, uint32_t n2, int bands,
+                       const uint32_t* __restrict__ cnt_off, uint32_t* __restrict__ outJ,
+                       uint2* __restrict__ outP) {
+  const uint32_t lane = threadIdx.x & 31;
+  const uint32_t nw = gridDim.x * kEmWarps;
+  for (uint32_t u = blockIdx.x * kEmWarps + (threadIdx.x >> 5); u < nunits; u += nw) {
+    const uint2 unit = units[u];
+    const uint32_t g0 = unit.x, mrem = unit.y;
+    const int b = (int)(g0 / n2);
+    const uint32_t* __restrict__ idp = ids + g0;
+    const uint32_t* __restrict__ mp = masks + (size_t)ubase[u] * 32 + lane;
+    const uint32_t myid = lane < mrem ? idp[lane] : 0u;
+    uint32_t acc = lane < min(32u, mrem - 1u) ? cnt_off[(int64_t)myid * bands + b] : 0u;
+    uint32_t mask = mp[0], idc = myid;
+    for (uint32_t c0 = 0; c0 < mrem; c0 += 32) {
+      uint32_t mask_n = 0, idc_n = 0;            // next tile, in flight during this one
+      if (c0 + 32 < mrem) {
+        mask_n = mp[(size_t)(c0 + 32)];          // (c0+32)/32 tiles further = (c0+32) words
+        if (c0 + 32 + lane < mrem) idc_n = idp[c0 + 32 + lane];
+      }
+      while (__any_sync(kFull, mask != 0u)) {
+        const int c = mask ? __ffs(mask) - 1 : 0;
+        const uint32_t j = __shfl_sync(kFull, idc, c);
+        if (mask) {
+          if (PAIRS) outP[acc] = make_uint2(myid, j); else outJ[acc] = j;
+          ++acc;
+          mask &= mask - 1;
+        }
+      }
+      mask = mask_n; idc = idc_n;
+    }
+  }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -477,7 +538,14 @@ sort_one_row(const uint32_t* __restrict__ off, int64_t n, int bands, uint32_t to
   for (int q = 0; q < kRsBins / 128; ++q)
     *reinterpret_cast<uint4*>(bins + q * 128 + lane * 4) = make_uint4(0, 0, 0, 0);
   __syncwarp();
-  for (uint32_t t = lane; t < T; t += 32) atomicAdd(&bins[bin_of(J[t])], 1u);
+  // (every pass loads 4 batches of 32 before it uses them: the passes are latency-bound)
+  for (uint32_t t0 = lane; t0 < T; t0 += 128) {
+    uint32_t x[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) x[u] = t0 + 32 * u < T ? J[t0 + 32 * u] : 0u;
+#pragma unroll
+    for (int u = 0; u < 4; ++u) if (t0 + 32 * u < T) atomicAdd(&bins[bin_of(x[u])], 1u);
+  }
   __syncwarp();
   {                                          // exclusive scan of the bin counts
     constexpr int PER = kRsBins / 32;
@@ -495,21 +563,37 @@ sort_one_row(const uint32_t* __restrict__ off, int64_t n, int bands, uint32_t to
     for (int q = 0; q < PER; ++q) { bins[lane * PER + q] = run; run += v[q]; }
   }
   __syncwarp();
-  for (uint32_t t = lane; t < T; t += 32) {  // group by bin (arrival order inside a bin)
-    const uint32_t x = J[t];
-    X[atomicAdd(&bins[bin_of(x)], 1u)] = x;
+  for (uint32_t t0 = lane; t0 < T; t0 += 128) {   // group by bin (arrival order inside a bin)
+    uint32_t x[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) x[u] = t0 + 32 * u < T ? J[t0 + 32 * u] : 0u;
+#pragma unroll
+    for (int u = 0; u < 4; ++u) if (t0 + 32 * u < T) X[atomicAdd(&bins[bin_of(x[u])], 1u)] = x[u];
   }
   __syncwarp();                              // now bins[b] = end of bin b = start of bin b+1
-  for (uint32_t t = lane; t < T; t += 32) {  // rank inside the bin -> sorted, back into J
-    const uint32_t x = X[t];
-    const uint32_t b = bin_of(x);
-    const uint32_t s = b ? bins[b - 1] : 0u, e = bins[b];
-    uint32_t r = s;
-    for (uint32_t q = s; q < e; ++q) r += X[q] < x ? 1u : 0u;
-    J[r] = x;
+  for (uint32_t t0 = lane; t0 < T; t0 += 128) {   // rank inside the bin -> sorted, back into J
+    uint32_t x[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) x[u] = t0 + 32 * u < T ? X[t0 + 32 * u] : 0u;
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      if (t0 + 32 * u < T) {
+        const uint32_t b = bin_of(x[u]);
+        const uint32_t s = b ? bins[b - 1] : 0u, e = bins[b];
+        uint32_t r = s;
+        for (uint32_t q = s; q < e; ++q) r += X[q] < x[u] ? 1u : 0u;
+        J[r] = x[u];
+      }
+    }
   }
   __syncwarp();
-  for (uint32_t t = lane; t < T; t += 32) out[base + t] = make_uint2(row, J[t]);
+  for (uint32_t t0 = lane; t0 < T; t0 += 128) {
+    uint32_t x[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) x[u] = t0 + 32 * u < T ? J[t0 + 32 * u] : 0u;
+#pragma unroll
+    for (int u = 0; u < 4; ++u) if (t0 + 32 * u < T) out[base + t0 + 32 * u] = make_uint2(row, x[u]);
+  }
 }
 
 constexpr int kRsChunk = 8;
@@ -535,7 +619,7 @@ row_sort_kernel(const uint32_t* __restrict__ off, int64_t n, int bands, uint32_t
 template <int BW>
 int launch_emit(sq_ctx* c, int mode, const uint2* units, uint32_t nunits, const uint32_t* ids,
                 uint32_t n2, int bands, const uint32_t* S, uint32_t* cnt_off, uint32_t* outJ,
-                uint2* outP) {
+                uint2* outP, const uint32_t* ubase, uint32_t* masks) {
   // persistent warps: exactly the resident blocks of every SM, never more warps than units
   int per_sm = 0;
   cudaError_t e;
@@ -551,13 +635,13 @@ int launch_emit(sq_ctx* c, int mode, const uint2* units, uint32_t nunits, const 
   if (g > need) g = need;
   if (mode == EM_COUNT)
     SQ_TIMED(c, SQ_K_EMIT, emit_kernel<BW, EM_COUNT><<<g, kEmWarps * 32, 0, c->stream>>>(
-        units, nunits, ids, n2, bands, S, cnt_off, outJ, outP));
+        units, nunits, ids, n2, bands, S, cnt_off, outJ, outP, ubase, masks));
   else if (mode == EM_FILL_J)
     SQ_TIMED(c, SQ_K_EMIT, emit_kernel<BW, EM_FILL_J><<<g, kEmWarps * 32, 0, c->stream>>>(
-        units, nunits, ids, n2, bands, S, cnt_off, outJ, outP));
+        units, nunits, ids, n2, bands, S, cnt_off, outJ, outP, ubase, masks));
   else
     SQ_TIMED(c, SQ_K_EMIT, emit_kernel<BW, EM_FILL_PAIRS><<<g, kEmWarps * 32, 0, c->stream>>>(
-        units, nunits, ids, n2, bands, S, cnt_off, outJ, outP));
+        units, nunits, ids, n2, bands, S, cnt_off, outJ, outP, ubase, masks));
   SQ_LAUNCH_CHECK(c);
   return SQ_OK;
 }
@@ -579,18 +663,39 @@ int launch_emit_band0(sq_ctx* c, int mode, const uint2* units0, uint32_t nunits0
   return SQ_OK;
 }
 
-// both unit lists, one mode
+int launch_fill_masks(sq_ctx* c, bool pairs, const uint2* units, uint32_t nunits,
+                      const uint32_t* ubase, const uint32_t* masks, const uint32_t* ids, uint32_t n2,
+                      int bands, const uint32_t* cnt_off, uint32_t* outJ, uint2* outP) {
+  unsigned g = (unsigned)c->sm_count * 16u;          // 64 warps per SM, persistent
+  const unsigned need = (nunits + kEmWarps - 1) / kEmWarps;
+  if (g > need) g = need;
+  if (pairs)
+    SQ_TIMED(c, SQ_K_EMIT, emit_fill_masks_kernel<true><<<g, kEmWarps * 32, 0, c->stream>>>(
+        units, nunits, ubase, masks, ids, n2, bands, cnt_off, outJ, outP));
+  else
+    SQ_TIMED(c, SQ_K_EMIT, emit_fill_masks_kernel<false><<<g, kEmWarps * 32, 0, c->stream>>>(
+        units, nunits, ubase, masks, ids, n2, bands, cnt_off, outJ, outP));
+  SQ_LAUNCH_CHECK(c);
+  return SQ_OK;
+}
+
+// both unit lists, one mode.  `masks` (may be nullptr): the per-tile masks of new pairs, written
+// by the count pass and, when present, read by the fill pass instead of repeating the compares.
 int dispatch_emit(sq_ctx* c, int bw, int mode, const uint2* units, uint32_t nunits,
                   const uint2* units0, uint32_t nunits0, const uint32_t* ids, uint32_t n2, int bands,
-                  const uint32_t* S, uint32_t* cnt_off, uint32_t* outJ, uint2* outP) {
+                  const uint32_t* S, uint32_t* cnt_off, uint32_t* outJ, uint2* outP,
+                  const uint32_t* ubase, uint32_t* masks) {
   int rc = SQ_OK;
   if (nunits0) rc = launch_emit_band0(c, mode, units0, nunits0, ids, bands, cnt_off, outJ, outP);
   if (rc != SQ_OK || nunits == 0) return rc;
+  if (mode != EM_COUNT && masks)
+    return launch_fill_masks(c, mode == EM_FILL_PAIRS, units, nunits, ubase, masks, ids, n2, bands,
+                             cnt_off, outJ, outP);
   switch (bw) {
-    case 1: return launch_emit<1>(c, mode, units, nunits, ids, n2, bands, S, cnt_off, outJ, outP);
-    case 2: return launch_emit<2>(c, mode, units, nunits, ids, n2, bands, S, cnt_off, outJ, outP);
-    case 4: return launch_emit<4>(c, mode, units, nunits, ids, n2, bands, S, cnt_off, outJ, outP);
-    default: return launch_emit<8>(c, mode, units, nunits, ids, n2, bands, S, cnt_off, outJ, outP);
+    case 1: return launch_emit<1>(c, mode, units, nunits, ids, n2, bands, S, cnt_off, outJ, outP, ubase, masks);
+    case 2: return launch_emit<2>(c, mode, units, nunits, ids, n2, bands, S, cnt_off, outJ, outP, ubase, masks);
+    case 4: return launch_emit<4>(c, mode, units, nunits, ids, n2, bands, S, cnt_off, outJ, outP, ubase, masks);
+    default: return launch_emit<8>(c, mode, units, nunits, ids, n2, bands, S, cnt_off, outJ, outP, ubase, masks);
   }
 }
 
@@ -610,6 +715,7 @@ size_t sq_lsh_scratch_bytes(int64_t n, int bands, int64_t pair_capacity) {
   s += sq_align_up((nn + 2) * 4 + 16);         // non-empty flags / ranks
   s += sq_sort_scratch_bytes(n, bands);
   s += sq_align_up((size_t)(pair_capacity > 0 ? pair_capacity : 0) * 4 + 16);   // SORTED: partners
+  s += sq_align_up(rec * 32 + 16);             // mask cache of the count pass (used if it fits)
   return s + 4096;
 }
 
@@ -674,20 +780,25 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
   // a5.1: buckets -> S table + unit list (the unit list lives in the dead key buffer)
   uint2* units = reinterpret_cast<uint2*>(kalt);
   uint2* units0 = units + rec / 2 + 1;           // <= n2/2 units of band 0, <= rec/2 in all
+  uint32_t* ubase = valt;                        // the dead id buffer: one word per unit
   SQ_CUDA(c, cudaMemsetAsync(cnt, 0, (rec + 2) * 4, st));
   {
     dim3 grid((unsigned)((n2 + kBsTile - 1) / kBsTile), (unsigned)bands);
     SQ_TIMED(c, SQ_K_SEGMENT, bucket_scan_kernel<<<grid, kBsThreads, 0, st>>>(
-        kin, vin, n2, bucket_cap, sw, S, units, units0, counters));
+        kin, vin, n2, bucket_cap, sw, S, units, units0, ubase, counters));
     SQ_LAUNCH_CHECK(c);
   }
-  SQ_CUDA(c, cudaMemcpyAsync(c->pinned, counters, 48, cudaMemcpyDeviceToHost, st));
+  SQ_CUDA(c, cudaMemcpyAsync(c->pinned, counters, 64, cudaMemcpyDeviceToHost, st));
   SQ_CUDA(c, cudaStreamSynchronize(st));
   c->last_raw_pairs = (int64_t)c->pinned[1];
   const uint32_t nunits = (uint32_t)c->pinned[4], nunits0 = (uint32_t)c->pinned[5];
   if (nunits + nunits0 == 0) return SQ_OK;
+  // mask cache: 32 words per (unit, column tile); optional -- without it pass 2 repeats the compares
+  const unsigned long long ntiles = c->pinned[7];
+  uint32_t* masks = (nunits && ntiles) ? sq_scratch<uint32_t>(c, (size_t)ntiles * 32) : nullptr;
   // a5.2 pass 1: counts per (sequence, band) -> offsets
-  rc = dispatch_emit(c, bw, EM_COUNT, units, nunits, units0, nunits0, vin, (uint32_t)n2, bands, S, cnt, nullptr, nullptr);
+  rc = dispatch_emit(c, bw, EM_COUNT, units, nunits, units0, nunits0, vin, (uint32_t)n2, bands, S, cnt,
+                     nullptr, nullptr, ubase, masks);
   if (rc != SQ_OK) return rc;
   rc = sq_exclusive_scan_u32(c, cnt, cnt, (int64_t)rec, reinterpret_cast<uint32_t*>(tmp), counters);
   if (rc != SQ_OK) return rc;
@@ -701,12 +812,14 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
   // a5.2 pass 2 (+ a5.3)
   uint2* out = reinterpret_cast<uint2*>(pairs_out);
   if (flags == SQ_LSH_UNORDERED) {
-    rc = dispatch_emit(c, bw, EM_FILL_PAIRS, units, nunits, units0, nunits0, vin, (uint32_t)n2, bands, S, cnt, nullptr, out);
+    rc = dispatch_emit(c, bw, EM_FILL_PAIRS, units, nunits, units0, nunits0, vin, (uint32_t)n2, bands, S, cnt,
+                       nullptr, out, ubase, masks);
     if (rc != SQ_OK) return rc;
   } else {
     uint32_t* tmpJ = sq_scratch<uint32_t>(c, (size_t)uniq);
     if (!tmpJ) return SQ_ERR_WORKSPACE;
-    rc = dispatch_emit(c, bw, EM_FILL_J, units, nunits, units0, nunits0, vin, (uint32_t)n2, bands, S, cnt, tmpJ, nullptr);
+    rc = dispatch_emit(c, bw, EM_FILL_J, units, nunits, units0, nunits0, vin, (uint32_t)n2, bands, S, cnt,
+                       tmpJ, nullptr, ubase, masks);
     if (rc != SQ_OK) return rc;
     int per_sm = 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, row_sort_kernel, kRsWarps * 32, 0) != cudaSuccess ||
