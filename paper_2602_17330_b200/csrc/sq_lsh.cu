@@ -73,6 +73,30 @@ compact_kernel(const uint64_t* __restrict__ keys_in, const uint32_t* __restrict_
   }
 }
 
+// internal row of a sequence = its position in band 0's sorted order (families end up adjacent)
+__global__ void __launch_bounds__(256)
+rowidx_kernel(const uint32_t* __restrict__ ids0, int64_t n2, uint32_t* __restrict__ rowidx) {
+  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p < n2) rowidx[ids0[p]] = (uint32_t)p;
+}
+
+__global__ void __launch_bounds__(256)
+translate_kernel(const uint32_t* __restrict__ ids, int64_t total, const uint32_t* __restrict__ rowidx,
+                 uint32_t* __restrict__ ids_int) {
+  const int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (g < total) ids_int[g] = rowidx[ids[g]];
+}
+
+// partners of every EXTERNAL id (0 for sequences without a signature), to be scanned into ext_off
+__global__ void __launch_bounds__(256)
+ext_count_kernel(const uint32_t* __restrict__ rowidx, const uint32_t* __restrict__ off, int64_t n,
+                 int bands, uint32_t* __restrict__ ext_cnt) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const uint32_t r = rowidx[i];
+  ext_cnt[i] = r == 0xFFFFFFFFu ? 0u : off[((int64_t)r + 1) * bands] - off[(int64_t)r * bands];
+}
+
 // ---------------------------------------------------------------------------------------------
 // a5.1  bucket scan
 // ---------------------------------------------------------------------------------------------
@@ -258,7 +282,7 @@ bucket_scan_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict
 // a5.2  emission: lane = row, columns swept through shared memory
 // ---------------------------------------------------------------------------------------------
 constexpr int kEmWarps = 4;
-enum { EM_COUNT = 0, EM_FILL_J = 1, EM_FILL_PAIRS = 2 };
+enum { EM_COUNT = 0, EM_FILL_J = 1 };
 
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
   const uint32_t s = (uint32_t)__cvta_generic_to_shared(smem);
@@ -272,8 +296,7 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 template <int MODE>
 __global__ void __launch_bounds__(kEmWarps * 32)
 emit_band0_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint32_t* __restrict__ ids,
-                  int bands, uint32_t* __restrict__ cnt_off, uint32_t* __restrict__ outJ,
-                  uint2* __restrict__ outP) {
+                  int bands, uint32_t* __restrict__ cnt_off, uint32_t* __restrict__ outJ) {
   const int lane = threadIdx.x & 31;
   const uint32_t u = blockIdx.x * kEmWarps + (threadIdx.x >> 5);
   if (u >= nunits) return;
@@ -282,19 +305,16 @@ emit_band0_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint32
   const uint32_t* __restrict__ idp = ids + unit.x;
   const uint32_t nrows = min(32u, mrem - 1u);
   const bool rowok = (uint32_t)lane < nrows;
-  const uint32_t myid = rowok ? idp[lane] : 0u;
+  // internal row of a band-0 record = its sorted position: the rows of a unit are consecutive
+  const int64_t myrow = (int64_t)unit.x + lane;
   if (MODE == EM_COUNT) {
-    if (rowok) cnt_off[(int64_t)myid * bands] = mrem - 1u - (uint32_t)lane;
+    if (rowok) cnt_off[myrow * bands] = mrem - 1u - (uint32_t)lane;
     return;
   }
-  const uint32_t off = rowok ? cnt_off[(int64_t)myid * bands] : 0u;
+  const uint32_t off = rowok ? cnt_off[myrow * bands] : 0u;
   for (uint32_t l = 0; l < nrows; ++l) {     // coalesced: the warp writes row l's partners
-    const uint32_t o = __shfl_sync(kFull, off, l), i = __shfl_sync(kFull, myid, l);
-    for (uint32_t cc = l + 1 + lane; cc < mrem; cc += 32) {
-      const uint32_t j = idp[cc];
-      if (MODE == EM_FILL_J) outJ[o + cc - l - 1] = j;
-      else outP[o + cc - l - 1] = make_uint2(i, j);
-    }
+    const uint32_t o = __shfl_sync(kFull, off, l);
+    for (uint32_t cc = l + 1 + lane; cc < mrem; cc += 32) outJ[o + cc - l - 1] = idp[cc];
   }
 }
 
@@ -304,8 +324,7 @@ __device__ __forceinline__ void sweep_tile(const uint32_t* __restrict__ sm,
                                            const uint32_t* __restrict__ idt, const uint4 (&R)[BW],
                                            uint32_t cbeg, uint32_t ncol, uint32_t c0, uint32_t lane,
                                            bool rowok, uint32_t myid, uint32_t& acc,
-                                           uint32_t& tmask, uint32_t* __restrict__ outJ,
-                                           uint2* __restrict__ outP) {
+                                           uint32_t& tmask, uint32_t* __restrict__ outJ) {
   constexpr int RS = 4 * BW + 4;
   if constexpr (NCH <= BW) {
 #pragma unroll 4
@@ -320,8 +339,7 @@ __device__ __forceinline__ void sweep_tile(const uint32_t* __restrict__ sm,
       if (MODE == EM_COUNT) {
         tmask |= isnew ? (1u << c) : 0u;
       } else if (isnew) {
-        const uint32_t j = idt[c];
-        if (MODE == EM_FILL_J) outJ[acc] = j; else outP[acc] = make_uint2(myid, j);
+        outJ[acc] = idt[c];
         ++acc;
       }
     }
@@ -334,15 +352,17 @@ struct EmDesc { uint32_t u, g0, mrem, c0; int b; bool ok; };
 // items is software-pipelined: ids two tiles ahead (registers), S rows one tile ahead
 // (cp.async into the other shared-memory buffer), compares on the current tile.
 // BW = 16-byte chunks per S row (S row width SW = 4*BW >= bands).
-// MODE EM_COUNT:      cnt[id*bands + b] = number of NEW partners of row id in band b.
-// MODE EM_FILL_J:     outJ[off[id*bands + b] + t] = t-th new partner (ascending).
-// MODE EM_FILL_PAIRS: outP[...] = (id, partner).
+// ids = external sequence ids of the sorted records (the values that are emitted); ids_int =
+// their internal rows (position in band 0's sorted order), which index S and the counts.
+// MODE EM_COUNT:  cnt[row*bands + b] = number of NEW partners of internal row `row` in band b.
+// MODE EM_FILL_J: outJ[off[row*bands + b] + t] = external id of the t-th new partner.
 template <int BW, int MODE>
 __global__ void __launch_bounds__(kEmWarps * 32)
 emit_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint32_t* __restrict__ ids,
-            uint32_t n2, int bands, const uint32_t* __restrict__ S, uint32_t* __restrict__ cnt_off,
-            uint32_t* __restrict__ outJ, uint2* __restrict__ outP,
-            const uint32_t* __restrict__ ubase, uint32_t* __restrict__ masks) {
+            const uint32_t* __restrict__ ids_int, uint32_t n2, int bands,
+            const uint32_t* __restrict__ S, uint32_t* __restrict__ cnt_off,
+            uint32_t* __restrict__ outJ, const uint32_t* __restrict__ ubase,
+            uint32_t* __restrict__ masks) {
   constexpr int SW = 4 * BW;
   constexpr int RS = SW + 4;                 // shared row stride in words (16-byte aligned)
   constexpr int RPR = 32 / BW;               // S rows fetched per load round
@@ -364,8 +384,11 @@ emit_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint32_t* __
     if (r.ok && r.u + nw < nunits) unit_pref = units[r.u + nw];
     return r;
   };
-  auto load_ids = [&](const EmDesc& d) -> uint32_t {
-    return (d.ok && d.c0 + lane < d.mrem) ? ids[(int64_t)d.g0 + d.c0 + lane] : 0u;
+  auto load_ids = [&](const EmDesc& d) -> uint32_t {          // internal rows of a column tile
+    return (d.ok && d.c0 + lane < d.mrem) ? ids_int[(int64_t)d.g0 + d.c0 + lane] : 0u;
+  };
+  auto load_ext = [&](const EmDesc& d) -> uint32_t {          // external ids (fill mode only)
+    return (MODE != EM_COUNT && d.ok && d.c0 + lane < d.mrem) ? ids[(int64_t)d.g0 + d.c0 + lane] : 0u;
   };
   auto issue_rows = [&](const EmDesc& d, uint32_t idc, uint32_t* sm) {
     const uint32_t ncol = min(32u, d.mrem - d.c0);
@@ -382,9 +405,9 @@ emit_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint32_t* __
   EmDesc dc;                                  // current tile
   dc.u = wg - nw; dc.ok = true; dc.mrem = 0; dc.c0 = 0; dc.g0 = 0; dc.b = 0;
   dc = next_desc(dc);
-  uint32_t idc_c = load_ids(dc);
+  uint32_t idc_c = load_ids(dc), idx_c = load_ext(dc);
   EmDesc dn = next_desc(dc);                  // next tile
-  uint32_t idc_n = load_ids(dn);
+  uint32_t idc_n = load_ids(dn), idx_n = load_ext(dn);
   issue_rows(dc, idc_c, Sm[w][0]);
   cp_async_commit();
 
@@ -396,7 +419,7 @@ emit_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint32_t* __
     if (dn.ok) issue_rows(dn, idc_n, Sm[w][(k + 1) & 1]);
     cp_async_commit();
     const EmDesc d2 = next_desc(dn);
-    const uint32_t id2 = load_ids(d2);
+    const uint32_t id2 = load_ids(d2), ix2 = load_ext(d2);
     cp_async_wait<1>();
     __syncwarp();
     const uint32_t* sm = Sm[w][k & 1];
@@ -418,20 +441,20 @@ emit_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint32_t* __
         }
       }
     }
-    if (MODE != EM_COUNT) { idsm[w][k & 1][lane] = idc_c; __syncwarp(); }
+    if (MODE != EM_COUNT) { idsm[w][k & 1][lane] = idx_c; __syncwarp(); }
     const uint32_t ncol = min(32u, dc.mrem - dc.c0);
     const uint32_t cbeg = dc.c0 == 0 ? 1u : 0u;
     const uint32_t* idt = idsm[w][k & 1];
     uint32_t tmask = 0;                       // EM_COUNT: bit c = pair (my row, column c) is new
     switch ((b + 3) >> 2) {
-      case 1: sweep_tile<BW, 1, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, tmask, outJ, outP); break;
-      case 2: sweep_tile<BW, 2, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, tmask, outJ, outP); break;
-      case 3: sweep_tile<BW, 3, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, tmask, outJ, outP); break;
-      case 4: sweep_tile<BW, 4, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, tmask, outJ, outP); break;
-      case 5: sweep_tile<BW, 5, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, tmask, outJ, outP); break;
-      case 6: sweep_tile<BW, 6, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, tmask, outJ, outP); break;
-      case 7: sweep_tile<BW, 7, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, tmask, outJ, outP); break;
-      default: sweep_tile<BW, 8, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, tmask, outJ, outP); break;
+      case 1: sweep_tile<BW, 1, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, tmask, outJ); break;
+      case 2: sweep_tile<BW, 2, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, tmask, outJ); break;
+      case 3: sweep_tile<BW, 3, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, tmask, outJ); break;
+      case 4: sweep_tile<BW, 4, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, tmask, outJ); break;
+      case 5: sweep_tile<BW, 5, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, tmask, outJ); break;
+      case 6: sweep_tile<BW, 6, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, tmask, outJ); break;
+      case 7: sweep_tile<BW, 7, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, tmask, outJ); break;
+      default: sweep_tile<BW, 8, MODE>(sm, idt, R, cbeg, ncol, dc.c0, lane, rowok, myid, acc, tmask, outJ); break;
     }
     if (MODE == EM_COUNT) {
       acc += __popc(tmask);
@@ -439,7 +462,7 @@ emit_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint32_t* __
       if (rowok && dc.c0 + 32 >= dc.mrem) cnt_off[(int64_t)myid * bands + b] = acc;
     }
     __syncwarp();
-    dc = dn; idc_c = idc_n; dn = d2; idc_n = id2; ++k;
+    dc = dn; idc_c = idc_n; idx_c = idx_n; dn = d2; idc_n = id2; idx_n = ix2; ++k;
   }
   cp_async_wait<0>();
 }
@@ -448,13 +471,12 @@ emit_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint32_t* __
 // (persistent) warp per unit walks the unit's tiles; lane = row holds the mask of its new columns
 // of the tile and the id of column `lane`; every round each lane with a bit left takes its next
 // column's id from the owning lane (SHFL) and appends it to its row's output.
-template <bool PAIRS>
 __global__ void __launch_bounds__(kEmWarps * 32)
 emit_fill_masks_kernel(const uint2* __restrict__ units, uint32_t nunits,
                        const uint32_t* __restrict__ ubase, const uint32_t* __restrict__ masks,
-                       const uint32_t* __restrict__ ids, uint32_t n2, int bands,
-                       const uint32_t* __restrict__ cnt_off, uint32_t* __restrict__ outJ,
-                       uint2* __restrict__ outP) {
+                       const uint32_t* __restrict__ ids, const uint32_t* __restrict__ ids_int,
+                       uint32_t n2, int bands, const uint32_t* __restrict__ cnt_off,
+                       uint32_t* __restrict__ outJ) {
   const uint32_t lane = threadIdx.x & 31;
   const uint32_t nw = gridDim.x * kEmWarps;
   for (uint32_t u = blockIdx.x * kEmWarps + (threadIdx.x >> 5); u < nunits; u += nw) {
@@ -464,7 +486,8 @@ emit_fill_masks_kernel(const uint2* __restrict__ units, uint32_t nunits,
     const uint32_t* __restrict__ idp = ids + g0;
     const uint32_t* __restrict__ mp = masks + (size_t)ubase[u] * 32 + lane;
     const uint32_t myid = lane < mrem ? idp[lane] : 0u;
-    uint32_t acc = lane < min(32u, mrem - 1u) ? cnt_off[(int64_t)myid * bands + b] : 0u;
+    uint32_t acc = 0;
+    if (lane < min(32u, mrem - 1u)) acc = cnt_off[(int64_t)ids_int[g0 + lane] * bands + b];
     uint32_t mask = mp[0], idc = myid;
     for (uint32_t c0 = 0; c0 < mrem; c0 += 32) {
       uint32_t mask_n = 0, idc_n = 0;            // next tile, in flight during this one
@@ -476,7 +499,7 @@ emit_fill_masks_kernel(const uint2* __restrict__ units, uint32_t nunits,
         const int c = mask ? __ffs(mask) - 1 : 0;
         const uint32_t j = __shfl_sync(kFull, idc, c);
         if (mask) {
-          if (PAIRS) outP[acc] = make_uint2(myid, j); else outJ[acc] = j;
+          outJ[acc] = j;
           ++acc;
           mask &= mask - 1;
         }
@@ -489,7 +512,9 @@ emit_fill_masks_kernel(const uint2* __restrict__ units, uint32_t nunits,
 // ---------------------------------------------------------------------------------------------
 // a5.3  SQ_LSH_SORTED: put every row's partners in ascending order
 // ---------------------------------------------------------------------------------------------
-// One warp per row.  The row's partners sit in inJ[base, base+T) as <= B ascending groups.  The
+// One warp per INTERNAL row r (rows are visited in band 0's sorted order, i.e. family by family,
+// and written to the slice of `out` that belongs to the row's EXTERNAL id: ext_off).  The row's
+// partners (external ids) sit in inJ[base, base+T) as <= B ascending groups.  The
 // ids of a repertoire carry no structure, so the partners of a row are spread evenly between the
 // row's smallest and largest partner: ONE most-significant-digit pass over kRsBins equal-width
 // value bins (shared-memory counters) groups them, and an element's final place is its bin's
@@ -500,11 +525,11 @@ constexpr int kRsWarps = 8;
 constexpr int kRsBins = 1024;
 
 __device__ __forceinline__ void
-sort_one_row(const uint32_t* __restrict__ off, int64_t n, int bands, uint32_t total,
-             uint32_t* inJ, uint2* out, int64_t i, uint32_t* bins, int lane) {
+sort_one_row(const uint32_t* __restrict__ off, int bands, uint32_t* inJ, uint2* out, int64_t r,
+             uint32_t row, uint32_t obase, bool do_sort, uint32_t* bins, int lane) {
   // lane b holds the start of group b; the lanes past `bands` hold the row end
-  const uint32_t row_end = (i + 1 < n) ? off[(i + 1) * bands] : total;
-  const uint32_t gs = lane < bands ? off[i * bands + lane] : row_end;
+  const uint32_t row_end = off[(r + 1) * bands];
+  const uint32_t gs = lane < bands ? off[r * bands + lane] : row_end;
   uint32_t ge = __shfl_down_sync(kFull, gs, 1);
   if (lane == 31 || lane + 1 >= bands) ge = row_end;
   const uint32_t base = __shfl_sync(kFull, gs, 0);
@@ -512,17 +537,17 @@ sort_one_row(const uint32_t* __restrict__ off, int64_t n, int bands, uint32_t to
   if (T == 0) return;
   const bool has = lane < bands && ge > gs;
   const uint32_t nonempty = __ballot_sync(kFull, has);
-  const uint32_t row = (uint32_t)i;
   uint32_t* J = inJ + base;
-  if (__popc(nonempty) == 1) {               // already ascending
-    for (uint32_t t = lane; t < T; t += 32) out[base + t] = make_uint2(row, J[t]);
+  out += obase;                              // the row's slice of the output
+  if (__popc(nonempty) == 1 || !do_sort) {   // already ascending, or the grouped order is asked for
+    for (uint32_t t = lane; t < T; t += 32) out[t] = make_uint2(row, J[t]);
     return;
   }
   if (T <= 32) {                             // rank by counting inside the warp
     const uint32_t x = (uint32_t)lane < T ? J[lane] : kFull;
     uint32_t rank = 0;
     for (uint32_t s = 0; s < T; ++s) rank += __shfl_sync(kFull, x, s) < x ? 1u : 0u;
-    if ((uint32_t)lane < T) out[base + rank] = make_uint2(row, x);
+    if ((uint32_t)lane < T) out[rank] = make_uint2(row, x);
     return;
   }
   // value range of the row: every group is ascending, so its ends are its extremes
@@ -533,7 +558,7 @@ sort_one_row(const uint32_t* __restrict__ off, int64_t n, int bands, uint32_t to
   auto bin_of = [&](uint32_t x) -> uint32_t {     // monotone in x, < kRsBins
     return min((uint32_t)kRsBins - 1u, (uint32_t)((float)(x - lo) * scale));
   };
-  uint32_t* X = reinterpret_cast<uint32_t*>(out + base);     // scratch: first T words of the slice
+  uint32_t* X = reinterpret_cast<uint32_t*>(out);            // scratch: first T words of the slice
 #pragma unroll
   for (int q = 0; q < kRsBins / 128; ++q)
     *reinterpret_cast<uint4*>(bins + q * 128 + lane * 4) = make_uint4(0, 0, 0, 0);
@@ -592,15 +617,17 @@ sort_one_row(const uint32_t* __restrict__ off, int64_t n, int bands, uint32_t to
 #pragma unroll
     for (int u = 0; u < 4; ++u) x[u] = t0 + 32 * u < T ? J[t0 + 32 * u] : 0u;
 #pragma unroll
-    for (int u = 0; u < 4; ++u) if (t0 + 32 * u < T) out[base + t0 + 32 * u] = make_uint2(row, x[u]);
+    for (int u = 0; u < 4; ++u) if (t0 + 32 * u < T) out[t0 + 32 * u] = make_uint2(row, x[u]);
   }
 }
 
 constexpr int kRsChunk = 8;
 
 __global__ void __launch_bounds__(kRsWarps * 32)
-row_sort_kernel(const uint32_t* __restrict__ off, int64_t n, int bands, uint32_t total,
-                uint32_t* inJ, uint2* out, unsigned long long* __restrict__ next_row) {
+row_sort_kernel(const uint32_t* __restrict__ off, int64_t n2, int bands,
+                const uint32_t* __restrict__ ids0, const uint32_t* __restrict__ ext_off,
+                bool do_sort, uint32_t* inJ, uint2* out,
+                unsigned long long* __restrict__ next_row) {
   __shared__ uint32_t bins_sh[kRsWarps][kRsBins];
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   // Rows differ by four orders of magnitude in size: persistent warps fetch rows kRsChunk at a
@@ -609,72 +636,61 @@ row_sort_kernel(const uint32_t* __restrict__ off, int64_t n, int bands, uint32_t
     unsigned long long first = 0;
     if (lane == 0) first = atomicAdd(next_row, (unsigned long long)kRsChunk);
     first = __shfl_sync(kFull, first, 0);
-    if ((int64_t)first >= n) return;
-    const int64_t last = min(n, (int64_t)first + kRsChunk);
-    for (int64_t i = (int64_t)first; i < last; ++i)
-      sort_one_row(off, n, bands, total, inJ, out, i, bins_sh[w], lane);
+    if ((int64_t)first >= n2) return;
+    const int64_t last = min(n2, (int64_t)first + kRsChunk);
+    for (int64_t r = (int64_t)first; r < last; ++r) {
+      const uint32_t i = ids0[r];            // external id of internal row r
+      sort_one_row(off, bands, inJ, out, r, i, ext_off[i], do_sort, bins_sh[w], lane);
+    }
   }
 }
 
 template <int BW>
 int launch_emit(sq_ctx* c, int mode, const uint2* units, uint32_t nunits, const uint32_t* ids,
-                uint32_t n2, int bands, const uint32_t* S, uint32_t* cnt_off, uint32_t* outJ,
-                uint2* outP, const uint32_t* ubase, uint32_t* masks) {
+                const uint32_t* ids_int, uint32_t n2, int bands, const uint32_t* S,
+                uint32_t* cnt_off, uint32_t* outJ, const uint32_t* ubase, uint32_t* masks) {
   // persistent warps: exactly the resident blocks of every SM, never more warps than units
   int per_sm = 0;
   cudaError_t e;
   if (mode == EM_COUNT)
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, emit_kernel<BW, EM_COUNT>, kEmWarps * 32, 0);
-  else if (mode == EM_FILL_J)
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, emit_kernel<BW, EM_FILL_J>, kEmWarps * 32, 0);
   else
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, emit_kernel<BW, EM_FILL_PAIRS>, kEmWarps * 32, 0);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, emit_kernel<BW, EM_FILL_J>, kEmWarps * 32, 0);
   if (e != cudaSuccess || per_sm < 1) per_sm = 4;
   unsigned g = (unsigned)(c->sm_count * per_sm);
   const unsigned need = (nunits + kEmWarps - 1) / kEmWarps;
   if (g > need) g = need;
   if (mode == EM_COUNT)
     SQ_TIMED(c, SQ_K_EMIT, emit_kernel<BW, EM_COUNT><<<g, kEmWarps * 32, 0, c->stream>>>(
-        units, nunits, ids, n2, bands, S, cnt_off, outJ, outP, ubase, masks));
-  else if (mode == EM_FILL_J)
-    SQ_TIMED(c, SQ_K_EMIT, emit_kernel<BW, EM_FILL_J><<<g, kEmWarps * 32, 0, c->stream>>>(
-        units, nunits, ids, n2, bands, S, cnt_off, outJ, outP, ubase, masks));
+        units, nunits, ids, ids_int, n2, bands, S, cnt_off, outJ, ubase, masks));
   else
-    SQ_TIMED(c, SQ_K_EMIT, emit_kernel<BW, EM_FILL_PAIRS><<<g, kEmWarps * 32, 0, c->stream>>>(
-        units, nunits, ids, n2, bands, S, cnt_off, outJ, outP, ubase, masks));
+    SQ_TIMED(c, SQ_K_EMIT, emit_kernel<BW, EM_FILL_J><<<g, kEmWarps * 32, 0, c->stream>>>(
+        units, nunits, ids, ids_int, n2, bands, S, cnt_off, outJ, ubase, masks));
   SQ_LAUNCH_CHECK(c);
   return SQ_OK;
 }
 
 int launch_emit_band0(sq_ctx* c, int mode, const uint2* units0, uint32_t nunits0,
-                      const uint32_t* ids, int bands, uint32_t* cnt_off, uint32_t* outJ,
-                      uint2* outP) {
+                      const uint32_t* ids, int bands, uint32_t* cnt_off, uint32_t* outJ) {
   const unsigned g = (nunits0 + kEmWarps - 1) / kEmWarps;
   if (mode == EM_COUNT)
     SQ_TIMED(c, SQ_K_EMIT, emit_band0_kernel<EM_COUNT><<<g, kEmWarps * 32, 0, c->stream>>>(
-        units0, nunits0, ids, bands, cnt_off, outJ, outP));
-  else if (mode == EM_FILL_J)
-    SQ_TIMED(c, SQ_K_EMIT, emit_band0_kernel<EM_FILL_J><<<g, kEmWarps * 32, 0, c->stream>>>(
-        units0, nunits0, ids, bands, cnt_off, outJ, outP));
+        units0, nunits0, ids, bands, cnt_off, outJ));
   else
-    SQ_TIMED(c, SQ_K_EMIT, emit_band0_kernel<EM_FILL_PAIRS><<<g, kEmWarps * 32, 0, c->stream>>>(
-        units0, nunits0, ids, bands, cnt_off, outJ, outP));
+    SQ_TIMED(c, SQ_K_EMIT, emit_band0_kernel<EM_FILL_J><<<g, kEmWarps * 32, 0, c->stream>>>(
+        units0, nunits0, ids, bands, cnt_off, outJ));
   SQ_LAUNCH_CHECK(c);
   return SQ_OK;
 }
 
-int launch_fill_masks(sq_ctx* c, bool pairs, const uint2* units, uint32_t nunits,
-                      const uint32_t* ubase, const uint32_t* masks, const uint32_t* ids, uint32_t n2,
-                      int bands, const uint32_t* cnt_off, uint32_t* outJ, uint2* outP) {
+int launch_fill_masks(sq_ctx* c, const uint2* units, uint32_t nunits, const uint32_t* ubase,
+                      const uint32_t* masks, const uint32_t* ids, const uint32_t* ids_int,
+                      uint32_t n2, int bands, const uint32_t* cnt_off, uint32_t* outJ) {
   unsigned g = (unsigned)c->sm_count * 16u;          // 64 warps per SM, persistent
   const unsigned need = (nunits + kEmWarps - 1) / kEmWarps;
   if (g > need) g = need;
-  if (pairs)
-    SQ_TIMED(c, SQ_K_EMIT, emit_fill_masks_kernel<true><<<g, kEmWarps * 32, 0, c->stream>>>(
-        units, nunits, ubase, masks, ids, n2, bands, cnt_off, outJ, outP));
-  else
-    SQ_TIMED(c, SQ_K_EMIT, emit_fill_masks_kernel<false><<<g, kEmWarps * 32, 0, c->stream>>>(
-        units, nunits, ubase, masks, ids, n2, bands, cnt_off, outJ, outP));
+  SQ_TIMED(c, SQ_K_EMIT, emit_fill_masks_kernel<<<g, kEmWarps * 32, 0, c->stream>>>(
+      units, nunits, ubase, masks, ids, ids_int, n2, bands, cnt_off, outJ));
   SQ_LAUNCH_CHECK(c);
   return SQ_OK;
 }
@@ -682,20 +698,19 @@ int launch_fill_masks(sq_ctx* c, bool pairs, const uint2* units, uint32_t nunits
 // both unit lists, one mode.  `masks` (may be nullptr): the per-tile masks of new pairs, written
 // by the count pass and, when present, read by the fill pass instead of repeating the compares.
 int dispatch_emit(sq_ctx* c, int bw, int mode, const uint2* units, uint32_t nunits,
-                  const uint2* units0, uint32_t nunits0, const uint32_t* ids, uint32_t n2, int bands,
-                  const uint32_t* S, uint32_t* cnt_off, uint32_t* outJ, uint2* outP,
-                  const uint32_t* ubase, uint32_t* masks) {
+                  const uint2* units0, uint32_t nunits0, const uint32_t* ids,
+                  const uint32_t* ids_int, uint32_t n2, int bands, const uint32_t* S,
+                  uint32_t* cnt_off, uint32_t* outJ, const uint32_t* ubase, uint32_t* masks) {
   int rc = SQ_OK;
-  if (nunits0) rc = launch_emit_band0(c, mode, units0, nunits0, ids, bands, cnt_off, outJ, outP);
+  if (nunits0) rc = launch_emit_band0(c, mode, units0, nunits0, ids, bands, cnt_off, outJ);
   if (rc != SQ_OK || nunits == 0) return rc;
   if (mode != EM_COUNT && masks)
-    return launch_fill_masks(c, mode == EM_FILL_PAIRS, units, nunits, ubase, masks, ids, n2, bands,
-                             cnt_off, outJ, outP);
+    return launch_fill_masks(c, units, nunits, ubase, masks, ids, ids_int, n2, bands, cnt_off, outJ);
   switch (bw) {
-    case 1: return launch_emit<1>(c, mode, units, nunits, ids, n2, bands, S, cnt_off, outJ, outP, ubase, masks);
-    case 2: return launch_emit<2>(c, mode, units, nunits, ids, n2, bands, S, cnt_off, outJ, outP, ubase, masks);
-    case 4: return launch_emit<4>(c, mode, units, nunits, ids, n2, bands, S, cnt_off, outJ, outP, ubase, masks);
-    default: return launch_emit<8>(c, mode, units, nunits, ids, n2, bands, S, cnt_off, outJ, outP, ubase, masks);
+    case 1: return launch_emit<1>(c, mode, units, nunits, ids, ids_int, n2, bands, S, cnt_off, outJ, ubase, masks);
+    case 2: return launch_emit<2>(c, mode, units, nunits, ids, ids_int, n2, bands, S, cnt_off, outJ, ubase, masks);
+    case 4: return launch_emit<4>(c, mode, units, nunits, ids, ids_int, n2, bands, S, cnt_off, outJ, ubase, masks);
+    default: return launch_emit<8>(c, mode, units, nunits, ids, ids_int, n2, bands, S, cnt_off, outJ, ubase, masks);
   }
 }
 
@@ -708,13 +723,14 @@ size_t sq_lsh_scratch_bytes(int64_t n, int bands, int64_t pair_capacity) {
   const size_t rec = nn * B;
   const size_t sw = 4 * (size_t)chunks_for((int)B);
   size_t s = 0;
-  s += 2 * sq_align_up(rec * 8 + 16);          // keys ping-pong (the unit list reuses one)
-  s += 2 * sq_align_up(rec * 4 + 16);          // ids ping-pong
+  s += 2 * sq_align_up(rec * 8 + 16);          // keys ping-pong (the unit lists reuse one)
+  s += 2 * sq_align_up(rec * 4 + 16);          // ids ping-pong (the internal rows reuse one)
   s += sq_align_up(nn * sw * 4 + 16);          // bucket-id table S
-  s += sq_align_up((rec + 2) * 4 + 16);        // per (sequence, band) counts -> offsets
-  s += sq_align_up((nn + 2) * 4 + 16);         // non-empty flags / ranks
+  s += sq_align_up((rec + 2) * 4 + 16);        // per (row, band) counts -> offsets
+  s += sq_align_up((rec / 2 + 2) * 4 + 16);    // first mask tile of every unit
+  s += 3 * sq_align_up((nn + 2) * 4 + 16);     // non-empty flags / ranks; rowidx; ext_off
   s += sq_sort_scratch_bytes(n, bands);
-  s += sq_align_up((size_t)(pair_capacity > 0 ? pair_capacity : 0) * 4 + 16);   // SORTED: partners
+  s += sq_align_up((size_t)(pair_capacity > 0 ? pair_capacity : 0) * 4 + 16);   // partners
   s += sq_align_up(rec * 32 + 16);             // mask cache of the count pass (used if it fits)
   return s + 4096;
 }
@@ -744,9 +760,13 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
   uint32_t* v1 = sq_scratch<uint32_t>(c, rec);
   uint32_t* S = sq_scratch<uint32_t>(c, (size_t)n * sw);
   uint32_t* cnt = sq_scratch<uint32_t>(c, rec + 2);
+  uint32_t* ubase = sq_scratch<uint32_t>(c, rec / 2 + 2);
   uint32_t* nonempty = sq_scratch<uint32_t>(c, (size_t)n + 2);
+  uint32_t* rowidx = sq_scratch<uint32_t>(c, (size_t)n + 2);
+  uint32_t* ext_off = sq_scratch<uint32_t>(c, (size_t)n + 2);
   uint8_t* tmp = sq_scratch<uint8_t>(c, sq_sort_scratch_bytes(n, bands));
-  if (!k0 || !k1 || !v0 || !v1 || !S || !cnt || !nonempty || !tmp) return SQ_ERR_WORKSPACE;
+  if (!k0 || !k1 || !v0 || !v1 || !S || !cnt || !ubase || !nonempty || !rowidx || !ext_off || !tmp)
+    return SQ_ERR_WORKSPACE;
   cudaStream_t st = c->stream;
   unsigned long long* counters = c->dflags;      // [0] unique, [1] raw, [2] n2, [4] units
   SQ_CUDA(c, cudaMemsetAsync(counters, 0, 64, st));
@@ -777,15 +797,23 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
     if (rc != SQ_OK) return rc;
     if (in_alt) { uint64_t* t = kin; kin = kalt; kalt = t; uint32_t* tv = vin; vin = valt; valt = tv; }
   }
-  // a5.1: buckets -> S table + unit list (the unit list lives in the dead key buffer)
+  // internal rows: position in band 0's sorted order (band 0's records are vin[0, n2))
+  const int64_t total = n2 * bands;
+  const unsigned gt = (unsigned)((total + 255) / 256);
+  uint32_t* vint = valt;                         // the dead id buffer: internal row of every record
+  SQ_CUDA(c, cudaMemsetAsync(rowidx, 0xFF, (size_t)n * 4, st));
+  SQ_TIMED(c, SQ_K_SEGMENT, rowidx_kernel<<<(unsigned)((n2 + 255) / 256), 256, 0, st>>>(vin, n2, rowidx));
+  SQ_LAUNCH_CHECK(c);
+  SQ_TIMED(c, SQ_K_SEGMENT, translate_kernel<<<gt, 256, 0, st>>>(vin, total, rowidx, vint));
+  SQ_LAUNCH_CHECK(c);
+  // a5.1: buckets -> S table + unit lists (the unit lists live in the dead key buffer)
   uint2* units = reinterpret_cast<uint2*>(kalt);
   uint2* units0 = units + rec / 2 + 1;           // <= n2/2 units of band 0, <= rec/2 in all
-  uint32_t* ubase = valt;                        // the dead id buffer: one word per unit
   SQ_CUDA(c, cudaMemsetAsync(cnt, 0, (rec + 2) * 4, st));
   {
     dim3 grid((unsigned)((n2 + kBsTile - 1) / kBsTile), (unsigned)bands);
     SQ_TIMED(c, SQ_K_SEGMENT, bucket_scan_kernel<<<grid, kBsThreads, 0, st>>>(
-        kin, vin, n2, bucket_cap, sw, S, units, units0, ubase, counters));
+        kin, vint, n2, bucket_cap, sw, S, units, units0, ubase, counters));
     SQ_LAUNCH_CHECK(c);
   }
   SQ_CUDA(c, cudaMemcpyAsync(c->pinned, counters, 64, cudaMemcpyDeviceToHost, st));
@@ -796,11 +824,11 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
   // mask cache: 32 words per (unit, column tile); optional -- without it pass 2 repeats the compares
   const unsigned long long ntiles = c->pinned[7];
   uint32_t* masks = (nunits && ntiles) ? sq_scratch<uint32_t>(c, (size_t)ntiles * 32) : nullptr;
-  // a5.2 pass 1: counts per (sequence, band) -> offsets
-  rc = dispatch_emit(c, bw, EM_COUNT, units, nunits, units0, nunits0, vin, (uint32_t)n2, bands, S, cnt,
-                     nullptr, nullptr, ubase, masks);
+  // a5.2 pass 1: counts per (internal row, band) -> offsets
+  rc = dispatch_emit(c, bw, EM_COUNT, units, nunits, units0, nunits0, vin, vint, (uint32_t)n2, bands, S,
+                     cnt, nullptr, ubase, masks);
   if (rc != SQ_OK) return rc;
-  rc = sq_exclusive_scan_u32(c, cnt, cnt, (int64_t)rec, reinterpret_cast<uint32_t*>(tmp), counters);
+  rc = sq_exclusive_scan_u32(c, cnt, cnt, (int64_t)rec + 1, reinterpret_cast<uint32_t*>(tmp), counters);
   if (rc != SQ_OK) return rc;
   SQ_CUDA(c, cudaMemcpyAsync(c->pinned, counters, 8, cudaMemcpyDeviceToHost, st));
   SQ_CUDA(c, cudaStreamSynchronize(st));
@@ -809,28 +837,30 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
   if (uniq > capacity) return SQ_ERR_CAPACITY;
   if (uniq >= (1ll << 32) - 1) return SQ_ERR_UNSUPPORTED;   // 32-bit output offsets
   if (uniq == 0) return SQ_OK;
-  // a5.2 pass 2 (+ a5.3)
-  uint2* out = reinterpret_cast<uint2*>(pairs_out);
-  if (flags == SQ_LSH_UNORDERED) {
-    rc = dispatch_emit(c, bw, EM_FILL_PAIRS, units, nunits, units0, nunits0, vin, (uint32_t)n2, bands, S, cnt,
-                       nullptr, out, ubase, masks);
-    if (rc != SQ_OK) return rc;
-  } else {
-    uint32_t* tmpJ = sq_scratch<uint32_t>(c, (size_t)uniq);
-    if (!tmpJ) return SQ_ERR_WORKSPACE;
-    rc = dispatch_emit(c, bw, EM_FILL_J, units, nunits, units0, nunits0, vin, (uint32_t)n2, bands, S, cnt,
-                       tmpJ, nullptr, ubase, masks);
-    if (rc != SQ_OK) return rc;
+  // where every EXTERNAL row starts in the output
+  SQ_TIMED(c, SQ_K_SEGMENT, ext_count_kernel<<<gb, 256, 0, st>>>(rowidx, cnt, n, bands, ext_off));
+  SQ_LAUNCH_CHECK(c);
+  rc = sq_exclusive_scan_u32(c, ext_off, ext_off, n, reinterpret_cast<uint32_t*>(tmp), nullptr);
+  if (rc != SQ_OK) return rc;
+  // a5.2 pass 2: the partners of every internal row, grouped by band, into the partner scratch
+  uint32_t* tmpJ = sq_scratch<uint32_t>(c, (size_t)uniq);
+  if (!tmpJ) return SQ_ERR_WORKSPACE;
+  rc = dispatch_emit(c, bw, EM_FILL_J, units, nunits, units0, nunits0, vin, vint, (uint32_t)n2, bands, S,
+                     cnt, tmpJ, ubase, masks);
+  if (rc != SQ_OK) return rc;
+  // a5.3: every row (sorted if asked) into its slice of the output
+  {
     int per_sm = 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, row_sort_kernel, kRsWarps * 32, 0) != cudaSuccess ||
         per_sm < 1)
       per_sm = 2;
     unsigned g = (unsigned)(c->sm_count * per_sm);
-    const unsigned need = (unsigned)((n + kRsWarps * kRsChunk - 1) / (kRsWarps * kRsChunk));
+    const unsigned need = (unsigned)((n2 + kRsWarps * kRsChunk - 1) / (kRsWarps * kRsChunk));
     if (g > need) g = need;
     SQ_CUDA(c, cudaMemsetAsync(counters + 6, 0, 8, st));
     SQ_TIMED(c, SQ_K_ROWSORT, row_sort_kernel<<<g, kRsWarps * 32, 0, st>>>(
-        cnt, n, bands, (uint32_t)uniq, tmpJ, out, counters + 6));
+        cnt, n2, bands, vin, ext_off, flags == SQ_LSH_SORTED, tmpJ, reinterpret_cast<uint2*>(pairs_out),
+        counters + 6));
     SQ_LAUNCH_CHECK(c);
   }
   SQ_CUDA(c, cudaStreamSynchronize(st));
