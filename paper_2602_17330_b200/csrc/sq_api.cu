@@ -46,6 +46,7 @@ int sq_set_workspace(sq_ctx* c, void* dev_ptr, size_t bytes) {
   c->n = -1;
   c->packed = nullptr;
   c->order = nullptr;
+  c->sched = nullptr;
   return SQ_OK;
 }
 

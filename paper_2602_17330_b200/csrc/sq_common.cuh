@@ -32,6 +32,17 @@ struct sq_ctx {
   int alphabet = 0;
   uint8_t* packed = nullptr;    // [n][stride]
   uint32_t* order = nullptr;    // [n] sequence ids, longest first (processing order of the sketch)
+  // Family-ordered schedule of the last sq_lsh_candidates output, a performance hint for
+  // sq_edit_distance: chunk k = the pairs at positions [32k, 32k+32) of the INTERNAL row order
+  // (band 0's sorted order, family by family); sched[k] = (first row r0, delta[r0],
+  // rowstart[r0+1], -), position q of row r is pair delta[r] + q of the caller's buffer.
+  // It lives in the scratch part of the workspace and dies with the next scratch reset.
+  const uint4* sched = nullptr;
+  const uint32_t* sched_rowstart = nullptr;   // [n2 + 1]
+  const uint32_t* sched_delta = nullptr;      // [n2]
+  int64_t sched_chunks = 0;
+  const void* sched_pairs = nullptr;          // the pair buffer it describes
+  int64_t sched_npairs = 0;
   // bookkeeping
   int64_t launches = 0;
   int64_t last_raw_pairs = 0;
@@ -73,7 +84,7 @@ static inline T* sq_scratch(sq_ctx* c, size_t count) {
   c->scratch_top += bytes;
   return p;
 }
-static inline void sq_scratch_reset(sq_ctx* c) { c->scratch_top = c->persist; }
+static inline void sq_scratch_reset(sq_ctx* c) { c->scratch_top = c->persist; c->sched = nullptr; }
 
 #define SQ_CUDA(ctx, call)                                   \
   do {                                                       \

@@ -32,17 +32,35 @@ __global__ void edit_pairs_kernel(const uint8_t* __restrict__ packed, int stride
 // the Myers/Hyyro column step; the distance is read off the final vertical deltas:
 // D[m][n] = n + popc(Pv) - popc(Mv) over the m pattern bits, so no score is tracked per column.
 constexpr int kEdWarps = 8;
+constexpr int kEdRuns = 8;      // Peq tables resident per warp
 
-template <int STRIDE>
-__global__ void __launch_bounds__(kEdWarps * 32)
+// SCHED: warp k takes positions [32k, 32k+32) of the family-ordered schedule left by
+// sq_lsh_candidates (sq_common.cuh) instead of pairs [32k, 32k+32): consecutive warps then work
+// on rows of the same family, whose partners are the same few sequences -- the text gathers hit
+// L2.  The schedule only permutes the pair indices; every pair is still read from `pairs`.
+template <int STRIDE, bool SCHED>
+__global__ void __launch_bounds__(kEdWarps * 32, 8)
 edit_pairs_w1_kernel(const uint8_t* __restrict__ packed, int64_t n, const uint2* __restrict__ pairs,
-                     int64_t n_pairs, int max_d, uint16_t* __restrict__ dist) {
+                     int64_t n_pairs, int max_d, uint16_t* __restrict__ dist,
+                     const uint4* __restrict__ sched, const uint32_t* __restrict__ rowstart,
+                     const uint32_t* __restrict__ delta) {
   constexpr int WORDS = STRIDE / 4;
-  __shared__ uint32_t peq_sm[kEdWarps][32 * 33];
-  __shared__ uint32_t mlen_sm[kEdWarps][32];
+  __shared__ uint32_t peq_sm[kEdWarps][kEdRuns * 33];
+  __shared__ uint32_t mlen_sm[kEdWarps][kEdRuns];
   const uint32_t lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  const int64_t p = ((int64_t)blockIdx.x * kEdWarps + w) * 32 + lane;
-  const bool valid = p < n_pairs;
+  const int64_t wk = (int64_t)blockIdx.x * kEdWarps + w;
+  int64_t p = wk * 32 + lane;
+  bool valid = p < n_pairs;
+  if (SCHED && valid) {
+    const uint4 ch = sched[wk];                       // (first row, its delta, end of that row)
+    const uint32_t q = (uint32_t)p;
+    if (q < ch.z) p = (int64_t)(uint32_t)(ch.y + q);
+    else {
+      uint32_t r = ch.x + 1;
+      while (q >= rowstart[r + 1]) ++r;               // empty rows are stepped over
+      p = (int64_t)(uint32_t)(delta[r] + q);
+    }
+  }
   uint2 pr = make_uint2(0xFFFFFFFFu, 0xFFFFFFFFu);
   if (valid) pr = pairs[p];
   const bool inrange = valid && pr.x < (uint64_t)n && pr.y < (uint64_t)n;
@@ -65,56 +83,63 @@ edit_pairs_w1_kernel(const uint8_t* __restrict__ packed, int64_t n, const uint2*
   const int nruns = __popc(hm);
   uint32_t* peq = peq_sm[w];
   uint32_t rem = hm;
-#pragma unroll 1
-  for (int r = 0; r < nruns; ++r) {
-    const int hl = __ffs(rem) - 1;
-    rem &= rem - 1;
-    const uint32_t ir = __shfl_sync(0xFFFFFFFFu, i, hl);
-    uint32_t ch = 0xFFu;
-    if (ir != 0xFFFFFFFFu && lane < (uint32_t)STRIDE) ch = packed[(int64_t)ir * STRIDE + lane];
-    const uint32_t m = ir != 0xFFFFFFFFu ? __shfl_sync(0xFFFFFFFFu, ch, STRIDE - 1) : 0u;
-    peq[r * 33 + lane] = 0u;
-    __syncwarp();
-    const uint32_t mm = __match_any_sync(0xFFFFFFFFu, ch);
-    if (lane < m) peq[r * 33 + ch] = mm & ((1u << m) - 1u);       // m <= 31
-    if (lane == 0) mlen_sm[w][r] = m;
-  }
-  __syncwarp();
-  if (!valid) return;
-  if (!inrange) { dist[p] = 0xFFFFu; return; }
-  const int m = (int)mlen_sm[w][run];
   const int nlen = (int)(tw[WORDS - 1] >> 24);
-  const int diff = m > nlen ? m - nlen : nlen - m;
-  int d;
-  if (max_d >= 0 && diff > max_d) d = max_d + 1;
-  else if (m == 0) d = nlen;
-  else if (nlen == 0) d = m;
-  else {
-    const uint32_t* pq = peq + run * 33;
-    uint32_t Pv = 0xFFFFFFFFu, Mv = 0u;
+  int d = 0;
+  // kEdRuns Peq tables fit at a time; a warp with more runs (many tiny rows) takes several rounds
+#pragma unroll 1
+  for (int rbase = 0; rbase < nruns; rbase += kEdRuns) {
+    const int nr = min(kEdRuns, nruns - rbase);
+    __syncwarp();
+#pragma unroll 1
+    for (int r = 0; r < nr; ++r) {
+      const int hl = __ffs(rem) - 1;
+      rem &= rem - 1;
+      const uint32_t ir = __shfl_sync(0xFFFFFFFFu, i, hl);
+      uint32_t ch = 0xFFu;
+      if (ir != 0xFFFFFFFFu && lane < (uint32_t)STRIDE) ch = packed[(int64_t)ir * STRIDE + lane];
+      const uint32_t m = ir != 0xFFFFFFFFu ? __shfl_sync(0xFFFFFFFFu, ch, STRIDE - 1) : 0u;
+      peq[r * 33 + lane] = 0u;
+      __syncwarp();
+      const uint32_t mm = __match_any_sync(0xFFFFFFFFu, ch);
+      if (lane < m) peq[r * 33 + ch] = mm & ((1u << m) - 1u);     // m <= 31
+      if (lane == 0) mlen_sm[w][r] = m;
+    }
+    __syncwarp();
+    if (!inrange || (int)run < rbase || (int)run >= rbase + nr) continue;
+    const int m = (int)mlen_sm[w][run - rbase];
+    const int diff = m > nlen ? m - nlen : nlen - m;
+    if (max_d >= 0 && diff > max_d) d = max_d + 1;
+    else if (m == 0) d = nlen;
+    else if (nlen == 0) d = m;
+    else {
+      const uint32_t* pq = peq + (run - rbase) * 33;
+      uint32_t Pv = 0xFFFFFFFFu, Mv = 0u;
 #pragma unroll
-    for (int wi = 0; wi < WORDS; ++wi) {
-      if (4 * wi < nlen) {
-        const uint32_t word = tw[wi];
+      for (int wi = 0; wi < WORDS; ++wi) {
+        if (4 * wi < nlen) {
+          const uint32_t word = tw[wi];
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          if (4 * wi + q < nlen) {
-            const uint32_t Eq = pq[(word >> (8 * q)) & 0xFFu];
-            const uint32_t Xv = Eq | Mv;
-            const uint32_t Xh = (((Eq & Pv) + Pv) ^ Pv) | Eq;
-            uint32_t Ph = Mv | ~(Xh | Pv);
-            uint32_t Mh = Pv & Xh;
-            Ph = (Ph << 1) | 1u;
-            Mh <<= 1;
-            Pv = Mh | ~(Xv | Ph);
-            Mv = Ph & Xv;
+          for (int q = 0; q < 4; ++q) {
+            if (4 * wi + q < nlen) {
+              const uint32_t Eq = pq[(word >> (8 * q)) & 0xFFu];
+              const uint32_t Xv = Eq | Mv;
+              const uint32_t Xh = (((Eq & Pv) + Pv) ^ Pv) | Eq;
+              uint32_t Ph = Mv | ~(Xh | Pv);
+              uint32_t Mh = Pv & Xh;
+              Ph = (Ph << 1) | 1u;
+              Mh <<= 1;
+              Pv = Mh | ~(Xv | Ph);
+              Mv = Ph & Xv;
+            }
           }
         }
       }
+      const uint32_t mask = (1u << m) - 1u;                        // m <= 31
+      d = nlen + __popc(Pv & mask) - __popc(Mv & mask);
     }
-    const uint32_t mask = (1u << m) - 1u;                          // m <= 31
-    d = nlen + __popc(Pv & mask) - __popc(Mv & mask);
   }
+  if (!valid) return;
+  if (!inrange) { dist[p] = 0xFFFFu; return; }
   if (max_d >= 0 && d > max_d) d = max_d + 1;
   dist[p] = (uint16_t)d;
 }
@@ -122,9 +147,19 @@ edit_pairs_w1_kernel(const uint8_t* __restrict__ packed, int64_t n, const uint2*
 template <int STRIDE>
 int launch_edit_w1(sq_ctx* c, const uint32_t* pairs, int64_t n_pairs, int max_d, uint16_t* dist_out) {
   const int64_t per_block = kEdWarps * 32;
+  // the schedule pays off only when the packed sequences do not fit the L2 anyway
+  const bool big = (size_t)c->n * (size_t)c->stride > ((size_t)96 << 20);
+  if (big && c->sched && c->sched_pairs == pairs && c->sched_npairs == n_pairs && c->sched_chunks > 0) {
+    const int64_t blocks = (c->sched_chunks + kEdWarps - 1) / kEdWarps;
+    SQ_TIMED(c, SQ_K_EDIT, edit_pairs_w1_kernel<STRIDE, true><<<(unsigned)blocks, kEdWarps * 32, 0, c->stream>>>(
+        c->packed, c->n, reinterpret_cast<const uint2*>(pairs), n_pairs, max_d, dist_out, c->sched,
+        c->sched_rowstart, c->sched_delta));
+    SQ_LAUNCH_CHECK(c);
+    return SQ_OK;
+  }
   const int64_t blocks = (n_pairs + per_block - 1) / per_block;
-  SQ_TIMED(c, SQ_K_EDIT, edit_pairs_w1_kernel<STRIDE><<<(unsigned)blocks, kEdWarps * 32, 0, c->stream>>>(
-      c->packed, c->n, reinterpret_cast<const uint2*>(pairs), n_pairs, max_d, dist_out));
+  SQ_TIMED(c, SQ_K_EDIT, edit_pairs_w1_kernel<STRIDE, false><<<(unsigned)blocks, kEdWarps * 32, 0, c->stream>>>(
+      c->packed, c->n, reinterpret_cast<const uint2*>(pairs), n_pairs, max_d, dist_out, nullptr, nullptr, nullptr));
   SQ_LAUNCH_CHECK(c);
   return SQ_OK;
 }

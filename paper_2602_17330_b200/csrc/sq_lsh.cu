@@ -97,6 +97,33 @@ ext_count_kernel(const uint32_t* __restrict__ rowidx, const uint32_t* __restrict
   ext_cnt[i] = r == 0xFFFFFFFFu ? 0u : off[((int64_t)r + 1) * bands] - off[(int64_t)r * bands];
 }
 
+// compact per-row tables of the schedule: rowstart[r] = first internal position of row r,
+// delta[r] = (first pair of row r in the caller's buffer) - rowstart[r]
+__global__ void __launch_bounds__(256)
+rowstart_kernel(const uint32_t* __restrict__ off, const uint32_t* __restrict__ ids0,
+                const uint32_t* __restrict__ ext_off, int64_t n2, int bands,
+                uint32_t* __restrict__ rowstart, uint32_t* __restrict__ delta) {
+  const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (r > n2) return;
+  const uint32_t rs = off[r * bands];
+  rowstart[r] = rs;
+  if (r < n2) delta[r] = ext_off[ids0[r]] - rs;
+}
+
+// sched[k] for every chunk k whose first position 32k falls into row r (one warp per row)
+__global__ void __launch_bounds__(256)
+sched_fill_kernel(const uint32_t* __restrict__ rowstart, const uint32_t* __restrict__ delta,
+                  int64_t n2, uint4* __restrict__ sched) {
+  const int lane = threadIdx.x & 31;
+  const int64_t r = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (r >= n2) return;
+  const uint32_t b = rowstart[r], e = rowstart[r + 1];
+  if (e == b) return;
+  const uint32_t d = delta[r];
+  for (uint32_t k = (b + 31) / 32 + lane; (uint64_t)k * 32 < e; k += 32)
+    sched[k] = make_uint4((uint32_t)r, d, e, 0u);
+}
+
 // ---------------------------------------------------------------------------------------------
 // a5.1  bucket scan
 // ---------------------------------------------------------------------------------------------
@@ -732,6 +759,8 @@ size_t sq_lsh_scratch_bytes(int64_t n, int bands, int64_t pair_capacity) {
   s += sq_sort_scratch_bytes(n, bands);
   s += sq_align_up((size_t)(pair_capacity > 0 ? pair_capacity : 0) * 4 + 16);   // partners
   s += sq_align_up(rec * 32 + 16);             // mask cache of the count pass (used if it fits)
+  s += sq_align_up(((size_t)(pair_capacity > 0 ? pair_capacity : 0) / 32 + 2) * 16 + 16) +
+       2 * sq_align_up((nn + 2) * 4 + 16);     // chunk schedule of the edit-distance stage
   return s + 4096;
 }
 
@@ -862,6 +891,27 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
         cnt, n2, bands, vin, ext_off, flags == SQ_LSH_SORTED, tmpJ, reinterpret_cast<uint2*>(pairs_out),
         counters + 6));
     SQ_LAUNCH_CHECK(c);
+  }
+  // family-ordered chunk schedule for sq_edit_distance (a hint; skipped if it does not fit)
+  {
+    const size_t nchunks = ((size_t)uniq + 31) / 32;
+    uint4* sched = sq_scratch<uint4>(c, nchunks);
+    uint32_t* rowstart = sq_scratch<uint32_t>(c, (size_t)n2 + 1);
+    uint32_t* delta = sq_scratch<uint32_t>(c, (size_t)n2 + 1);
+    if (sched && rowstart && delta) {
+      SQ_TIMED(c, SQ_K_MISC, rowstart_kernel<<<(unsigned)((n2 + 256) / 256), 256, 0, st>>>(
+          cnt, vin, ext_off, n2, bands, rowstart, delta));
+      SQ_LAUNCH_CHECK(c);
+      SQ_TIMED(c, SQ_K_MISC, sched_fill_kernel<<<(unsigned)((n2 * 32 + 255) / 256), 256, 0, st>>>(
+          rowstart, delta, n2, sched));
+      SQ_LAUNCH_CHECK(c);
+      c->sched = sched;
+      c->sched_rowstart = rowstart;
+      c->sched_delta = delta;
+      c->sched_chunks = (int64_t)nchunks;
+      c->sched_pairs = pairs_out;
+      c->sched_npairs = uniq;
+    }
   }
   SQ_CUDA(c, cudaStreamSynchronize(st));
   return SQ_OK;

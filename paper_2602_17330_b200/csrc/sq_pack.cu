@@ -74,6 +74,7 @@ extern "C" int sq_pack(sq_ctx* c, const uint8_t* seqs, const int64_t* offsets, i
   if (max_len > SQ_MAX_LEN) return SQ_ERR_UNSUPPORTED;
   if (!c->ws) return SQ_ERR_WORKSPACE;
   c->n = -1;
+  c->sched = nullptr;
   const int stride = sq_stride_for(max_len);
   const size_t nn = (size_t)(n > 0 ? n : 1);
   // persistent region
