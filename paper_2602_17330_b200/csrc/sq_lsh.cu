@@ -87,27 +87,33 @@ translate_kernel(const uint32_t* __restrict__ ids, int64_t total, const uint32_t
   if (g < total) ids_int[g] = rowidx[ids[g]];
 }
 
+// partners of internal row r over all bands (offsets are band-major: off[b*n2 + r])
+__global__ void __launch_bounds__(256)
+row_total_kernel(const uint32_t* __restrict__ off, int64_t n2, int bands, uint32_t* __restrict__ row_tot) {
+  const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (r > n2) return;
+  uint32_t t = 0;
+  if (r < n2)
+    for (int b = 0; b < bands; ++b) t += off[(int64_t)b * n2 + r + 1] - off[(int64_t)b * n2 + r];
+  row_tot[r] = t;                              // row_tot[n2] = 0: the scan leaves the total there
+}
+
 // partners of every EXTERNAL id (0 for sequences without a signature), to be scanned into ext_off
 __global__ void __launch_bounds__(256)
-ext_count_kernel(const uint32_t* __restrict__ rowidx, const uint32_t* __restrict__ off, int64_t n,
-                 int bands, uint32_t* __restrict__ ext_cnt) {
+ext_count_kernel(const uint32_t* __restrict__ rowidx, const uint32_t* __restrict__ row_tot, int64_t n,
+                 uint32_t* __restrict__ ext_cnt) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   const uint32_t r = rowidx[i];
-  ext_cnt[i] = r == 0xFFFFFFFFu ? 0u : off[((int64_t)r + 1) * bands] - off[(int64_t)r * bands];
+  ext_cnt[i] = r == 0xFFFFFFFFu ? 0u : row_tot[r];
 }
 
-// compact per-row tables of the schedule: rowstart[r] = first internal position of row r,
-// delta[r] = (first pair of row r in the caller's buffer) - rowstart[r]
+// delta[r] = (first pair of row r in the caller's buffer) - rowstart[r], rowstart = scan of row_tot
 __global__ void __launch_bounds__(256)
-rowstart_kernel(const uint32_t* __restrict__ off, const uint32_t* __restrict__ ids0,
-                const uint32_t* __restrict__ ext_off, int64_t n2, int bands,
-                uint32_t* __restrict__ rowstart, uint32_t* __restrict__ delta) {
+delta_kernel(const uint32_t* __restrict__ rowstart, const uint32_t* __restrict__ ids0,
+             const uint32_t* __restrict__ ext_off, int64_t n2, uint32_t* __restrict__ delta) {
   const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (r > n2) return;
-  const uint32_t rs = off[r * bands];
-  rowstart[r] = rs;
-  if (r < n2) delta[r] = ext_off[ids0[r]] - rs;
+  if (r < n2) delta[r] = ext_off[ids0[r]] - rowstart[r];
 }
 
 // sched[k] for every chunk k whose first position 32k falls into row r (one warp per row)
@@ -335,10 +341,10 @@ emit_band0_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint32
   // internal row of a band-0 record = its sorted position: the rows of a unit are consecutive
   const int64_t myrow = (int64_t)unit.x + lane;
   if (MODE == EM_COUNT) {
-    if (rowok) cnt_off[myrow * bands] = mrem - 1u - (uint32_t)lane;
+    if (rowok) cnt_off[myrow] = mrem - 1u - (uint32_t)lane;       // band 0: index 0*n2 + row
     return;
   }
-  const uint32_t off = rowok ? cnt_off[myrow * bands] : 0u;
+  const uint32_t off = rowok ? cnt_off[myrow] : 0u;
   for (uint32_t l = 0; l < nrows; ++l) {     // coalesced: the warp writes row l's partners
     const uint32_t o = __shfl_sync(kFull, off, l);
     for (uint32_t cc = l + 1 + lane; cc < mrem; cc += 32) outJ[o + cc - l - 1] = idp[cc];
@@ -381,8 +387,11 @@ struct EmDesc { uint32_t u, g0, mrem, c0; int b; bool ok; };
 // BW = 16-byte chunks per S row (S row width SW = 4*BW >= bands).
 // ids = external sequence ids of the sorted records (the values that are emitted); ids_int =
 // their internal rows (position in band 0's sorted order), which index S and the counts.
-// MODE EM_COUNT:  cnt[row*bands + b] = number of NEW partners of internal row `row` in band b.
-// MODE EM_FILL_J: outJ[off[row*bands + b] + t] = external id of the t-th new partner.
+// Counts / offsets are BAND-major, [b][n2]: the rows of a unit are bucket neighbours, hence (for
+// family members) near neighbours in band 0's order too, so the 32 lanes of a warp append to
+// adjacent small groups of the partner scratch and their partial sectors merge in L1/L2.
+// MODE EM_COUNT:  cnt[b*n2 + row] = number of NEW partners of internal row `row` in band b.
+// MODE EM_FILL_J: outJ[off[b*n2 + row] + t] = external id of the t-th new partner.
 template <int BW, int MODE>
 __global__ void __launch_bounds__(kEmWarps * 32)
 emit_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint32_t* __restrict__ ids,
@@ -455,7 +464,7 @@ emit_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint32_t* __
       myid = idc_c;
       rowok = lane < min(32u, dc.mrem - 1u);
       acc = 0;
-      if (MODE != EM_COUNT && rowok) acc = cnt_off[(int64_t)myid * bands + b];
+      if (MODE != EM_COUNT && rowok) acc = cnt_off[(int64_t)b * n2 + myid];
       if (MODE == EM_COUNT && masks) ub = ubase[dc.u];
 #pragma unroll
       for (int ch = 0; ch < BW; ++ch) {
@@ -486,7 +495,7 @@ emit_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint32_t* __
     if (MODE == EM_COUNT) {
       acc += __popc(tmask);
       if (masks) masks[((size_t)ub + (dc.c0 >> 5)) * 32 + lane] = tmask;   // kept for the fill pass
-      if (rowok && dc.c0 + 32 >= dc.mrem) cnt_off[(int64_t)myid * bands + b] = acc;
+      if (rowok && dc.c0 + 32 >= dc.mrem) cnt_off[(int64_t)b * n2 + myid] = acc;
     }
     __syncwarp();
     dc = dn; idc_c = idc_n; idx_c = idx_n; dn = d2; idc_n = id2; idx_n = ix2; ++k;
@@ -497,7 +506,9 @@ emit_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint32_t* __
 // Pass 2 when the count pass could keep its per-tile masks: no S rows, no compares.  One
 // (persistent) warp per unit walks the unit's tiles; lane = row holds the mask of its new columns
 // of the tile and the id of column `lane`; every round each lane with a bit left takes its next
-// column's id from the owning lane (SHFL) and appends it to its row's output.
+// column's id from the owning lane (SHFL) and appends it to its row's group.  A unit is a chain
+// of three dependent loads (descriptor -> ids + first mask -> output offset); the warp keeps the
+// chains of its next three units in flight while it works on the current one.
 __global__ void __launch_bounds__(kEmWarps * 32)
 emit_fill_masks_kernel(const uint2* __restrict__ units, uint32_t nunits,
                        const uint32_t* __restrict__ ubase, const uint32_t* __restrict__ masks,
@@ -506,20 +517,44 @@ emit_fill_masks_kernel(const uint2* __restrict__ units, uint32_t nunits,
                        uint32_t* __restrict__ outJ) {
   const uint32_t lane = threadIdx.x & 31;
   const uint32_t nw = gridDim.x * kEmWarps;
-  for (uint32_t u = blockIdx.x * kEmWarps + (threadIdx.x >> 5); u < nunits; u += nw) {
-    const uint2 unit = units[u];
-    const uint32_t g0 = unit.x, mrem = unit.y;
-    const int b = (int)(g0 / n2);
+  uint32_t u = blockIdx.x * kEmWarps + (threadIdx.x >> 5);
+  if (u >= nunits) return;
+  struct L1 { uint2 un; uint32_t tb; };
+  struct L2 { uint32_t idx, idi, msk; };
+  auto load1 = [&](uint32_t uu) -> L1 {              // needs only the unit index
+    L1 r; r.un = make_uint2(0u, 0u); r.tb = 0u;
+    if (uu < nunits) { r.un = units[uu]; r.tb = ubase[uu]; }
+    return r;
+  };
+  auto load2 = [&](const L1& a) -> L2 {              // needs the descriptor
+    L2 r; r.idx = 0u; r.idi = 0u; r.msk = 0u;
+    if (a.un.y) {
+      if (lane < a.un.y) { r.idx = ids[a.un.x + lane]; r.idi = ids_int[a.un.x + lane]; }
+      r.msk = masks[(size_t)a.tb * 32 + lane];
+    }
+    return r;
+  };
+  auto load3 = [&](const L1& a, const L2& b2) -> uint32_t {   // needs the row's internal id
+    if (a.un.y && lane < min(32u, a.un.y - 1u))
+      return cnt_off[(int64_t)(a.un.x / n2) * n2 + b2.idi];
+    return 0u;
+  };
+  L1 a0 = load1(u), a1 = load1(u + nw), a2 = load1(u + 2 * nw);
+  L2 b0 = load2(a0), b1 = load2(a1);
+  uint32_t acc = load3(a0, b0);
+  for (; u < nunits; u += nw) {
+    const uint32_t acc1 = load3(a1, b1);             // chains of the next units advance one level
+    const L2 b2 = load2(a2);
+    const L1 a3 = load1(u + 3 * nw);
+    // ---- the current unit
+    const uint32_t g0 = a0.un.x, mrem = a0.un.y;
     const uint32_t* __restrict__ idp = ids + g0;
-    const uint32_t* __restrict__ mp = masks + (size_t)ubase[u] * 32 + lane;
-    const uint32_t myid = lane < mrem ? idp[lane] : 0u;
-    uint32_t acc = 0;
-    if (lane < min(32u, mrem - 1u)) acc = cnt_off[(int64_t)ids_int[g0 + lane] * bands + b];
-    uint32_t mask = mp[0], idc = myid;
+    const uint32_t* __restrict__ mp = masks + (size_t)a0.tb * 32 + lane;
+    uint32_t mask = b0.msk, idc = b0.idx;
     for (uint32_t c0 = 0; c0 < mrem; c0 += 32) {
-      uint32_t mask_n = 0, idc_n = 0;            // next tile, in flight during this one
+      uint32_t mask_n = 0, idc_n = 0;                // next tile, in flight during this one
       if (c0 + 32 < mrem) {
-        mask_n = mp[(size_t)(c0 + 32)];          // (c0+32)/32 tiles further = (c0+32) words
+        mask_n = mp[(size_t)(c0 + 32)];              // (c0+32)/32 tiles further = (c0+32) words
         if (c0 + 32 + lane < mrem) idc_n = idp[c0 + 32 + lane];
       }
       while (__any_sync(kFull, mask != 0u)) {
@@ -533,77 +568,113 @@ emit_fill_masks_kernel(const uint2* __restrict__ units, uint32_t nunits,
       }
       mask = mask_n; idc = idc_n;
     }
+    a0 = a1; a1 = a2; a2 = a3; b0 = b1; b1 = b2; acc = acc1;
   }
 }
 
 // ---------------------------------------------------------------------------------------------
-// a5.3  SQ_LSH_SORTED: put every row's partners in ascending order
+// a5.3  every row into its slice of the output, in ascending j if asked
 // ---------------------------------------------------------------------------------------------
 // One warp per INTERNAL row r (rows are visited in band 0's sorted order, i.e. family by family,
 // and written to the slice of `out` that belongs to the row's EXTERNAL id: ext_off).  The row's
-// partners (external ids) sit in inJ[base, base+T) as <= B ascending groups.  The
-// ids of a repertoire carry no structure, so the partners of a row are spread evenly between the
-// row's smallest and largest partner: ONE most-significant-digit pass over kRsBins equal-width
-// value bins (shared-memory counters) groups them, and an element's final place is its bin's
-// start plus the number of smaller elements in its own bin (1-2 on average, any number is
-// correct).  Passes: count per bin -> scan -> group into the row's slice of `out` (as uint32
-// scratch) -> rank inside the bin, back into inJ (now sorted) -> write (i, j) pairs.
+// partners (external ids) sit in the partner scratch as <= B ascending groups, group b at
+// inJ[off[b*n2+r], off[b*n2+r+1]).  The ids of a repertoire carry no structure, so the partners
+// of a row are spread evenly between the row's smallest and largest partner: ONE
+// most-significant-digit pass over kRsBins equal-width value bins (shared-memory counters)
+// groups them, and an element's final place is its bin's start plus the number of smaller
+// elements in its own bin (1-2 on average, any number is correct).  The row's output slice (2T
+// words) is the scratch: X = words [0,T), Y = words [T,2T).  Passes: gather the groups into X ->
+// count per bin -> scan -> group by bin into Y -> rank inside the bin, sorted, back into X ->
+// expand X into (i, j) pairs in place, from the top down.
 constexpr int kRsWarps = 8;
 constexpr int kRsBins = 1024;
 
 __device__ __forceinline__ void
-sort_one_row(const uint32_t* __restrict__ off, int bands, uint32_t* inJ, uint2* out, int64_t r,
-             uint32_t row, uint32_t obase, bool do_sort, uint32_t* bins, int lane) {
-  // lane b holds the start of group b; the lanes past `bands` hold the row end
-  const uint32_t row_end = off[(r + 1) * bands];
-  const uint32_t gs = lane < bands ? off[r * bands + lane] : row_end;
-  uint32_t ge = __shfl_down_sync(kFull, gs, 1);
-  if (lane == 31 || lane + 1 >= bands) ge = row_end;
-  const uint32_t base = __shfl_sync(kFull, gs, 0);
-  const uint32_t T = row_end - base;
+sort_one_row(const uint32_t* __restrict__ off, int64_t n2, int bands, const uint32_t* __restrict__ inJ,
+             uint2* out, int64_t r, uint32_t row, uint32_t obase, bool do_sort, uint32_t* bins,
+             int lane) {
+  // lane b holds group b
+  uint32_t gs = 0, len = 0;
+  if (lane < bands) {
+    gs = off[(int64_t)lane * n2 + r];
+    len = off[(int64_t)lane * n2 + r + 1] - gs;
+  }
+  uint32_t pre = len;                        // inclusive -> exclusive prefix of the group lengths
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const uint32_t o = __shfl_up_sync(kFull, pre, d);
+    if (lane >= d) pre += o;
+  }
+  const uint32_t T = __shfl_sync(kFull, pre, 31);
   if (T == 0) return;
-  const bool has = lane < bands && ge > gs;
-  const uint32_t nonempty = __ballot_sync(kFull, has);
-  uint32_t* J = inJ + base;
+  pre -= len;
+  const uint32_t nonempty = __ballot_sync(kFull, len > 0);
   out += obase;                              // the row's slice of the output
+  uint32_t* X = reinterpret_cast<uint32_t*>(out);
+  // the groups are small (a few elements each): four are gathered per step, loads first
+  auto gather = [&](auto&& put) {
+    uint32_t gm = nonempty;
+    while (gm) {
+      uint32_t s[4], l[4], p[4], v[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        l[k] = 0; s[k] = 0; p[k] = 0;
+        if (gm) {
+          const int g = __ffs(gm) - 1;
+          gm &= gm - 1;
+          s[k] = __shfl_sync(kFull, gs, g); l[k] = __shfl_sync(kFull, len, g); p[k] = __shfl_sync(kFull, pre, g);
+        }
+      }
+#pragma unroll
+      for (int k = 0; k < 4; ++k) v[k] = (uint32_t)lane < l[k] ? inJ[s[k] + lane] : 0u;
+#pragma unroll
+      for (int k = 0; k < 4; ++k) if ((uint32_t)lane < l[k]) put(p[k] + lane, v[k]);
+#pragma unroll
+      for (int k = 0; k < 4; ++k)
+        for (uint32_t e = 32 + lane; e < l[k]; e += 32) put(p[k] + e, inJ[s[k] + e]);
+    }
+  };
   if (__popc(nonempty) == 1 || !do_sort) {   // already ascending, or the grouped order is asked for
-    for (uint32_t t = lane; t < T; t += 32) out[t] = make_uint2(row, J[t]);
+    gather([&](uint32_t at, uint32_t x) { out[at] = make_uint2(row, x); });
     return;
   }
+  uint32_t lo = kFull, hi = 0;               // value range: every group is ascending
+  if (len > 0) { lo = inJ[gs]; hi = inJ[gs + len - 1]; }
+  gather([&](uint32_t at, uint32_t x) { X[at] = x; });
+  __syncwarp();
   if (T <= 32) {                             // rank by counting inside the warp
-    const uint32_t x = (uint32_t)lane < T ? J[lane] : kFull;
+    const uint32_t x = (uint32_t)lane < T ? X[lane] : kFull;
     uint32_t rank = 0;
     for (uint32_t s = 0; s < T; ++s) rank += __shfl_sync(kFull, x, s) < x ? 1u : 0u;
+    __syncwarp();
     if ((uint32_t)lane < T) out[rank] = make_uint2(row, x);
     return;
   }
-  // value range of the row: every group is ascending, so its ends are its extremes
-  uint32_t lo = has ? inJ[gs] : kFull, hi = has ? inJ[ge - 1] : 0u;
   lo = __reduce_min_sync(kFull, lo);
   hi = __reduce_max_sync(kFull, hi);
   const float scale = (float)kRsBins / ((float)(hi - lo) + 1.0f);
   auto bin_of = [&](uint32_t x) -> uint32_t {     // monotone in x, < kRsBins
     return min((uint32_t)kRsBins - 1u, (uint32_t)((float)(x - lo) * scale));
   };
-  uint32_t* X = reinterpret_cast<uint32_t*>(out);            // scratch: first T words of the slice
-#pragma unroll
-  for (int q = 0; q < kRsBins / 128; ++q)
-    *reinterpret_cast<uint4*>(bins + q * 128 + lane * 4) = make_uint4(0, 0, 0, 0);
+  auto bin_at = [&](uint32_t x) -> uint32_t { const uint32_t b = bin_of(x); return b + (b >> 5); };
+  uint32_t* Y = X + T;
+  // bin b lives at word b + b/32: lane-major walks of the scan below are then conflict-free
+  for (int q = lane; q < kRsBins + kRsBins / 32; q += 32) bins[q] = 0u;
   __syncwarp();
   // (every pass loads 4 batches of 32 before it uses them: the passes are latency-bound)
   for (uint32_t t0 = lane; t0 < T; t0 += 128) {
     uint32_t x[4];
 #pragma unroll
-    for (int u = 0; u < 4; ++u) x[u] = t0 + 32 * u < T ? J[t0 + 32 * u] : 0u;
+    for (int u = 0; u < 4; ++u) x[u] = t0 + 32 * u < T ? X[t0 + 32 * u] : 0u;
 #pragma unroll
-    for (int u = 0; u < 4; ++u) if (t0 + 32 * u < T) atomicAdd(&bins[bin_of(x[u])], 1u);
+    for (int u = 0; u < 4; ++u) if (t0 + 32 * u < T) atomicAdd(&bins[bin_at(x[u])], 1u);
   }
   __syncwarp();
   {                                          // exclusive scan of the bin counts
     constexpr int PER = kRsBins / 32;
     uint32_t v[PER], s = 0;
 #pragma unroll
-    for (int q = 0; q < PER; ++q) { v[q] = bins[lane * PER + q]; s += v[q]; }
+    for (int q = 0; q < PER; ++q) { v[q] = bins[lane * (PER + 1) + q]; s += v[q]; }
     uint32_t inc = s;
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) {
@@ -612,37 +683,41 @@ sort_one_row(const uint32_t* __restrict__ off, int bands, uint32_t* inJ, uint2* 
     }
     uint32_t run = inc - s;
 #pragma unroll
-    for (int q = 0; q < PER; ++q) { bins[lane * PER + q] = run; run += v[q]; }
+    for (int q = 0; q < PER; ++q) { bins[lane * (PER + 1) + q] = run; run += v[q]; }
   }
   __syncwarp();
   for (uint32_t t0 = lane; t0 < T; t0 += 128) {   // group by bin (arrival order inside a bin)
     uint32_t x[4];
 #pragma unroll
-    for (int u = 0; u < 4; ++u) x[u] = t0 + 32 * u < T ? J[t0 + 32 * u] : 0u;
+    for (int u = 0; u < 4; ++u) x[u] = t0 + 32 * u < T ? X[t0 + 32 * u] : 0u;
 #pragma unroll
-    for (int u = 0; u < 4; ++u) if (t0 + 32 * u < T) X[atomicAdd(&bins[bin_of(x[u])], 1u)] = x[u];
+    for (int u = 0; u < 4; ++u) if (t0 + 32 * u < T) Y[atomicAdd(&bins[bin_at(x[u])], 1u)] = x[u];
   }
   __syncwarp();                              // now bins[b] = end of bin b = start of bin b+1
-  for (uint32_t t0 = lane; t0 < T; t0 += 128) {   // rank inside the bin -> sorted, back into J
+  for (uint32_t t0 = lane; t0 < T; t0 += 128) {   // rank inside the bin -> sorted, back into X
     uint32_t x[4];
 #pragma unroll
-    for (int u = 0; u < 4; ++u) x[u] = t0 + 32 * u < T ? X[t0 + 32 * u] : 0u;
+    for (int u = 0; u < 4; ++u) x[u] = t0 + 32 * u < T ? Y[t0 + 32 * u] : 0u;
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
       if (t0 + 32 * u < T) {
         const uint32_t b = bin_of(x[u]);
-        const uint32_t s = b ? bins[b - 1] : 0u, e = bins[b];
-        uint32_t r = s;
-        for (uint32_t q = s; q < e; ++q) r += X[q] < x[u] ? 1u : 0u;
-        J[r] = x[u];
+        const uint32_t s = b ? bins[(b - 1) + ((b - 1) >> 5)] : 0u, e = bins[b + (b >> 5)];
+        uint32_t rk = s;
+        for (uint32_t q = s; q < e; ++q) rk += Y[q] < x[u] ? 1u : 0u;
+        X[rk] = x[u];
       }
     }
   }
   __syncwarp();
-  for (uint32_t t0 = lane; t0 < T; t0 += 128) {
+  // expand in place, top down: pair t lands on words 2t, 2t+1 >= t, i.e. never on an element
+  // of a lower batch; inside a batch every load precedes every store
+  for (uint32_t t1 = (T + 127) / 128 * 128; t1 > 0; t1 -= 128) {
+    const uint32_t t0 = t1 - 128 + lane;
     uint32_t x[4];
 #pragma unroll
-    for (int u = 0; u < 4; ++u) x[u] = t0 + 32 * u < T ? J[t0 + 32 * u] : 0u;
+    for (int u = 0; u < 4; ++u) x[u] = t0 + 32 * u < T ? X[t0 + 32 * u] : 0u;
+    __syncwarp();
 #pragma unroll
     for (int u = 0; u < 4; ++u) if (t0 + 32 * u < T) out[t0 + 32 * u] = make_uint2(row, x[u]);
   }
@@ -650,12 +725,12 @@ sort_one_row(const uint32_t* __restrict__ off, int bands, uint32_t* inJ, uint2* 
 
 constexpr int kRsChunk = 8;
 
-__global__ void __launch_bounds__(kRsWarps * 32)
+__global__ void __launch_bounds__(kRsWarps * 32, 6)
 row_sort_kernel(const uint32_t* __restrict__ off, int64_t n2, int bands,
                 const uint32_t* __restrict__ ids0, const uint32_t* __restrict__ ext_off,
-                bool do_sort, uint32_t* inJ, uint2* out,
+                bool do_sort, const uint32_t* __restrict__ inJ, uint2* out,
                 unsigned long long* __restrict__ next_row) {
-  __shared__ uint32_t bins_sh[kRsWarps][kRsBins];
+  __shared__ __align__(16) uint32_t bins_sh[kRsWarps][kRsBins + kRsBins / 32];
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   // Rows differ by four orders of magnitude in size: persistent warps fetch rows kRsChunk at a
   // time from a global counter, so no warp idles behind a heavy row of its block.
@@ -667,7 +742,8 @@ row_sort_kernel(const uint32_t* __restrict__ off, int64_t n2, int bands,
     const int64_t last = min(n2, (int64_t)first + kRsChunk);
     for (int64_t r = (int64_t)first; r < last; ++r) {
       const uint32_t i = ids0[r];            // external id of internal row r
-      sort_one_row(off, bands, inJ, out, r, i, ext_off[i], do_sort, bins_sh[w], lane);
+      sort_one_row(off, n2, bands, inJ, out, r, i, ext_off[i], do_sort, bins_sh[w], lane);
+      __syncwarp();
     }
   }
 }
@@ -755,7 +831,7 @@ size_t sq_lsh_scratch_bytes(int64_t n, int bands, int64_t pair_capacity) {
   s += sq_align_up(nn * sw * 4 + 16);          // bucket-id table S
   s += sq_align_up((rec + 2) * 4 + 16);        // per (row, band) counts -> offsets
   s += sq_align_up((rec / 2 + 2) * 4 + 16);    // first mask tile of every unit
-  s += 3 * sq_align_up((nn + 2) * 4 + 16);     // non-empty flags / ranks; rowidx; ext_off
+  s += 4 * sq_align_up((nn + 2) * 4 + 16);     // non-empty flags / ranks; rowidx; ext_off; rowstart
   s += sq_sort_scratch_bytes(n, bands);
   s += sq_align_up((size_t)(pair_capacity > 0 ? pair_capacity : 0) * 4 + 16);   // partners
   s += sq_align_up(rec * 32 + 16);             // mask cache of the count pass (used if it fits)
@@ -793,8 +869,9 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
   uint32_t* nonempty = sq_scratch<uint32_t>(c, (size_t)n + 2);
   uint32_t* rowidx = sq_scratch<uint32_t>(c, (size_t)n + 2);
   uint32_t* ext_off = sq_scratch<uint32_t>(c, (size_t)n + 2);
+  uint32_t* rowstart = sq_scratch<uint32_t>(c, (size_t)n + 2);
   uint8_t* tmp = sq_scratch<uint8_t>(c, sq_sort_scratch_bytes(n, bands));
-  if (!k0 || !k1 || !v0 || !v1 || !S || !cnt || !ubase || !nonempty || !rowidx || !ext_off || !tmp)
+  if (!k0 || !k1 || !v0 || !v1 || !S || !cnt || !ubase || !nonempty || !rowidx || !ext_off || !rowstart || !tmp)
     return SQ_ERR_WORKSPACE;
   cudaStream_t st = c->stream;
   unsigned long long* counters = c->dflags;      // [0] unique, [1] raw, [2] n2, [4] units
@@ -857,7 +934,7 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
   rc = dispatch_emit(c, bw, EM_COUNT, units, nunits, units0, nunits0, vin, vint, (uint32_t)n2, bands, S,
                      cnt, nullptr, ubase, masks);
   if (rc != SQ_OK) return rc;
-  rc = sq_exclusive_scan_u32(c, cnt, cnt, (int64_t)rec + 1, reinterpret_cast<uint32_t*>(tmp), counters);
+  rc = sq_exclusive_scan_u32(c, cnt, cnt, total + 1, reinterpret_cast<uint32_t*>(tmp), counters);
   if (rc != SQ_OK) return rc;
   SQ_CUDA(c, cudaMemcpyAsync(c->pinned, counters, 8, cudaMemcpyDeviceToHost, st));
   SQ_CUDA(c, cudaStreamSynchronize(st));
@@ -867,10 +944,14 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
   if (uniq >= (1ll << 32) - 1) return SQ_ERR_UNSUPPORTED;   // 32-bit output offsets
   if (uniq == 0) return SQ_OK;
   // where every EXTERNAL row starts in the output
-  SQ_TIMED(c, SQ_K_SEGMENT, ext_count_kernel<<<gb, 256, 0, st>>>(rowidx, cnt, n, bands, ext_off));
+  SQ_TIMED(c, SQ_K_SEGMENT, row_total_kernel<<<(unsigned)((n2 + 256) / 256), 256, 0, st>>>(cnt, n2, bands, rowstart));
+  SQ_LAUNCH_CHECK(c);
+  SQ_TIMED(c, SQ_K_SEGMENT, ext_count_kernel<<<gb, 256, 0, st>>>(rowidx, rowstart, n, ext_off));
   SQ_LAUNCH_CHECK(c);
   rc = sq_exclusive_scan_u32(c, ext_off, ext_off, n, reinterpret_cast<uint32_t*>(tmp), nullptr);
   if (rc != SQ_OK) return rc;
+  rc = sq_exclusive_scan_u32(c, rowstart, rowstart, n2 + 1, reinterpret_cast<uint32_t*>(tmp), nullptr);
+  if (rc != SQ_OK) return rc;                     // rowstart[r] = first internal position of row r
   // a5.2 pass 2: the partners of every internal row, grouped by band, into the partner scratch
   uint32_t* tmpJ = sq_scratch<uint32_t>(c, (size_t)uniq);
   if (!tmpJ) return SQ_ERR_WORKSPACE;
@@ -896,11 +977,10 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
   {
     const size_t nchunks = ((size_t)uniq + 31) / 32;
     uint4* sched = sq_scratch<uint4>(c, nchunks);
-    uint32_t* rowstart = sq_scratch<uint32_t>(c, (size_t)n2 + 1);
     uint32_t* delta = sq_scratch<uint32_t>(c, (size_t)n2 + 1);
-    if (sched && rowstart && delta) {
-      SQ_TIMED(c, SQ_K_MISC, rowstart_kernel<<<(unsigned)((n2 + 256) / 256), 256, 0, st>>>(
-          cnt, vin, ext_off, n2, bands, rowstart, delta));
+    if (sched && delta) {
+      SQ_TIMED(c, SQ_K_MISC, delta_kernel<<<(unsigned)((n2 + 255) / 256), 256, 0, st>>>(
+          rowstart, vin, ext_off, n2, delta));
       SQ_LAUNCH_CHECK(c);
       SQ_TIMED(c, SQ_K_MISC, sched_fill_kernel<<<(unsigned)((n2 * 32 + 255) / 256), 256, 0, st>>>(
           rowstart, delta, n2, sched));
