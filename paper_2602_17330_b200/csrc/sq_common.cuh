@@ -120,6 +120,12 @@ int sq_radix_sort(sq_ctx* c, uint64_t* keys_in, uint64_t* keys_alt, uint32_t* va
                   uint32_t* vals_alt, int64_t n, int nbatch, const int* shifts, const int* widths,
                   int npasses, void* tmp, int* result_in_alt);
 
+// The same sort for byte-wise passes 0..npasses-1 (shift 8p, width 8) in ONE kernel per pass
+// (all histograms up front, decoupled look-back between tiles).  n < 2^30 per batch.
+int sq_onesweep_sort(sq_ctx* c, uint64_t* keys_in, uint64_t* keys_alt, uint32_t* vals_in,
+                     uint32_t* vals_alt, int64_t n, int nbatch, int npasses, void* tmp,
+                     int* result_in_alt);
+
 // exclusive prefix sum of uint32 (offsets wrap mod 2^32; the grand total is returned in 64 bits
 // so callers can detect the wrap).  In-place capable (out may equal in).
 // `tmp` needs (n/2048 + 2) * 4 bytes.

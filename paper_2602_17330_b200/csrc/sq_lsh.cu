@@ -57,6 +57,38 @@ band_key_kernel(const uint32_t* __restrict__ sig, int64_t n, int H, int bands, i
   nonempty[i] = (all != SQ_EMPTY_SIG) ? 1u : 0u;
 }
 
+// rows == 4 (every BASELINE config): a band is one aligned 16-byte chunk of the signature row.
+// Four bands (four independent 16-byte loads) are in flight per step.
+__global__ void __launch_bounds__(256)
+band_key4_kernel(const uint32_t* __restrict__ sig, int64_t n, int H, int bands,
+                 uint64_t* __restrict__ keys, uint32_t* __restrict__ ids,
+                 uint32_t* __restrict__ nonempty) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const uint4* __restrict__ row = reinterpret_cast<const uint4*>(sig + i * H);
+  uint32_t all = 0xFFFFFFFFu;
+  for (int j = bands; j < H / 4; ++j) { const uint4 v = row[j]; all &= v.x & v.y & v.z & v.w; }
+  for (int b0 = 0; b0 < bands; b0 += 4) {
+    uint4 v[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) v[q] = b0 + q < bands ? row[b0 + q] : make_uint4(0, 0, 0, 0);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      if (b0 + q < bands) {
+        all &= v[q].x & v[q].y & v[q].z & v[q].w;
+        uint64_t acc = kKeyInit;
+        acc = (acc ^ (uint64_t)v[q].x) * kKeyMult; acc ^= acc >> 29;
+        acc = (acc ^ (uint64_t)v[q].y) * kKeyMult; acc ^= acc >> 29;
+        acc = (acc ^ (uint64_t)v[q].z) * kKeyMult; acc ^= acc >> 29;
+        acc = (acc ^ (uint64_t)v[q].w) * kKeyMult; acc ^= acc >> 29;
+        keys[(int64_t)(b0 + q) * n + i] = acc;
+        ids[(int64_t)(b0 + q) * n + i] = (uint32_t)i;
+      }
+    }
+  }
+  nonempty[i] = (all != SQ_EMPTY_SIG) ? 1u : 0u;
+}
+
 // drop the records of empty signatures: record of sequence i moves to slot rank[i]
 __global__ void __launch_bounds__(256)
 compact_kernel(const uint64_t* __restrict__ keys_in, const uint32_t* __restrict__ rank,
@@ -879,7 +911,10 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
 
   // a3: band keys + non-empty flags
   const unsigned gb = (unsigned)((n + 255) / 256);
-  SQ_TIMED(c, SQ_K_BANDKEY, band_key_kernel<<<gb, 256, 0, st>>>(sig, n, H, bands, rows, k0, v0, nonempty));
+  if (rows == 4 && (H & 3) == 0 && (reinterpret_cast<uintptr_t>(sig) & 15) == 0)
+    SQ_TIMED(c, SQ_K_BANDKEY, band_key4_kernel<<<gb, 256, 0, st>>>(sig, n, H, bands, k0, v0, nonempty));
+  else
+    SQ_TIMED(c, SQ_K_BANDKEY, band_key_kernel<<<gb, 256, 0, st>>>(sig, n, H, bands, rows, k0, v0, nonempty));
   SQ_LAUNCH_CHECK(c);
   int rc = sq_exclusive_scan_u32(c, nonempty, nonempty, n, reinterpret_cast<uint32_t*>(tmp),
                                  counters + 2);
@@ -896,10 +931,14 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
   }
   // a4: stable radix sort of every band's records by the 64-bit key
   {
-    int shifts[8], widths[8];
-    for (int p = 0; p < 8; ++p) { shifts[p] = 8 * p; widths[p] = 8; }
     int in_alt = 0;
-    rc = sq_radix_sort(c, kin, kalt, vin, valt, n2, bands, shifts, widths, 8, tmp, &in_alt);
+    if (n2 < (1ll << 30)) {
+      rc = sq_onesweep_sort(c, kin, kalt, vin, valt, n2, bands, 8, tmp, &in_alt);
+    } else {
+      int shifts[8], widths[8];
+      for (int p = 0; p < 8; ++p) { shifts[p] = 8 * p; widths[p] = 8; }
+      rc = sq_radix_sort(c, kin, kalt, vin, valt, n2, bands, shifts, widths, 8, tmp, &in_alt);
+    }
     if (rc != SQ_OK) return rc;
     if (in_alt) { uint64_t* t = kin; kin = kalt; kalt = t; uint32_t* tv = vin; vin = valt; valt = tv; }
   }
