@@ -29,6 +29,9 @@ from paper_2602_17330_b200 import shard  # noqa: E402
 METRIC = "candidate_pairs_verified_per_s"
 UNIT = "pairs/s"
 ALU_OPS_PER_COLUMN_WORD = 7         # ALU-pipe logic ops of one Myers/Hyyro column step
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
+# committed `ncu --set full` capture of this very command line (profiles/r1_v22_top_config4.md)
+NCU_TRAFFIC_BYTES = {("config4", 10_000_000, "edit_distance"): 57.245364e9 + 3.723914e9}
 # bounded oracle samples (first n_s sequences of the same workload)
 ORACLE_SAMPLE = {"config1": 2000, "config2": 100_000, "config3": 300_000, "config4": 300_000}
 CAP_PER_SEQ = {"config2": 40, "config3": 60, "config4": 200}
@@ -356,16 +359,17 @@ def run_ours(args):
     K = args.steps
     rec = n * B                                    # (sequence, band) records
     sw = 4 * (1 if B <= 4 else 2 if B <= 8 else 4 if B <= 16 else 8)   # S row width (words)
-    alg_bytes = {   # algorithmic bytes per STEP of each kernel class (DESIGN.md "Kernels")
+    alg_bytes = {   # algorithmic bytes per STEP of each kernel class (DESIGN.md 5)
         "pack": total_len + 8 * (n + 1) + n * stride + 12 * n,
         "minhash": n * (stride + 4 + 4 * P["H"]),
         "band_key": n * (4 * P["H"] + 12 * B + 4),
-        "sort_hist": 8 * (8 * rec + n),            # 8 key passes of the LSH sort + pack's 1 pass
+        "sort_hist": 8 * (rec + n),                # keys read once for all digit histograms
         "sort_scatter": 24 * (8 * rec + n),        # read + write (key 8 B, id 4 B) per pass
-        "scan": 12 * (rec + 2 * n),                # counts -> offsets; flag scans (read 2x, write 1x)
-        "bucket_scan": rec * (8 + 4 + 4),          # keys + ids in, S out
-        "emit": 2 * rec * (4 + 4 * sw) + 4 * rec + 4 * rec + 4 * cnt,   # 2 passes: ids + S rows; counts; offsets; partners
+        "scan": 12 * (rec + 4 * n),                # counts -> offsets; per-sequence scans
+        "bucket_scan": rec * (8 + 4 + 4) + rec * 12 + 8 * n,   # keys + ids in, S out; id -> internal row
+        "emit": rec * (4 + 4 * sw) + 8 * rec + 4 * cnt,        # ids + S rows; counts out, offsets in; partners out
         "row_sort": 4 * cnt + 4 * rec + 8 * cnt,   # partners + offsets in, pairs out
+        "misc": 16 * (cnt // 32) + 12 * n,         # chunk schedule of the edit-distance stage
     }
     kernels = {}
     tot_prof = sum(ms for ms, _ in prof.values()) or 1.0
@@ -398,6 +402,9 @@ def run_ours(args):
         roof = {"kernel": dom, "bound": "hbm", "achieved": kd.get("achieved_GBs"), "peak": hbm_peak,
                 "unit": "GB/s", "frac": kd.get("frac"), "traffic": None, "peak_source": peak_src}
     roof["avg_launch_ms"] = kd["ms_per_step"] / max(kd["launches_per_step"], 1)
+    roof["traffic"] = NCU_TRAFFIC_BYTES.get((workload, n, dom))
+    if roof["traffic"] is not None:
+        roof["traffic_source"] = "profiles/r1_v22_top_config4.md (ncu --set full, bytes per launch)"
 
     cpu = None if args.no_cpu_baseline else cpu_baseline(rep, workload, P)
     line = {
