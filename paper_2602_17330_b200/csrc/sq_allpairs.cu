@@ -71,6 +71,97 @@ all_pairs_kernel(const uint8_t* __restrict__ packed, int stride, int64_t n, int 
   }
 }
 
+
+// ---- thresholded path, phase 1: the bag-distance filter -----------------------------------------
+// d(a, b) >= bag(a, b) = max(|A minus B|, |B minus A|) over the residue multisets = (L1 + |m - n|) / 2
+// with L1 the L1 distance of the residue histograms: an edit changes one count by one (indel) or
+// two counts by one each (substitution).  A pair whose bag distance exceeds max_d cannot be a hit,
+// so it is dropped before any DP.  The histograms (<= 32 residues, one byte each: 8 words) are
+// compared with 8 byte-wise sum-of-absolute-differences instructions.
+__global__ void __launch_bounds__(256)
+residue_hist_kernel(const uint8_t* __restrict__ packed, int stride, int64_t n,
+                    uint32_t* __restrict__ rh, uint32_t* __restrict__ lens) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const uint32_t* __restrict__ row = reinterpret_cast<const uint32_t*>(packed + i * stride);
+  const int nw = stride >> 2;
+  const uint32_t lastw = row[nw - 1];
+  lens[i] = lastw >> 24;
+  uint32_t h[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  for (int wi = 0; wi < nw; ++wi) {
+    uint32_t word = row[wi];
+    if (wi == nw - 1) word |= 0xFF000000u;                 // the length byte is not a residue
+    if (word == 0xFFFFFFFFu) continue;                     // padding only
+#pragma unroll
+    for (int c = 0; c < 32; ++c) {
+      const uint32_t eq = __vcmpeq4(word, (uint32_t)c * 0x01010101u);   // 0xFF per equal byte
+      h[c >> 2] += (__popc(eq) >> 3) << (8 * (c & 3));
+    }
+  }
+#pragma unroll
+  for (int q = 0; q < 8; ++q) rh[i * 8 + q] = h[q];
+}
+
+__global__ void __launch_bounds__(kApThreads)
+all_pairs_filter_kernel(const uint32_t* __restrict__ rh, const uint32_t* __restrict__ lens, int64_t n,
+                        int max_d, uint2* __restrict__ surv, unsigned long long scap,
+                        unsigned long long* __restrict__ counter) {
+  const int64_t i = blockIdx.x;
+  const int64_t jbase = (int64_t)blockIdx.y * kApThreads;
+  if (jbase + kApThreads <= i + 1) return;                 // whole block below / on the diagonal
+  const uint4* __restrict__ rh4 = reinterpret_cast<const uint4*>(rh);
+  const uint4 a0 = rh4[i * 2], a1 = rh4[i * 2 + 1];
+  const int m = (int)lens[i];
+  const int64_t j = jbase + threadIdx.x;
+  bool pass = false;
+  if (j > i && j < n) {
+    const uint4 b0 = rh4[j * 2], b1 = rh4[j * 2 + 1];
+    const int nl = (int)lens[j];
+    uint32_t l1 = __vsadu4(a0.x, b0.x);
+    l1 += __vsadu4(a0.y, b0.y); l1 += __vsadu4(a0.z, b0.z); l1 += __vsadu4(a0.w, b0.w);
+    l1 += __vsadu4(a1.x, b1.x); l1 += __vsadu4(a1.y, b1.y); l1 += __vsadu4(a1.z, b1.z);
+    l1 += __vsadu4(a1.w, b1.w);
+    const int diff = m > nl ? m - nl : nl - m;
+    pass = (int)((l1 + (uint32_t)diff) >> 1) <= max_d;
+  }
+  const uint32_t mask = __ballot_sync(0xFFFFFFFFu, pass);
+  if (mask) {
+    const int lane = threadIdx.x & 31;
+    unsigned long long base = 0;
+    if (lane == __ffs(mask) - 1) base = atomicAdd(counter, (unsigned long long)__popc(mask));
+    base = __shfl_sync(0xFFFFFFFFu, base, __ffs(mask) - 1);
+    if (pass) {
+      const unsigned long long slot = base + __popc(mask & ((1u << lane) - 1u));
+      if (slot < scap) surv[slot] = make_uint2((uint32_t)i, (uint32_t)j);
+    }
+  }
+}
+
+// phase 3: the survivors that are hits, as (i | j << 32, d) records for the final ordering
+__global__ void __launch_bounds__(256)
+hit_compact_kernel(const uint2* __restrict__ surv, const uint16_t* __restrict__ sdist, int64_t ns,
+                   int max_d, uint64_t* __restrict__ hit_pairs, uint32_t* __restrict__ hit_dist,
+                   unsigned long long capacity, unsigned long long* __restrict__ counter) {
+  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int d = p < ns ? (int)sdist[p] : 0xFFFF;
+  const bool hit = p < ns && d <= max_d;
+  const uint32_t mask = __ballot_sync(0xFFFFFFFFu, hit);
+  if (mask) {
+    const int lane = threadIdx.x & 31;
+    unsigned long long base = 0;
+    if (lane == __ffs(mask) - 1) base = atomicAdd(counter, (unsigned long long)__popc(mask));
+    base = __shfl_sync(0xFFFFFFFFu, base, __ffs(mask) - 1);
+    if (hit) {
+      const unsigned long long slot = base + __popc(mask & ((1u << lane) - 1u));
+      if (slot < capacity) {
+        const uint2 pr = surv[p];
+        hit_pairs[slot] = (uint64_t)pr.x | ((uint64_t)pr.y << 32);
+        hit_dist[slot] = (uint32_t)d;
+      }
+    }
+  }
+}
+
 __global__ void narrow_dist_kernel(const uint32_t* __restrict__ in, int64_t n,
                                    uint16_t* __restrict__ out) {
   const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -97,10 +188,18 @@ inline int bits_for(int64_t n) {
 
 }  // namespace
 
-size_t sq_allpairs_scratch_bytes(int64_t, int64_t pair_capacity) {
+// survivors of the bag-distance filter the scratch is sized for (more -> the fused kernel runs)
+static inline size_t sq_survivor_cap(int64_t pair_capacity) {
+  return 4 * (size_t)(pair_capacity > 0 ? pair_capacity : 1) + 65536;
+}
+
+size_t sq_allpairs_scratch_bytes(int64_t n, int64_t pair_capacity) {
   size_t cap = (size_t)(pair_capacity > 0 ? pair_capacity : 1);
+  size_t nn = (size_t)(n > 0 ? n : 1), scap = sq_survivor_cap(pair_capacity);
   return 2 * sq_align_up(cap * 8 + 16) + 2 * sq_align_up(cap * 4 + 16) +
-         sq_sort_scratch_bytes(pair_capacity, 1) + 4096;
+         sq_sort_scratch_bytes(pair_capacity, 1) +
+         sq_align_up(nn * 32 + 16) + sq_align_up(nn * 4 + 16) +          // histograms, lengths
+         sq_align_up(scap * 8 + 16) + sq_align_up(scap * 2 + 16) + 4096;   // survivors, distances
 }
 
 extern "C" int sq_all_pairs(sq_ctx* c, int max_d, uint32_t* pairs_out, uint16_t* dist_out,
@@ -136,7 +235,40 @@ extern "C" int sq_all_pairs(sq_ctx* c, int max_d, uint32_t* pairs_out, uint16_t*
     SQ_CUDA(c, cudaMemsetAsync(c->dflags, 0, 64, st));
   }
   int rc;
-  if (words <= 1) rc = launch_all_pairs<1>(c, max_d, dist_out, hp, hd, capacity);
+  bool filtered = false;
+  if (max_d >= 0) {
+    // phases 1-3: bag-distance filter -> DP on the survivors only -> hits.  If the survivors do
+    // not fit their scratch, the fused kernel below does the whole job instead.
+    const size_t scap = sq_survivor_cap(capacity);
+    uint32_t* rh = sq_scratch<uint32_t>(c, (size_t)n * 8);
+    uint32_t* lens = sq_scratch<uint32_t>(c, (size_t)n);
+    uint2* surv = sq_scratch<uint2>(c, scap);
+    uint16_t* sdist = sq_scratch<uint16_t>(c, scap);
+    if (rh && lens && surv && sdist && c->alphabet <= 32) {
+      SQ_TIMED(c, SQ_K_ALLPAIRS, residue_hist_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(
+          c->packed, c->stride, n, rh, lens));
+      SQ_LAUNCH_CHECK(c);
+      dim3 grid((unsigned)n, (unsigned)((n + kApThreads - 1) / kApThreads));
+      SQ_TIMED(c, SQ_K_ALLPAIRS, all_pairs_filter_kernel<<<grid, kApThreads, 0, st>>>(
+          rh, lens, n, max_d, surv, (unsigned long long)scap, c->dflags + 1));
+      SQ_LAUNCH_CHECK(c);
+      SQ_CUDA(c, cudaMemcpyAsync(c->pinned, c->dflags + 1, 8, cudaMemcpyDeviceToHost, st));
+      SQ_CUDA(c, cudaStreamSynchronize(st));
+      const int64_t ns = (int64_t)c->pinned[0];
+      if ((size_t)ns <= scap) {
+        filtered = true;
+        if (ns > 0) {
+          rc = sq_edit_distance_impl(c, reinterpret_cast<const uint32_t*>(surv), ns, max_d, sdist);
+          if (rc != SQ_OK) return rc;
+          SQ_TIMED(c, SQ_K_ALLPAIRS, hit_compact_kernel<<<(unsigned)((ns + 255) / 256), 256, 0, st>>>(
+              surv, sdist, ns, max_d, hp, hd, (unsigned long long)capacity, c->dflags));
+          SQ_LAUNCH_CHECK(c);
+        }
+      }
+    }
+  }
+  if (filtered) rc = SQ_OK;
+  else if (words <= 1) rc = launch_all_pairs<1>(c, max_d, dist_out, hp, hd, capacity);
   else if (words <= 2) rc = launch_all_pairs<2>(c, max_d, dist_out, hp, hd, capacity);
   else if (words <= 4) rc = launch_all_pairs<4>(c, max_d, dist_out, hp, hd, capacity);
   else if (words <= 5) rc = launch_all_pairs<5>(c, max_d, dist_out, hp, hd, capacity);

@@ -274,3 +274,28 @@ def test_error_codes():
     assert ei.value.code == binding.SQ_ERR_WORKSPACE
     small.close()
     sq.close()
+
+
+def test_all_pairs_bag_filter_and_its_fallback():
+    """Thresholded all-pairs: (a) the bag-distance filter never drops a hit; (b) when more pairs
+    survive the filter than its scratch holds (anagrams: equal histograms, large distances), the
+    fused kernel takes over and the result is the same."""
+    binding, sq = _ctx()
+    rng = np.random.default_rng(11)
+    base = rng.integers(0, 20, 40).astype(np.uint8)
+    seqs = [rng.permutation(base) for _ in range(700)]            # 244,650 pairs, all with bag distance 0
+    seqs += [base.copy(), np.concatenate([base[:20], base[21:]]), np.concatenate([base, [3]])]   # a few true hits
+    rep = dg.from_list(seqs)
+    want_p, want_d = oracle.all_pairs_threshold(rep.seqs, rep.offsets, 3, use_cutoff=True)
+    assert 0 < want_p.shape[0] < 1000
+    for cap in (1000, 100_000):                                   # 69,536 < survivors < 465,536
+        ws = sq.workspace_bytes(binding.OP_ALL_PAIRS, rep.n, int(rep.offsets[-1]), 41, 0, 1, 0, cap)
+        sq.set_workspace(ws)
+        sq.pack(torch.from_numpy(rep.seqs).cuda(), torch.from_numpy(rep.offsets).cuda(), 20, 41)
+        pairs = torch.empty((cap, 2), dtype=torch.int32, device="cuda")
+        dist = torch.empty(cap, dtype=torch.int16, device="cuda")
+        cnt = sq.all_pairs(3, pairs, dist)
+        assert cnt == want_p.shape[0]
+        assert np.array_equal(_u32(pairs)[:cnt], want_p)
+        assert np.array_equal(_u16(dist)[:cnt], want_d)
+    sq.close()
