@@ -41,6 +41,11 @@ def _declare(L):
     L.orc_wagner_fischer_cutoff.argtypes = [u8p, C.c_int, u8p, C.c_int, C.c_int]
     L.orc_edit_distance_pairs.restype = None
     L.orc_edit_distance_pairs.argtypes = [u8p, i64p, u32p, C.c_int64, C.c_int, u16p]
+    L.orc_wagner_fischer_weighted.restype = C.c_int
+    L.orc_wagner_fischer_weighted.argtypes = [u8p, C.c_int, u8p, C.c_int, u8p, C.c_int, C.c_int]
+    L.orc_edit_distance_weighted_pairs.restype = None
+    L.orc_edit_distance_weighted_pairs.argtypes = [u8p, i64p, u32p, C.c_int64, u8p, C.c_int, C.c_int,
+                                                   C.c_int, u16p]
     L.orc_all_pairs_full.restype = None
     L.orc_all_pairs_full.argtypes = [u8p, i64p, C.c_int64, u16p]
     L.orc_all_pairs_threshold.restype = C.c_int64
@@ -118,6 +123,29 @@ def edit_distance_pairs(seqs, offsets, pairs, max_d: int) -> np.ndarray:
         lib().orc_edit_distance_pairs(_p(seqs, C.c_uint8), _p(offsets, C.c_int64),
                                       _p(pairs, C.c_uint32), pairs.shape[0], int(max_d),
                                       _p(out, C.c_uint16))
+    return out
+
+
+def edit_distance_weighted(a, b, sub, indel: int) -> int:
+    """Weighted edit distance (Eq. 46 with a substitution table)."""
+    aa, bb = np.asarray(a, np.uint8), np.asarray(b, np.uint8)
+    sub = np.ascontiguousarray(sub, dtype=np.uint8)
+    assert sub.ndim == 2 and sub.shape[0] == sub.shape[1]
+    return int(lib().orc_wagner_fischer_weighted(_p(_u8(aa), C.c_uint8), int(aa.size),
+                                                 _p(_u8(bb), C.c_uint8), int(bb.size),
+                                                 _p(sub, C.c_uint8), int(sub.shape[0]), int(indel)))
+
+
+def edit_distance_weighted_pairs(seqs, offsets, pairs, sub, indel: int, max_d: int) -> np.ndarray:
+    seqs, offsets = _u8(seqs), _off(offsets)
+    pairs = np.ascontiguousarray(pairs, dtype=np.uint32).reshape(-1, 2)
+    sub = np.ascontiguousarray(sub, dtype=np.uint8)
+    out = np.zeros(pairs.shape[0], np.uint16)
+    if pairs.shape[0]:
+        lib().orc_edit_distance_weighted_pairs(_p(seqs, C.c_uint8), _p(offsets, C.c_int64),
+                                               _p(pairs, C.c_uint32), pairs.shape[0],
+                                               _p(sub, C.c_uint8), int(sub.shape[0]), int(indel),
+                                               int(max_d), _p(out, C.c_uint16))
     return out
 
 

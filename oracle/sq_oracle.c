@@ -139,6 +139,48 @@ int orc_wagner_fischer_cutoff(const uint8_t* a, int la, const uint8_t* b, int lb
   return d > max_d ? max_d + 1 : d;
 }
 
+/* ------------------------------------------------------------------------ */
+/* C1w. Weighted edit distance (reading 22). */
+/* PAPER.md L754 Eq. (46) as printed: D(i,j) = min(D(i-1,j) + deletion_cost,  */
+/* D(i,j-1) + insertion_cost, D(i-1,j-1) + substitution_cost(a_i, b_j)), with */
+/* the substitution cost taken from a table ("typically based on biochemical  */
+/* similarity", L760) and one common insertion/deletion cost `indel`.         */
+/* Boundary D[x][0] = x*indel, D[0][y] = y*indel.  sub is [sigma][sigma],     */
+/* row = residue of a, column = residue of b.  Wagner-Fischer, written out.   */
+/* ------------------------------------------------------------------------ */
+int orc_wagner_fischer_weighted(const uint8_t* a, int la, const uint8_t* b, int lb,
+                                const uint8_t* sub, int sigma, int indel) {
+  int* prev = (int*)malloc(sizeof(int) * (size_t)(lb + 1));
+  int* cur = (int*)malloc(sizeof(int) * (size_t)(lb + 1));
+  for (int y = 0; y <= lb; ++y) prev[y] = y * indel;
+  for (int x = 1; x <= la; ++x) {
+    cur[0] = x * indel;
+    for (int y = 1; y <= lb; ++y) {
+      int del = prev[y] + indel;
+      int ins = cur[y - 1] + indel;
+      int sb = prev[y - 1] + (int)sub[(int)a[x - 1] * sigma + (int)b[y - 1]];
+      int m = del < ins ? del : ins;
+      cur[y] = m < sb ? m : sb;
+    }
+    int* t = prev; prev = cur; cur = t;
+  }
+  int d = prev[lb];
+  free(prev); free(cur);
+  return d;
+}
+
+void orc_edit_distance_weighted_pairs(const uint8_t* seqs, const int64_t* off, const uint32_t* pairs,
+                                      int64_t n_pairs, const uint8_t* sub, int sigma, int indel,
+                                      int max_d, uint16_t* dist_out) {
+#pragma omp parallel for schedule(dynamic, 1024)
+  for (int64_t p = 0; p < n_pairs; ++p) {
+    uint32_t i = pairs[2 * p], j = pairs[2 * p + 1];
+    int d = orc_wagner_fischer_weighted(seqs + off[i], (int)(off[i + 1] - off[i]),
+                                        seqs + off[j], (int)(off[j + 1] - off[j]), sub, sigma, indel);
+    dist_out[p] = saturate(d, max_d);
+  }
+}
+
 /* exhaustive all pairs with threshold: hits (i<j, d <= max_d) in ascending (i,j) order.
  * use_cutoff = 0: Tier A (full Wagner-Fischer); 1: Tier B (cut-off DP).
  * Returns the number of hits; writes at most `capacity` of them. */

@@ -32,6 +32,7 @@ void sq_destroy(sq_ctx* c) {
     delete[] c->prof_ev;
   }
   if (c->pinned) cudaFreeHost(c->pinned);
+  if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
   delete c;
 }
 
@@ -176,13 +177,20 @@ int sq_pipeline_host(sq_ctx* c, const uint8_t* seqs_host, const int64_t* offsets
     if ((rc = sq_minhash(c, k, H, seed, d_sig)) != SQ_OK) break;
     if ((rc = sq_lsh_candidates(c, d_sig, H, bands, rows, bucket_cap, SQ_LSH_SORTED, d_pairs,
                                 capacity, n_pairs)) != SQ_OK) break;
-    if ((rc = sq_edit_distance(c, d_pairs, *n_pairs, max_d, d_dist)) != SQ_OK) break;
-    if (*n_pairs > 0) {
-      if (cudaMemcpyAsync(pairs_out_host, d_pairs, (size_t)*n_pairs * 8, cudaMemcpyDeviceToHost,
-                          c->stream) != cudaSuccess) { rc = SQ_ERR_CUDA; break; }
-      if (cudaMemcpyAsync(dist_out_host, d_dist, (size_t)*n_pairs * 2, cudaMemcpyDeviceToHost,
-                          c->stream) != cudaSuccess) { rc = SQ_ERR_CUDA; break; }
+    // sq_lsh_candidates has synchronised: the pairs are final.  Their copy to the host (the bulk
+    // of the output) runs on a second stream while the DP kernel works on the first.
+    if (!c->copy_stream &&
+        cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) != cudaSuccess) {
+      rc = SQ_ERR_CUDA; break;
     }
+    if (*n_pairs > 0 &&
+        cudaMemcpyAsync(pairs_out_host, d_pairs, (size_t)*n_pairs * 8, cudaMemcpyDeviceToHost,
+                        c->copy_stream) != cudaSuccess) { rc = SQ_ERR_CUDA; break; }
+    if ((rc = sq_edit_distance(c, d_pairs, *n_pairs, max_d, d_dist)) != SQ_OK) break;
+    if (*n_pairs > 0 &&
+        cudaMemcpyAsync(dist_out_host, d_dist, (size_t)*n_pairs * 2, cudaMemcpyDeviceToHost,
+                        c->stream) != cudaSuccess) { rc = SQ_ERR_CUDA; break; }
+    if (cudaStreamSynchronize(c->copy_stream) != cudaSuccess) { rc = SQ_ERR_CUDA; break; }
     if (cudaStreamSynchronize(c->stream) != cudaSuccess) { rc = SQ_ERR_CUDA; break; }
   } while (0);
   if (rc == SQ_ERR_CUDA) c->last_err = cudaGetLastError();

@@ -19,6 +19,7 @@ constexpr int kSqProfSlots = 1024;
 struct sq_ctx {
   int device = 0;
   cudaStream_t stream = nullptr;
+  cudaStream_t copy_stream = nullptr;   // sq_pipeline_host: device->host copy of the pairs, beside the DP
   int sm_count = 148;
   // workspace arena: [0, persist) holds the packed copy, [persist, ws_bytes) is per-call scratch
   uint8_t* ws = nullptr;

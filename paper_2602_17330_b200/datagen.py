@@ -296,3 +296,31 @@ PARAMS = {
 GENERATORS = {"config1": config1, "config2": config2, "config3": config3,
               "config4": config4, "config5": config5}
 DEFAULT_SEED64 = 0x5EED5EED12345678  # MinHash seed used by tests and bench
+
+
+# ---------------------------------------------------------------------------
+# substitution-cost tables for the weighted edit distance (an INPUT of the path;
+# the paper prints no matrix: "typically based on biochemical similarity", L760)
+# ---------------------------------------------------------------------------
+RESIDUE_CLASSES = ("AGSTP", "ILVMC", "FWYH", "DENQ", "KR")   # small / aliphatic / aromatic / acid+amide / basic
+
+
+def class_substitution_costs(same_class: int = 1, other_class: int = 2) -> np.ndarray:
+    """uint8[20][20]: 0 on the diagonal, `same_class` inside a physico-chemical class,
+    `other_class` across classes.  With 1 <= same <= other <= 2*same it is a metric."""
+    cls = np.zeros(SIGMA, np.int32)
+    for k, members in enumerate(RESIDUE_CLASSES):
+        for ch in members:
+            cls[ALPHABET.index(ch)] = k
+    cost = np.where(cls[:, None] == cls[None, :], same_class, other_class).astype(np.uint8)
+    np.fill_diagonal(cost, 0)
+    return cost
+
+
+def random_substitution_costs(sigma: int, lo: int, hi: int, seed: int) -> np.ndarray:
+    """uint8[sigma][sigma], zero diagonal, symmetric, off-diagonal uniform in [lo, hi]."""
+    rng = np.random.default_rng(seed)
+    c = rng.integers(lo, hi + 1, (sigma, sigma)).astype(np.uint8)
+    c = np.triu(c, 1)
+    c = c + c.T
+    return c.astype(np.uint8)
