@@ -325,6 +325,27 @@ def run_ours(args):
     step_ms_all, tot = shard.aggregate(step_ms, {"pairs": cnt, "seqs": n, "cells": cells}, dev)
     cnt_all, n_all, cells_all = tot["pairs"], tot["seqs"], tot["cells"]
 
+    # ---- next-1: weighted edit distance on the same candidates, timed beside the path
+    weighted = None
+    try:
+        sub_d = torch.from_numpy(dg.class_substitution_costs()).to(dev)
+        wd = torch.empty_like(dist_out)
+        sq.edit_distance_weighted(pairs, cnt, sub_d, 1, 2 * P["max_d"], wd)
+        torch.cuda.synchronize()
+        tw_ms = []
+        for _ in range(3):
+            flush.fill_(1); torch.cuda.synchronize()
+            a, b = ev(), ev()
+            a.record(); sq.edit_distance_weighted(pairs, cnt, sub_d, 1, 2 * P["max_d"], wd); b.record()
+            b.synchronize(); tw_ms.append(a.elapsed_time(b))
+        tw = sum(tw_ms) / len(tw_ms)
+        weighted = {"ms": tw, "pairs_per_s": cnt / (tw * 1e-3), "gcups": cells / (tw * 1e-3) / 1e9,
+                    "table": "class costs 0/1/2, indel 1, max_d %d" % (2 * P["max_d"]),
+                    "hits": int((wd[:cnt] <= 2 * P["max_d"]).sum().item())}
+        del wd
+    except Exception as ex:
+        weighted = {"error": repr(ex)[:200]}
+
     # ---- e2e: through the C ABI with HOST buffers -------------------------------------------
     e2e = None
     if not args.no_e2e:
@@ -431,6 +452,7 @@ def run_ours(args):
                    "edit_pairs_per_s": cnt / (st_ms[3] * 1e-3),
                    "edit_gcups": cells / (st_ms[3] * 1e-3) / 1e9,
                    "wall_s_timed_region": wall},
+        "weighted_edit_distance": weighted,
         "roofline": roof, "kernels": kernels, "int_peak_ops_per_s": int_peak,
         "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
     }

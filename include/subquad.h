@@ -132,6 +132,16 @@ int  sq_lsh_candidates(sq_ctx* ctx, const uint32_t* sig, int H, int bands, int r
 int  sq_edit_distance(sq_ctx* ctx, const uint32_t* pairs, int64_t n_pairs, int max_d,
                       uint16_t* dist_out);
 
+/* next-1  Weighted edit distance: Eq. 46 as printed, with
+ * substitution_cost(a, b) from a table ("typically based on biochemical similarity", L760) and
+ * one insertion/deletion cost; boundary D[x][0] = x*indel, D[0][y] = y*indel.
+ * sub_cost: DEVICE uint8[alphabet][alphabet] row-major (alphabet = the one given to sq_pack),
+ * entry [a][b] = cost of substituting residue a of sequence pairs[p][0] by residue b of sequence
+ * pairs[p][1]; the diagonal is normally 0 but is used as given.  1 <= indel <= 255.
+ * dist_out[p] = min(d, max_d + 1) for max_d >= 0, else min(d, 65535).  Asynchronous. */
+int  sq_edit_distance_weighted(sq_ctx* ctx, const uint32_t* pairs, int64_t n_pairs,
+                               const uint8_t* sub_cost, int indel, int max_d, uint16_t* dist_out);
+
 /* a7  Exhaustive tile path over all i<j (Eq. 45, read as a self-join).
  * max_d < 0 : dist_out = uint16[n(n-1)/2], condensed row-major (0,1),(0,2)..(n-2,n-1);
  *             pairs_out ignored (may be NULL); capacity must be >= n(n-1)/2.

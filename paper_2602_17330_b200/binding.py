@@ -23,7 +23,7 @@ OP_PACK, OP_MINHASH, OP_LSH, OP_EDIT_DISTANCE, OP_ALL_PAIRS, OP_PIPELINE_HOST = 
 LSH_SORTED, LSH_UNORDERED = 0, 1
 
 EXPORTS = ["sq_create", "sq_destroy", "sq_workspace_bytes", "sq_set_workspace", "sq_pack",
-           "sq_minhash", "sq_lsh_candidates", "sq_edit_distance", "sq_all_pairs",
+           "sq_minhash", "sq_lsh_candidates", "sq_edit_distance", "sq_edit_distance_weighted", "sq_all_pairs",
            "sq_pipeline_host", "sq_packed_n", "sq_packed_stride", "sq_last_raw_pairs",
            "sq_kernel_launches", "sq_last_cuda_error", "sq_strerror", "sq_int_peak",
            "sq_profile_enable", "sq_profile_reset", "sq_profile_read", "sq_profile_name"]
@@ -72,6 +72,8 @@ def load_library():
     L.sq_lsh_candidates.argtypes = [vp, vp, i32, i32, i32, i32, i32, vp, i64, C.POINTER(i64)]
     L.sq_edit_distance.restype = i32
     L.sq_edit_distance.argtypes = [vp, vp, i64, i32, vp]
+    L.sq_edit_distance_weighted.restype = i32
+    L.sq_edit_distance_weighted.argtypes = [vp, vp, i64, vp, i32, i32, vp]
     L.sq_all_pairs.restype = i32
     L.sq_all_pairs.argtypes = [vp, i32, vp, vp, i64, C.POINTER(i64)]
     L.sq_pipeline_host.restype = i32
@@ -205,6 +207,16 @@ class SubQuad:
         self._check(self.lib.sq_edit_distance(self.h, _dev_ptr(pairs, torch.int32, "pairs"),
                                               n_pairs, max_d,
                                               _dev_ptr(dist_out, torch.int16, "dist_out")))
+        return dist_out
+
+    def edit_distance_weighted(self, pairs, n_pairs, sub_cost, indel, max_d, dist_out=None):
+        """sub_cost: uint8 CUDA tensor [alphabet, alphabet]."""
+        if dist_out is None:
+            dist_out = torch.empty(max(n_pairs, 1), dtype=torch.int16, device=self.device)
+        self._check(self.lib.sq_edit_distance_weighted(
+            self.h, _dev_ptr(pairs, torch.int32, "pairs"), n_pairs,
+            _dev_ptr(sub_cost, torch.uint8, "sub_cost"), indel, max_d,
+            _dev_ptr(dist_out, torch.int16, "dist_out")))
         return dist_out
 
     def all_pairs(self, max_d, pairs_out, dist_out):

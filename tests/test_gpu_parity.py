@@ -299,3 +299,58 @@ def test_all_pairs_bag_filter_and_its_fallback():
         assert np.array_equal(_u32(pairs)[:cnt], want_p)
         assert np.array_equal(_u16(dist)[:cnt], want_d)
     sq.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# next-1: weighted edit distance (substitution table + indel cost)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("table,indel", [("class", 1), ("class3", 2), ("random", 3), ("unit", 1)])
+def test_weighted_edit_distance_short_sequences(table, indel):
+    binding, sq = _ctx()
+    rep = dg.config2(20_011, seed=6)                      # lengths 5..28, one 32-byte slot
+    _pack(sq, binding, rep, op=binding.OP_EDIT_DISTANCE)
+    rng = np.random.default_rng(7)
+    # pairs grouped by i (like LSH output) plus fully random ones (many runs per warp)
+    ii = np.repeat(rng.integers(0, rep.n, 3000), rng.integers(1, 90, 3000))
+    grouped = np.stack([ii, rng.integers(0, rep.n, ii.size)], 1)
+    pl = np.concatenate([grouped, rng.integers(0, rep.n, (40_003, 2))]).astype(np.uint32)
+    cost = {"class": dg.class_substitution_costs(), "class3": dg.class_substitution_costs(2, 3),
+            "random": dg.random_substitution_costs(20, 1, 9, 5),
+            "unit": (1 - np.eye(20)).astype(np.uint8)}[table]
+    sub = torch.from_numpy(cost).cuda()
+    pt = torch.from_numpy(pl.view(np.int32)).cuda()
+    for md in (-1, 3, 10):
+        want = oracle.edit_distance_weighted_pairs(rep.seqs, rep.offsets, pl, cost, indel, md)
+        d = sq.edit_distance_weighted(pt, pl.shape[0], sub, indel, md)
+        assert np.array_equal(_u16(d)[:pl.shape[0]], want)
+    if table == "unit":                                   # reduces to the bit-parallel kernel
+        d1 = sq.edit_distance(pt, pl.shape[0], -1)
+        d2 = sq.edit_distance_weighted(pt, pl.shape[0], sub, 1, -1)
+        assert torch.equal(d1[:pl.shape[0]], d2[:pl.shape[0]])
+    sq.close()
+
+
+def test_weighted_edit_distance_long_and_tiny_sequences():
+    binding, sq = _ctx()
+    rng = np.random.default_rng(8)
+    rep = dg.config5(1_000, seed=3)                       # lengths 100..140: the general kernel
+    _pack(sq, binding, rep, op=binding.OP_EDIT_DISTANCE)
+    pl = rng.integers(0, rep.n, (6_001, 2)).astype(np.uint32)
+    cost = dg.class_substitution_costs()
+    want = oracle.edit_distance_weighted_pairs(rep.seqs, rep.offsets, pl, cost, 1, 40)
+    d = sq.edit_distance_weighted(torch.from_numpy(pl.view(np.int32)).cuda(), pl.shape[0],
+                                  torch.from_numpy(cost).cuda(), 1, 40)
+    assert np.array_equal(_u16(d)[:pl.shape[0]], want)
+    # tiny and empty sequences, 16-byte slots
+    seqs = [[], [3], [3, 4], [4, 3], [1, 2, 3, 4, 5, 6, 7], [7, 6, 5, 4, 3, 2, 1], [0] * 15, [19] * 15]
+    rep2 = dg.from_list(seqs)
+    _pack(sq, binding, rep2, op=binding.OP_EDIT_DISTANCE, max_len=15)
+    n = rep2.n
+    pl2 = np.array([(i, j) for i in range(n) for j in range(n)], np.uint32)
+    cost2 = dg.random_substitution_costs(20, 1, 200, 9)
+    for indel in (1, 7, 255):
+        want = oracle.edit_distance_weighted_pairs(rep2.seqs, rep2.offsets, pl2, cost2, indel, -1)
+        d = sq.edit_distance_weighted(torch.from_numpy(pl2.view(np.int32)).cuda(), pl2.shape[0],
+                                      torch.from_numpy(cost2).cuda(), indel, -1)
+        assert np.array_equal(_u16(d)[:pl2.shape[0]], want)
+    sq.close()
