@@ -55,6 +55,7 @@ extern "C" {
 #define SQ_OP_EDIT_DISTANCE   3
 #define SQ_OP_ALL_PAIRS       4
 #define SQ_OP_PIPELINE_HOST   5
+#define SQ_OP_GRAPH           6   /* sizes->pair_capacity = number of pairs handed to the graph */
 
 /* flags of sq_lsh_candidates */
 #define SQ_LSH_SORTED     0   /* pairs_out ascending by (i, j) (default)                      */
@@ -141,6 +142,21 @@ int  sq_edit_distance(sq_ctx* ctx, const uint32_t* pairs, int64_t n_pairs, int m
  * dist_out[p] = min(d, max_d + 1) for max_d >= 0, else min(d, 65535).  Asynchronous. */
 int  sq_edit_distance_weighted(sq_ctx* ctx, const uint32_t* pairs, int64_t n_pairs,
                                const uint8_t* sub_cost, int indel, int max_d, uint16_t* dist_out);
+
+/* next-2  Verified candidates -> sparse similarity graph G = (V, E, W) (
+ * PAPER.md L71-73 Eq. 1, L185 Alg. 1 step 12; Jaccard estimate from the sketches L495-497 Eq. 30,
+ * thresholded at tau = 0.7 in L269 / L638).  Edge (i, j), i < j, is kept iff dist[p] <= max_d AND
+ * the signatures of i and j agree in at least `min_matches` of the H columns (the caller passes
+ * min_matches = ceil(tau * H); 0 = no sketch filter, sig may then be NULL).
+ * weight = 1 - d / max(len_i, len_j) in fp32 (1 for two empty sequences).
+ * pairs/dist: as produced by sq_lsh_candidates + sq_edit_distance (first index non-decreasing).
+ * Output, device: row_ptr int64[n+1], col uint32[capacity] (ascending inside a row when the pairs
+ * are SQ_LSH_SORTED), weight float[capacity]: the upper-triangular CSR.  *n_edges (host).
+ * Uses the workspace scratch (4 bytes per pair + 4 per sequence).  Synchronises.
+ * SQ_ERR_CAPACITY if *n_edges > capacity (row_ptr is still complete). */
+int  sq_affinity_graph(sq_ctx* ctx, const uint32_t* pairs, const uint16_t* dist, int64_t n_pairs,
+                       int max_d, const uint32_t* sig, int H, int min_matches, int64_t* row_ptr,
+                       uint32_t* col, float* weight, int64_t capacity, int64_t* n_edges);
 
 /* a7  Exhaustive tile path over all i<j (Eq. 45, read as a self-join).
  * max_d < 0 : dist_out = uint16[n(n-1)/2], condensed row-major (0,1),(0,2)..(n-2,n-1);

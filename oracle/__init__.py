@@ -249,3 +249,30 @@ def lsh_row(sig, bands: int, rows: int, cap: int, i: int) -> np.ndarray:
     tot = int(lib().orc_lsh_row(_p(sig, C.c_uint32), n, H, bands, rows, cap, int(i),
                                 _p(out, C.c_uint32), out.size))
     return out[:tot].copy()
+
+
+# ---- next-2: verified candidates -> sparse similarity graph (plain numpy, fp64) ----------------
+
+def affinity_graph(pairs, dist, max_d: int, sig, min_matches: int, lengths, n: int):
+    """Upper-triangular CSR of the similarity graph (Eq. 1; L185; Jaccard estimate
+    from the sketches L495-497 Eq. 30 thresholded as an integer count of equal columns).
+    Edge (i, j) kept iff dist <= max_d and #{c: sig[i][c] == sig[j][c]} >= min_matches;
+    weight = 1 - d / max(len_i, len_j) in fp64 (1 for two empty sequences).
+    Returns (row_ptr int64[n+1], col uint32[E], weight float64[E]) in the order of `pairs`."""
+    pairs = np.asarray(pairs, dtype=np.uint32).reshape(-1, 2)
+    dist = np.asarray(dist, dtype=np.uint16)
+    keep = dist.astype(np.int64) <= max_d
+    if min_matches > 0:
+        sig = np.asarray(sig, dtype=np.uint32)
+        matches = np.zeros(pairs.shape[0], np.int64)
+        for s in range(0, pairs.shape[0], 1 << 18):               # bounded memory
+            e = min(pairs.shape[0], s + (1 << 18))
+            matches[s:e] = (sig[pairs[s:e, 0]] == sig[pairs[s:e, 1]]).sum(axis=1)
+        keep &= matches >= min_matches
+    kp = pairs[keep]
+    kd = dist[keep].astype(np.float64)
+    L = np.maximum(np.asarray(lengths)[kp[:, 0]], np.asarray(lengths)[kp[:, 1]]).astype(np.float64)
+    weight = np.where(L > 0, 1.0 - kd / np.where(L > 0, L, 1.0), 1.0)
+    row_ptr = np.zeros(n + 1, np.int64)
+    np.cumsum(np.bincount(kp[:, 0], minlength=n), out=row_ptr[1:])
+    return row_ptr, kp[:, 1].copy(), weight

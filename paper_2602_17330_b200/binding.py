@@ -19,11 +19,11 @@ SQ_OK = 0
 SQ_ERR_INVALID_ARG, SQ_ERR_BAD_RESIDUE, SQ_ERR_NOT_PACKED, SQ_ERR_CAPACITY = -1, -2, -3, -4
 SQ_ERR_WORKSPACE, SQ_ERR_UNSUPPORTED, SQ_ERR_CUDA = -5, -6, -7
 SQ_MAX_LEN, SQ_MAX_H, SQ_MAX_BANDS = 240, 256, 32
-OP_PACK, OP_MINHASH, OP_LSH, OP_EDIT_DISTANCE, OP_ALL_PAIRS, OP_PIPELINE_HOST = range(6)
+OP_PACK, OP_MINHASH, OP_LSH, OP_EDIT_DISTANCE, OP_ALL_PAIRS, OP_PIPELINE_HOST, OP_GRAPH = range(7)
 LSH_SORTED, LSH_UNORDERED = 0, 1
 
 EXPORTS = ["sq_create", "sq_destroy", "sq_workspace_bytes", "sq_set_workspace", "sq_pack",
-           "sq_minhash", "sq_lsh_candidates", "sq_edit_distance", "sq_edit_distance_weighted", "sq_all_pairs",
+           "sq_minhash", "sq_lsh_candidates", "sq_edit_distance", "sq_edit_distance_weighted", "sq_affinity_graph", "sq_all_pairs",
            "sq_pipeline_host", "sq_packed_n", "sq_packed_stride", "sq_last_raw_pairs",
            "sq_kernel_launches", "sq_last_cuda_error", "sq_strerror", "sq_int_peak",
            "sq_profile_enable", "sq_profile_reset", "sq_profile_read", "sq_profile_name"]
@@ -74,6 +74,8 @@ def load_library():
     L.sq_edit_distance.argtypes = [vp, vp, i64, i32, vp]
     L.sq_edit_distance_weighted.restype = i32
     L.sq_edit_distance_weighted.argtypes = [vp, vp, i64, vp, i32, i32, vp]
+    L.sq_affinity_graph.restype = i32
+    L.sq_affinity_graph.argtypes = [vp, vp, vp, i64, i32, vp, i32, i32, vp, vp, vp, i64, C.POINTER(i64)]
     L.sq_all_pairs.restype = i32
     L.sq_all_pairs.argtypes = [vp, i32, vp, vp, i64, C.POINTER(i64)]
     L.sq_pipeline_host.restype = i32
@@ -218,6 +220,18 @@ class SubQuad:
             _dev_ptr(sub_cost, torch.uint8, "sub_cost"), indel, max_d,
             _dev_ptr(dist_out, torch.int16, "dist_out")))
         return dist_out
+
+    def affinity_graph(self, pairs, dist, n_pairs, max_d, sig, min_matches, row_ptr, col, weight):
+        """row_ptr int64[n+1], col int32[cap], weight float32[cap] (CUDA).  Returns the edge count."""
+        H = sig.shape[1] if sig is not None else 0
+        cnt = C.c_int64(0)
+        rc = self.lib.sq_affinity_graph(
+            self.h, _dev_ptr(pairs, torch.int32, "pairs"), _dev_ptr(dist, torch.int16, "dist"), n_pairs,
+            max_d, _dev_ptr(sig, torch.int32, "sig"), H, min_matches,
+            _dev_ptr(row_ptr, torch.int64, "row_ptr"), _dev_ptr(col, torch.int32, "col"),
+            _dev_ptr(weight, torch.float32, "weight"), col.shape[0], C.byref(cnt))
+        self._check(rc, required=cnt.value)
+        return cnt.value
 
     def all_pairs(self, max_d, pairs_out, dist_out):
         cnt = C.c_int64(0)

@@ -109,6 +109,7 @@ static inline int sq_stride_for(int max_len) { return ((max_len + 1) + 15) / 16 
 size_t sq_persist_bytes(int64_t n, int max_len);
 size_t sq_lsh_scratch_bytes(int64_t n, int bands, int64_t pair_capacity);
 size_t sq_allpairs_scratch_bytes(int64_t n, int64_t pair_capacity);
+size_t sq_graph_scratch_bytes(int64_t n, int64_t n_pairs);
 size_t sq_sort_scratch_bytes(int64_t n_per_batch, int nbatch);
 
 // ---- radix sort (sq_sort.cu) ----

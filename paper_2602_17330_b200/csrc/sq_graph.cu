@@ -1,0 +1,122 @@
+// sq_graph.cu -- from verified candidates to the sparse similarity graph:
+// PAPER.md L71-73 Eq. (1) G = (V, E, W); Alg. 1 step 12 "build similarity matrix A" (L185); the
+// MinHash Jaccard estimate (L495-497 Eq. 30) thresholded at tau (tau = 0.7 in L269, L638).
+//
+//   edge (i, j), i < j, is kept iff  d(i, j) <= max_d  AND  #{c : sig[i][c] == sig[j][c]} >= min_matches
+//   (the caller turns tau into the integer min_matches = ceil(tau * H), so no floating-point
+//   comparison decides anything);  weight = 1 - d / max(len_i, len_j)  in fp32.
+//
+// Output: upper-triangular CSR -- row_ptr[n+1], col[] ascending inside a row, weight[] -- built
+// from a pair list whose first index is non-decreasing (both orders of sq_lsh_candidates are).
+//   keep_kernel    one warp per pair: the two signature rows are read coalesced (lane = column),
+//                  equal columns counted with a ballot; kept pairs are flagged and counted per row.
+//   scans          flags -> edge slots (stable), row counts -> row_ptr.
+//   edge_kernel    kept pair p -> col / weight at its slot.
+#include "sq_common.cuh"
+
+namespace {
+
+__global__ void __launch_bounds__(256)
+graph_keep_kernel(const uint2* __restrict__ pairs, const uint16_t* __restrict__ dist, int64_t n_pairs,
+                  int max_d, const uint32_t* __restrict__ sig, int H, int min_matches, int64_t n,
+                  uint32_t* __restrict__ keep, uint32_t* __restrict__ row_cnt) {
+  const int lane = threadIdx.x & 31;
+  const int64_t p = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (p >= n_pairs) return;
+  const uint2 pr = pairs[p];
+  bool ok = pr.x < (uint64_t)n && pr.y < (uint64_t)n && (int)dist[p] <= max_d;
+  if (ok && min_matches > 0) {
+    const uint32_t* a = sig + (int64_t)pr.x * H;
+    const uint32_t* b = sig + (int64_t)pr.y * H;
+    int m = 0;
+    for (int c = lane; c < H; c += 32) m += __popc(__ballot_sync(0xFFFFFFFFu, a[c] == b[c]));
+    // (H is a multiple of 32, so every lane runs the same trips and every ballot is full)
+    ok = m >= min_matches;
+  }
+  if (lane == 0) {
+    keep[p] = ok ? 1u : 0u;
+    if (ok) atomicAdd(&row_cnt[pr.x], 1u);
+  }
+}
+
+__global__ void __launch_bounds__(256)
+graph_edge_kernel(const uint2* __restrict__ pairs, const uint16_t* __restrict__ dist, int64_t n_pairs,
+                  const uint32_t* __restrict__ slot, const uint8_t* __restrict__ packed, int stride,
+                  uint32_t* __restrict__ col, float* __restrict__ weight) {
+  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= n_pairs) return;
+  const uint32_t s = slot[p];
+  if (slot[p + 1] == s) return;                 // not kept (the scan covers n_pairs + 1 entries)
+  const uint2 pr = pairs[p];
+  const int la = packed[(int64_t)pr.x * stride + stride - 1], lb = packed[(int64_t)pr.y * stride + stride - 1];
+  const int L = la > lb ? la : lb;
+  col[s] = pr.y;
+  weight[s] = L > 0 ? 1.0f - (float)dist[p] / (float)L : 1.0f;
+}
+
+__global__ void __launch_bounds__(256)
+graph_rowptr_kernel(const uint32_t* __restrict__ row_off, int64_t n, unsigned long long total,
+                    int64_t* __restrict__ row_ptr) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) row_ptr[i] = (int64_t)row_off[i];
+  if (i == n) row_ptr[n] = (int64_t)total;
+}
+
+}  // namespace
+
+size_t sq_graph_scratch_bytes(int64_t n, int64_t n_pairs) {
+  const size_t np = (size_t)(n_pairs > 0 ? n_pairs : 1), nn = (size_t)(n > 0 ? n : 1);
+  return sq_align_up((np + 2) * 4 + 16) + sq_align_up((nn + 2) * 4 + 16) +
+         sq_align_up((np / 2048 + nn / 2048 + 8) * 4 + 16) + 4096;
+}
+
+extern "C" int sq_affinity_graph(sq_ctx* c, const uint32_t* pairs, const uint16_t* dist, int64_t n_pairs,
+                                 int max_d, const uint32_t* sig, int H, int min_matches,
+                                 int64_t* row_ptr, uint32_t* col, float* weight, int64_t capacity,
+                                 int64_t* n_edges) {
+  if (!c || !n_edges || !row_ptr) return SQ_ERR_INVALID_ARG;
+  *n_edges = 0;
+  if (c->n < 0) return SQ_ERR_NOT_PACKED;
+  if (n_pairs < 0 || capacity < 0 || max_d < 0 || min_matches < 0) return SQ_ERR_INVALID_ARG;
+  if (min_matches > 0 && (!sig || H < 32 || (H % 32) != 0 || H > SQ_MAX_H || min_matches > H))
+    return SQ_ERR_INVALID_ARG;
+  if (n_pairs >= (1ll << 32) - 1) return SQ_ERR_UNSUPPORTED;
+  const int64_t n = c->n;
+  cudaStream_t st = c->stream;
+  sq_scratch_reset(c);
+  uint32_t* keep = sq_scratch<uint32_t>(c, (size_t)n_pairs + 2);
+  uint32_t* row_cnt = sq_scratch<uint32_t>(c, (size_t)n + 2);
+  uint32_t* tmp = sq_scratch<uint32_t>(c, (size_t)n_pairs / 2048 + (size_t)n / 2048 + 8);
+  if (!keep || !row_cnt || !tmp) return SQ_ERR_WORKSPACE;
+  SQ_CUDA(c, cudaMemsetAsync(row_cnt, 0, ((size_t)n + 2) * 4, st));
+  SQ_CUDA(c, cudaMemsetAsync(keep + n_pairs, 0, 8, st));
+  SQ_CUDA(c, cudaMemsetAsync(c->dflags, 0, 64, st));
+  if (n_pairs > 0) {
+    if (!pairs || !dist) return SQ_ERR_INVALID_ARG;
+    const int64_t blocks = (n_pairs * 32 + 255) / 256;
+    if (blocks >= (1ll << 31)) return SQ_ERR_UNSUPPORTED;
+    SQ_TIMED(c, SQ_K_MISC, graph_keep_kernel<<<(unsigned)blocks, 256, 0, st>>>(
+        reinterpret_cast<const uint2*>(pairs), dist, n_pairs, max_d, sig, H, min_matches, n, keep, row_cnt));
+    SQ_LAUNCH_CHECK(c);
+    int rc = sq_exclusive_scan_u32(c, keep, keep, n_pairs + 1, tmp, c->dflags);
+    if (rc != SQ_OK) return rc;
+  }
+  int rc = sq_exclusive_scan_u32(c, row_cnt, row_cnt, n, tmp, nullptr);
+  if (rc != SQ_OK) return rc;
+  SQ_CUDA(c, cudaMemcpyAsync(c->pinned, c->dflags, 8, cudaMemcpyDeviceToHost, st));
+  SQ_CUDA(c, cudaStreamSynchronize(st));
+  const int64_t edges = (int64_t)c->pinned[0];
+  *n_edges = edges;
+  SQ_TIMED(c, SQ_K_MISC, graph_rowptr_kernel<<<(unsigned)((n + 256) / 256), 256, 0, st>>>(
+      row_cnt, n, (unsigned long long)edges, row_ptr));
+  SQ_LAUNCH_CHECK(c);
+  if (edges > capacity) { SQ_CUDA(c, cudaStreamSynchronize(st)); return SQ_ERR_CAPACITY; }
+  if (edges > 0) {
+    if (!col || !weight) return SQ_ERR_INVALID_ARG;
+    SQ_TIMED(c, SQ_K_MISC, graph_edge_kernel<<<(unsigned)((n_pairs + 255) / 256), 256, 0, st>>>(
+        reinterpret_cast<const uint2*>(pairs), dist, n_pairs, keep, c->packed, c->stride, col, weight));
+    SQ_LAUNCH_CHECK(c);
+  }
+  SQ_CUDA(c, cudaStreamSynchronize(st));
+  return SQ_OK;
+}

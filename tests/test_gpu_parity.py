@@ -354,3 +354,40 @@ def test_weighted_edit_distance_long_and_tiny_sequences():
                                       torch.from_numpy(cost2).cuda(), indel, -1)
         assert np.array_equal(_u16(d)[:pl2.shape[0]], want)
     sq.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# next-2: verified candidates -> sparse similarity graph
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("flags", [0, 1])
+def test_affinity_graph_against_oracle(flags):
+    binding, sq = _ctx()
+    P = dict(dg.PARAMS["config2"])
+    rep = dg.config2(30_011, seed=12)
+    cap = 1_200_000
+    max_len = int(rep.lengths.max())
+    ws = max(sq.workspace_bytes(binding.OP_LSH, rep.n, int(rep.offsets[-1]), max_len, P["H"], P["bands"],
+                                P["cap"], cap),
+             sq.workspace_bytes(binding.OP_GRAPH, rep.n, 0, max_len, 0, 0, 0, cap))
+    sq.set_workspace(ws)
+    sq.pack(torch.from_numpy(rep.seqs).cuda(), torch.from_numpy(rep.offsets).cuda(), 20, max_len)
+    sig = sq.minhash(P["k"], P["H"], SEED)
+    pairs = torch.empty((cap, 2), dtype=torch.int32, device="cuda")
+    cnt = sq.lsh_candidates(sig, P["bands"], P["rows"], P["cap"], pairs, flags=flags)
+    dist = sq.edit_distance(pairs, cnt, P["max_d"])
+    hp, hd, hs = _u32(pairs)[:cnt].copy(), _u16(dist)[:cnt].copy(), _u32(sig)
+    row_ptr = torch.empty(rep.n + 1, dtype=torch.int64, device="cuda")
+    col = torch.empty(cnt, dtype=torch.int32, device="cuda")
+    wgt = torch.empty(cnt, dtype=torch.float32, device="cuda")
+    for mm in (0, 20, 45, 64):
+        e = sq.affinity_graph(pairs, dist, cnt, P["max_d"], sig, mm, row_ptr, col, wgt)
+        rp, wc, ww = oracle.affinity_graph(hp, hd, P["max_d"], hs, mm, rep.lengths, rep.n)
+        assert e == rp[-1]
+        assert np.array_equal(row_ptr.cpu().numpy(), rp)
+        assert np.array_equal(_u32(col)[:e], wc)
+        # fp32 (1 - d/L, correctly rounded ops) against the fp64 oracle: half an ulp per op
+        assert np.allclose(wgt.cpu().numpy()[:e], ww, rtol=0, atol=1.5e-7)
+    with pytest.raises(binding.SubQuadError) as ei:           # capacity protocol
+        sq.affinity_graph(pairs, dist, cnt, P["max_d"], sig, 0, row_ptr, col[:10], wgt[:10])
+    assert ei.value.code == binding.SQ_ERR_CAPACITY and ei.value.required == (hd <= P["max_d"]).sum()
+    sq.close()
