@@ -246,6 +246,7 @@ def run_ours(args):
                                     P["cap"], cap),
                  0 if args.no_e2e else sq.workspace_bytes(binding.OP_PIPELINE_HOST, n, total_len,
                                                           max_len, P["H"], P["bands"], P["cap"], cap))
+        ws += 4 * cap + 8 * n + (1 << 20)      # room for the graph step's scratch above the LSH scratch
         sq.workspace = None
         sq.set_workspace(ws)
         pairs = torch.empty((cap, 2), dtype=torch.int32, device=dev)
@@ -345,6 +346,27 @@ def run_ours(args):
         del wd
     except Exception as ex:
         weighted = {"error": repr(ex)[:200]}
+
+    # ---- next-2: sparse similarity graph from the verified candidates, tau = 0.7
+    graph = None
+    try:
+        mm = int(np.ceil(0.7 * P["H"]))
+        row_ptr = torch.empty(n + 1, dtype=torch.int64, device=dev)
+        col = torch.empty(cnt, dtype=torch.int32, device=dev)
+        wgt = torch.empty(cnt, dtype=torch.float32, device=dev)
+        edges = sq.affinity_graph(pairs, dist_out, cnt, P["max_d"], sig, mm, row_ptr, col, wgt)
+        tg_ms = []
+        for _ in range(2):
+            flush.fill_(1); torch.cuda.synchronize()
+            a, b = ev(), ev()
+            a.record(); sq.affinity_graph(pairs, dist_out, cnt, P["max_d"], sig, mm, row_ptr, col, wgt); b.record()
+            b.synchronize(); tg_ms.append(a.elapsed_time(b))
+        tg = sum(tg_ms) / len(tg_ms)
+        graph = {"ms": tg, "edges": int(edges), "min_matches": mm, "pairs_per_s": cnt / (tg * 1e-3),
+                 "GBs_algorithmic": (cnt * (10 + 8 * P["H"]) + edges * 8 + 8 * n) / (tg * 1e-3) / 1e9}
+        del row_ptr, col, wgt
+    except Exception as ex:
+        graph = {"error": repr(ex)[:200]}
 
     # ---- e2e: through the C ABI with HOST buffers -------------------------------------------
     e2e = None
@@ -452,7 +474,7 @@ def run_ours(args):
                    "edit_pairs_per_s": cnt / (st_ms[3] * 1e-3),
                    "edit_gcups": cells / (st_ms[3] * 1e-3) / 1e9,
                    "wall_s_timed_region": wall},
-        "weighted_edit_distance": weighted,
+        "weighted_edit_distance": weighted, "affinity_graph": graph,
         "roofline": roof, "kernels": kernels, "int_peak_ops_per_s": int_peak,
         "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
     }

@@ -16,13 +16,53 @@
 
 namespace {
 
+// one pair, whole warp
+__device__ __forceinline__ void graph_keep_one(const uint2* __restrict__ pairs,
+                                               const uint16_t* __restrict__ dist, int64_t p, int max_d,
+                                               const uint32_t* __restrict__ sig, int H, int min_matches,
+                                               int64_t n, uint32_t* __restrict__ keep,
+                                               uint32_t* __restrict__ row_cnt, int lane);
+
+// SCHED: warp k walks positions [32k, 32k+32) of the family-ordered schedule left by
+// sq_lsh_candidates (sq_common.cuh) -- the signature rows of one family stay in L2.
+template <bool SCHED>
 __global__ void __launch_bounds__(256)
 graph_keep_kernel(const uint2* __restrict__ pairs, const uint16_t* __restrict__ dist, int64_t n_pairs,
                   int max_d, const uint32_t* __restrict__ sig, int H, int min_matches, int64_t n,
-                  uint32_t* __restrict__ keep, uint32_t* __restrict__ row_cnt) {
+                  uint32_t* __restrict__ keep, uint32_t* __restrict__ row_cnt,
+                  const uint4* __restrict__ sched, const uint32_t* __restrict__ rowstart,
+                  const uint32_t* __restrict__ delta) {
   const int lane = threadIdx.x & 31;
-  const int64_t p = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  if (p >= n_pairs) return;
+  const int64_t wk = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (!SCHED) {
+    if (wk < n_pairs) graph_keep_one(pairs, dist, wk, max_d, sig, H, min_matches, n, keep, row_cnt, lane);
+    return;
+  }
+  const int64_t q0 = wk * 32;
+  if (q0 >= n_pairs) return;
+  int64_t p = q0 + lane;                              // lane t decodes position q0 + t
+  if (p < n_pairs) {
+    const uint4 ch = sched[wk];
+    const uint32_t q = (uint32_t)p;
+    if (q < ch.z) p = (int64_t)(uint32_t)(ch.y + q);
+    else {
+      uint32_t r = ch.x + 1;
+      while (q >= rowstart[r + 1]) ++r;
+      p = (int64_t)(uint32_t)(delta[r] + q);
+    }
+  }
+  const int cntp = (int)min((int64_t)32, n_pairs - q0);
+  for (int t = 0; t < cntp; ++t) {
+    const int64_t pt = __shfl_sync(0xFFFFFFFFu, p, t);
+    graph_keep_one(pairs, dist, pt, max_d, sig, H, min_matches, n, keep, row_cnt, lane);
+  }
+}
+
+__device__ __forceinline__ void graph_keep_one(const uint2* __restrict__ pairs,
+                                               const uint16_t* __restrict__ dist, int64_t p, int max_d,
+                                               const uint32_t* __restrict__ sig, int H, int min_matches,
+                                               int64_t n, uint32_t* __restrict__ keep,
+                                               uint32_t* __restrict__ row_cnt, int lane) {
   const uint2 pr = pairs[p];
   bool ok = pr.x < (uint64_t)n && pr.y < (uint64_t)n && (int)dist[p] <= max_d;
   if (ok && min_matches > 0) {
@@ -83,20 +123,40 @@ extern "C" int sq_affinity_graph(sq_ctx* c, const uint32_t* pairs, const uint16_
   if (n_pairs >= (1ll << 32) - 1) return SQ_ERR_UNSUPPORTED;
   const int64_t n = c->n;
   cudaStream_t st = c->stream;
-  sq_scratch_reset(c);
-  uint32_t* keep = sq_scratch<uint32_t>(c, (size_t)n_pairs + 2);
-  uint32_t* row_cnt = sq_scratch<uint32_t>(c, (size_t)n + 2);
-  uint32_t* tmp = sq_scratch<uint32_t>(c, (size_t)n_pairs / 2048 + (size_t)n / 2048 + 8);
-  if (!keep || !row_cnt || !tmp) return SQ_ERR_WORKSPACE;
+  // the schedule of sq_lsh_candidates lives in the scratch: keep it (and allocate above it) when
+  // it describes these very pairs and the signatures do not fit the L2
+  bool use_sched = c->sched && c->sched_pairs == pairs && c->sched_npairs == n_pairs &&
+                   min_matches > 0 && (size_t)n * H * 4 > ((size_t)96 << 20);
+  const uint4* sched = c->sched; const uint32_t* srow = c->sched_rowstart; const uint32_t* sdel = c->sched_delta;
+  const size_t top_before = c->scratch_top;
+  uint32_t* keep = nullptr; uint32_t* row_cnt = nullptr; uint32_t* tmp = nullptr;
+  for (int attempt = 0; attempt < 2; ++attempt) {
+    if (!use_sched) sq_scratch_reset(c);
+    keep = sq_scratch<uint32_t>(c, (size_t)n_pairs + 2);
+    row_cnt = sq_scratch<uint32_t>(c, (size_t)n + 2);
+    tmp = sq_scratch<uint32_t>(c, (size_t)n_pairs / 2048 + (size_t)n / 2048 + 8);
+    if (keep && row_cnt && tmp) break;
+    if (!use_sched) return SQ_ERR_WORKSPACE;
+    c->scratch_top = top_before;                     // no room above the schedule: do without it
+    use_sched = false;
+  }
   SQ_CUDA(c, cudaMemsetAsync(row_cnt, 0, ((size_t)n + 2) * 4, st));
   SQ_CUDA(c, cudaMemsetAsync(keep + n_pairs, 0, 8, st));
   SQ_CUDA(c, cudaMemsetAsync(c->dflags, 0, 64, st));
   if (n_pairs > 0) {
     if (!pairs || !dist) return SQ_ERR_INVALID_ARG;
-    const int64_t blocks = (n_pairs * 32 + 255) / 256;
-    if (blocks >= (1ll << 31)) return SQ_ERR_UNSUPPORTED;
-    SQ_TIMED(c, SQ_K_MISC, graph_keep_kernel<<<(unsigned)blocks, 256, 0, st>>>(
-        reinterpret_cast<const uint2*>(pairs), dist, n_pairs, max_d, sig, H, min_matches, n, keep, row_cnt));
+    if (use_sched) {
+      const int64_t blocks = ((n_pairs + 31) / 32 * 32 + 255) / 256;
+      SQ_TIMED(c, SQ_K_MISC, graph_keep_kernel<true><<<(unsigned)blocks, 256, 0, st>>>(
+          reinterpret_cast<const uint2*>(pairs), dist, n_pairs, max_d, sig, H, min_matches, n, keep, row_cnt,
+          sched, srow, sdel));
+    } else {
+      const int64_t blocks = (n_pairs * 32 + 255) / 256;
+      if (blocks >= (1ll << 31)) return SQ_ERR_UNSUPPORTED;
+      SQ_TIMED(c, SQ_K_MISC, graph_keep_kernel<false><<<(unsigned)blocks, 256, 0, st>>>(
+          reinterpret_cast<const uint2*>(pairs), dist, n_pairs, max_d, sig, H, min_matches, n, keep, row_cnt,
+          nullptr, nullptr, nullptr));
+    }
     SQ_LAUNCH_CHECK(c);
     int rc = sq_exclusive_scan_u32(c, keep, keep, n_pairs + 1, tmp, c->dflags);
     if (rc != SQ_OK) return rc;
@@ -118,5 +178,6 @@ extern "C" int sq_affinity_graph(sq_ctx* c, const uint32_t* pairs, const uint16_
     SQ_LAUNCH_CHECK(c);
   }
   SQ_CUDA(c, cudaStreamSynchronize(st));
+  if (use_sched) c->scratch_top = top_before;           // give the scratch above the schedule back
   return SQ_OK;
 }
