@@ -121,12 +121,15 @@ translate_kernel(const uint32_t* __restrict__ ids, int64_t total, const uint32_t
 
 // partners of internal row r over all bands (offsets are band-major: off[b*n2 + r])
 __global__ void __launch_bounds__(256)
-row_total_kernel(const uint32_t* __restrict__ off, int64_t n2, int bands, uint32_t* __restrict__ row_tot) {
+row_total_kernel(const uint32_t* __restrict__ off, const uint2* __restrict__ loc, int64_t n2, int bands,
+                 uint32_t* __restrict__ row_tot) {
   const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (r > n2) return;
   uint32_t t = 0;
-  if (r < n2)
-    for (int b = 0; b < bands; ++b) t += off[(int64_t)b * n2 + r + 1] - off[(int64_t)b * n2 + r];
+  if (r < n2) {
+    t = off[r + 1] - off[r];                       // band 0: the record of row r is record r
+    for (int b = 1; b < bands; ++b) t += loc[(int64_t)b * n2 + r].y;
+  }
   row_tot[r] = t;                              // row_tot[n2] = 0: the scan leaves the total there
 }
 
@@ -419,18 +422,19 @@ struct EmDesc { uint32_t u, g0, mrem, c0; int b; bool ok; };
 // BW = 16-byte chunks per S row (S row width SW = 4*BW >= bands).
 // ids = external sequence ids of the sorted records (the values that are emitted); ids_int =
 // their internal rows (position in band 0's sorted order), which index S and the counts.
-// Counts / offsets are BAND-major, [b][n2]: the rows of a unit are bucket neighbours, hence (for
-// family members) near neighbours in band 0's order too, so the 32 lanes of a warp append to
-// adjacent small groups of the partner scratch and their partial sectors merge in L1/L2.
-// MODE EM_COUNT:  cnt[b*n2 + row] = number of NEW partners of internal row `row` in band b.
-// MODE EM_FILL_J: outJ[off[b*n2 + row] + t] = external id of the t-th new partner.
+// Counts / offsets are indexed by SORTED RECORD g (band-major, bucket order): the 32 rows of a
+// unit are 32 consecutive records, so a warp's counts are one coalesced store and its groups in
+// the partner scratch are adjacent -- the appends of a unit land in one contiguous piece.  The
+// fill pass leaves, for every non-empty group, loc[band][row] = (start, length) for the row kernel.
+// MODE EM_COUNT:  cnt[g] = number of NEW partners of the row at sorted record g.
+// MODE EM_FILL_J: outJ[off[g] + t] = external id of its t-th new partner.
 template <int BW, int MODE>
 __global__ void __launch_bounds__(kEmWarps * 32)
 emit_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint32_t* __restrict__ ids,
             const uint32_t* __restrict__ ids_int, uint32_t n2, int bands,
             const uint32_t* __restrict__ S, uint32_t* __restrict__ cnt_off,
             uint32_t* __restrict__ outJ, const uint32_t* __restrict__ ubase,
-            uint32_t* __restrict__ masks) {
+            uint32_t* __restrict__ masks, uint2* __restrict__ loc) {
   constexpr int SW = 4 * BW;
   constexpr int RS = SW + 4;                 // shared row stride in words (16-byte aligned)
   constexpr int RPR = 32 / BW;               // S rows fetched per load round
@@ -496,7 +500,11 @@ emit_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint32_t* __
       myid = idc_c;
       rowok = lane < min(32u, dc.mrem - 1u);
       acc = 0;
-      if (MODE != EM_COUNT && rowok) acc = cnt_off[(int64_t)b * n2 + myid];
+      if (MODE != EM_COUNT && rowok) {
+        acc = cnt_off[(int64_t)dc.g0 + lane];
+        const uint32_t nxt = cnt_off[(int64_t)dc.g0 + lane + 1];
+        if (nxt > acc) loc[(int64_t)b * n2 + myid] = make_uint2(acc, nxt - acc);
+      }
       if (MODE == EM_COUNT && masks) ub = ubase[dc.u];
 #pragma unroll
       for (int ch = 0; ch < BW; ++ch) {
@@ -527,7 +535,7 @@ emit_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint32_t* __
     if (MODE == EM_COUNT) {
       acc += __popc(tmask);
       if (masks) masks[((size_t)ub + (dc.c0 >> 5)) * 32 + lane] = tmask;   // kept for the fill pass
-      if (rowok && dc.c0 + 32 >= dc.mrem) cnt_off[(int64_t)b * n2 + myid] = acc;
+      if (rowok && dc.c0 + 32 >= dc.mrem) cnt_off[(int64_t)dc.g0 + lane] = acc;
     }
     __syncwarp();
     dc = dn; idc_c = idc_n; idx_c = idx_n; dn = d2; idc_n = id2; idx_n = ix2; ++k;
@@ -546,43 +554,43 @@ emit_fill_masks_kernel(const uint2* __restrict__ units, uint32_t nunits,
                        const uint32_t* __restrict__ ubase, const uint32_t* __restrict__ masks,
                        const uint32_t* __restrict__ ids, const uint32_t* __restrict__ ids_int,
                        uint32_t n2, int bands, const uint32_t* __restrict__ cnt_off,
-                       uint32_t* __restrict__ outJ) {
+                       uint32_t* __restrict__ outJ, uint2* __restrict__ loc) {
   const uint32_t lane = threadIdx.x & 31;
   const uint32_t nw = gridDim.x * kEmWarps;
   uint32_t u = blockIdx.x * kEmWarps + (threadIdx.x >> 5);
   if (u >= nunits) return;
   struct L1 { uint2 un; uint32_t tb; };
-  struct L2 { uint32_t idx, idi, msk; };
+  struct L2 { uint32_t idx, idi, msk, acc, nxt; };
   auto load1 = [&](uint32_t uu) -> L1 {              // needs only the unit index
     L1 r; r.un = make_uint2(0u, 0u); r.tb = 0u;
     if (uu < nunits) { r.un = units[uu]; r.tb = ubase[uu]; }
     return r;
   };
   auto load2 = [&](const L1& a) -> L2 {              // needs the descriptor
-    L2 r; r.idx = 0u; r.idi = 0u; r.msk = 0u;
+    L2 r; r.idx = 0u; r.idi = 0u; r.msk = 0u; r.acc = 0u; r.nxt = 0u;
     if (a.un.y) {
-      if (lane < a.un.y) { r.idx = ids[a.un.x + lane]; r.idi = ids_int[a.un.x + lane]; }
+      if (lane < a.un.y) r.idx = ids[a.un.x + lane];
+      if (lane < min(32u, a.un.y - 1u)) {
+        r.idi = ids_int[a.un.x + lane];
+        r.acc = cnt_off[a.un.x + lane];
+        r.nxt = cnt_off[a.un.x + lane + 1];
+      }
       r.msk = masks[(size_t)a.tb * 32 + lane];
     }
     return r;
   };
-  auto load3 = [&](const L1& a, const L2& b2) -> uint32_t {   // needs the row's internal id
-    if (a.un.y && lane < min(32u, a.un.y - 1u))
-      return cnt_off[(int64_t)(a.un.x / n2) * n2 + b2.idi];
-    return 0u;
-  };
   L1 a0 = load1(u), a1 = load1(u + nw), a2 = load1(u + 2 * nw);
   L2 b0 = load2(a0), b1 = load2(a1);
-  uint32_t acc = load3(a0, b0);
   for (; u < nunits; u += nw) {
-    const uint32_t acc1 = load3(a1, b1);             // chains of the next units advance one level
-    const L2 b2 = load2(a2);
+    const L2 b2 = load2(a2);                         // chains of the next units advance one level
     const L1 a3 = load1(u + 3 * nw);
     // ---- the current unit
     const uint32_t g0 = a0.un.x, mrem = a0.un.y;
     const uint32_t* __restrict__ idp = ids + g0;
     const uint32_t* __restrict__ mp = masks + (size_t)a0.tb * 32 + lane;
-    uint32_t mask = b0.msk, idc = b0.idx;
+    uint32_t mask = b0.msk, idc = b0.idx, acc = b0.acc;
+    if (b0.nxt > acc)                                // where the row kernel finds this group
+      loc[(size_t)(g0 / n2) * n2 + b0.idi] = make_uint2(acc, b0.nxt - acc);
     for (uint32_t c0 = 0; c0 < mrem; c0 += 32) {
       uint32_t mask_n = 0, idc_n = 0;                // next tile, in flight during this one
       if (c0 + 32 < mrem) {
@@ -600,7 +608,7 @@ emit_fill_masks_kernel(const uint2* __restrict__ units, uint32_t nunits,
       }
       mask = mask_n; idc = idc_n;
     }
-    a0 = a1; a1 = a2; a2 = a3; b0 = b1; b1 = b2; acc = acc1;
+    a0 = a1; a1 = a2; a2 = a3; b0 = b1; b1 = b2;
   }
 }
 
@@ -622,15 +630,14 @@ constexpr int kRsWarps = 8;
 constexpr int kRsBins = 1024;
 
 __device__ __forceinline__ void
-sort_one_row(const uint32_t* __restrict__ off, int64_t n2, int bands, const uint32_t* __restrict__ inJ,
+sort_one_row(const uint32_t* __restrict__ off, const uint2* __restrict__ loc, int64_t n2, int bands,
+             const uint32_t* __restrict__ inJ,
              uint2* out, int64_t r, uint32_t row, uint32_t obase, bool do_sort, uint32_t* bins,
              int lane) {
   // lane b holds group b
   uint32_t gs = 0, len = 0;
-  if (lane < bands) {
-    gs = off[(int64_t)lane * n2 + r];
-    len = off[(int64_t)lane * n2 + r + 1] - gs;
-  }
+  if (lane == 0) { gs = off[r]; len = off[r + 1] - gs; }
+  else if (lane < bands) { const uint2 l = loc[(int64_t)lane * n2 + r]; gs = l.x; len = l.y; }
   uint32_t pre = len;                        // inclusive -> exclusive prefix of the group lengths
 #pragma unroll
   for (int d = 1; d < 32; d <<= 1) {
@@ -758,7 +765,7 @@ sort_one_row(const uint32_t* __restrict__ off, int64_t n2, int bands, const uint
 constexpr int kRsChunk = 8;
 
 __global__ void __launch_bounds__(kRsWarps * 32, 6)
-row_sort_kernel(const uint32_t* __restrict__ off, int64_t n2, int bands,
+row_sort_kernel(const uint32_t* __restrict__ off, const uint2* __restrict__ loc, int64_t n2, int bands,
                 const uint32_t* __restrict__ ids0, const uint32_t* __restrict__ ext_off,
                 bool do_sort, const uint32_t* __restrict__ inJ, uint2* out,
                 unsigned long long* __restrict__ next_row) {
@@ -774,7 +781,7 @@ row_sort_kernel(const uint32_t* __restrict__ off, int64_t n2, int bands,
     const int64_t last = min(n2, (int64_t)first + kRsChunk);
     for (int64_t r = (int64_t)first; r < last; ++r) {
       const uint32_t i = ids0[r];            // external id of internal row r
-      sort_one_row(off, n2, bands, inJ, out, r, i, ext_off[i], do_sort, bins_sh[w], lane);
+      sort_one_row(off, loc, n2, bands, inJ, out, r, i, ext_off[i], do_sort, bins_sh[w], lane);
       __syncwarp();
     }
   }
@@ -783,7 +790,7 @@ row_sort_kernel(const uint32_t* __restrict__ off, int64_t n2, int bands,
 template <int BW>
 int launch_emit(sq_ctx* c, int mode, const uint2* units, uint32_t nunits, const uint32_t* ids,
                 const uint32_t* ids_int, uint32_t n2, int bands, const uint32_t* S,
-                uint32_t* cnt_off, uint32_t* outJ, const uint32_t* ubase, uint32_t* masks) {
+                uint32_t* cnt_off, uint32_t* outJ, const uint32_t* ubase, uint32_t* masks, uint2* loc) {
   // persistent warps: exactly the resident blocks of every SM, never more warps than units
   int per_sm = 0;
   cudaError_t e;
@@ -797,10 +804,10 @@ int launch_emit(sq_ctx* c, int mode, const uint2* units, uint32_t nunits, const 
   if (g > need) g = need;
   if (mode == EM_COUNT)
     SQ_TIMED(c, SQ_K_EMIT, emit_kernel<BW, EM_COUNT><<<g, kEmWarps * 32, 0, c->stream>>>(
-        units, nunits, ids, ids_int, n2, bands, S, cnt_off, outJ, ubase, masks));
+        units, nunits, ids, ids_int, n2, bands, S, cnt_off, outJ, ubase, masks, loc));
   else
     SQ_TIMED(c, SQ_K_EMIT, emit_kernel<BW, EM_FILL_J><<<g, kEmWarps * 32, 0, c->stream>>>(
-        units, nunits, ids, ids_int, n2, bands, S, cnt_off, outJ, ubase, masks));
+        units, nunits, ids, ids_int, n2, bands, S, cnt_off, outJ, ubase, masks, loc));
   SQ_LAUNCH_CHECK(c);
   return SQ_OK;
 }
@@ -820,12 +827,12 @@ int launch_emit_band0(sq_ctx* c, int mode, const uint2* units0, uint32_t nunits0
 
 int launch_fill_masks(sq_ctx* c, const uint2* units, uint32_t nunits, const uint32_t* ubase,
                       const uint32_t* masks, const uint32_t* ids, const uint32_t* ids_int,
-                      uint32_t n2, int bands, const uint32_t* cnt_off, uint32_t* outJ) {
+                      uint32_t n2, int bands, const uint32_t* cnt_off, uint32_t* outJ, uint2* loc) {
   unsigned g = (unsigned)c->sm_count * 16u;          // 64 warps per SM, persistent
   const unsigned need = (nunits + kEmWarps - 1) / kEmWarps;
   if (g > need) g = need;
   SQ_TIMED(c, SQ_K_EMIT, emit_fill_masks_kernel<<<g, kEmWarps * 32, 0, c->stream>>>(
-      units, nunits, ubase, masks, ids, ids_int, n2, bands, cnt_off, outJ));
+      units, nunits, ubase, masks, ids, ids_int, n2, bands, cnt_off, outJ, loc));
   SQ_LAUNCH_CHECK(c);
   return SQ_OK;
 }
@@ -835,17 +842,17 @@ int launch_fill_masks(sq_ctx* c, const uint2* units, uint32_t nunits, const uint
 int dispatch_emit(sq_ctx* c, int bw, int mode, const uint2* units, uint32_t nunits,
                   const uint2* units0, uint32_t nunits0, const uint32_t* ids,
                   const uint32_t* ids_int, uint32_t n2, int bands, const uint32_t* S,
-                  uint32_t* cnt_off, uint32_t* outJ, const uint32_t* ubase, uint32_t* masks) {
+                  uint32_t* cnt_off, uint32_t* outJ, const uint32_t* ubase, uint32_t* masks, uint2* loc) {
   int rc = SQ_OK;
   if (nunits0) rc = launch_emit_band0(c, mode, units0, nunits0, ids, bands, cnt_off, outJ);
   if (rc != SQ_OK || nunits == 0) return rc;
   if (mode != EM_COUNT && masks)
-    return launch_fill_masks(c, units, nunits, ubase, masks, ids, ids_int, n2, bands, cnt_off, outJ);
+    return launch_fill_masks(c, units, nunits, ubase, masks, ids, ids_int, n2, bands, cnt_off, outJ, loc);
   switch (bw) {
-    case 1: return launch_emit<1>(c, mode, units, nunits, ids, ids_int, n2, bands, S, cnt_off, outJ, ubase, masks);
-    case 2: return launch_emit<2>(c, mode, units, nunits, ids, ids_int, n2, bands, S, cnt_off, outJ, ubase, masks);
-    case 4: return launch_emit<4>(c, mode, units, nunits, ids, ids_int, n2, bands, S, cnt_off, outJ, ubase, masks);
-    default: return launch_emit<8>(c, mode, units, nunits, ids, ids_int, n2, bands, S, cnt_off, outJ, ubase, masks);
+    case 1: return launch_emit<1>(c, mode, units, nunits, ids, ids_int, n2, bands, S, cnt_off, outJ, ubase, masks, loc);
+    case 2: return launch_emit<2>(c, mode, units, nunits, ids, ids_int, n2, bands, S, cnt_off, outJ, ubase, masks, loc);
+    case 4: return launch_emit<4>(c, mode, units, nunits, ids, ids_int, n2, bands, S, cnt_off, outJ, ubase, masks, loc);
+    default: return launch_emit<8>(c, mode, units, nunits, ids, ids_int, n2, bands, S, cnt_off, outJ, ubase, masks, loc);
   }
 }
 
@@ -861,7 +868,8 @@ size_t sq_lsh_scratch_bytes(int64_t n, int bands, int64_t pair_capacity) {
   s += 2 * sq_align_up(rec * 8 + 16);          // keys ping-pong (the unit lists reuse one)
   s += 2 * sq_align_up(rec * 4 + 16);          // ids ping-pong (the internal rows reuse one)
   s += sq_align_up(nn * sw * 4 + 16);          // bucket-id table S
-  s += sq_align_up((rec + 2) * 4 + 16);        // per (row, band) counts -> offsets
+  s += sq_align_up((rec + 2) * 4 + 16);        // per record counts -> offsets
+  s += sq_align_up((rec + 2) * 8 + 16);        // loc[band][row]: where the row kernel finds a group
   s += sq_align_up((rec / 2 + 2) * 4 + 16);    // first mask tile of every unit
   s += 4 * sq_align_up((nn + 2) * 4 + 16);     // non-empty flags / ranks; rowidx; ext_off; rowstart
   s += sq_sort_scratch_bytes(n, bands);
@@ -898,12 +906,13 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
   uint32_t* S = sq_scratch<uint32_t>(c, (size_t)n * sw);
   uint32_t* cnt = sq_scratch<uint32_t>(c, rec + 2);
   uint32_t* ubase = sq_scratch<uint32_t>(c, rec / 2 + 2);
+  uint2* loc = sq_scratch<uint2>(c, rec + 2);
   uint32_t* nonempty = sq_scratch<uint32_t>(c, (size_t)n + 2);
   uint32_t* rowidx = sq_scratch<uint32_t>(c, (size_t)n + 2);
   uint32_t* ext_off = sq_scratch<uint32_t>(c, (size_t)n + 2);
   uint32_t* rowstart = sq_scratch<uint32_t>(c, (size_t)n + 2);
   uint8_t* tmp = sq_scratch<uint8_t>(c, sq_sort_scratch_bytes(n, bands));
-  if (!k0 || !k1 || !v0 || !v1 || !S || !cnt || !ubase || !nonempty || !rowidx || !ext_off || !rowstart || !tmp)
+  if (!k0 || !k1 || !v0 || !v1 || !S || !cnt || !ubase || !loc || !nonempty || !rowidx || !ext_off || !rowstart || !tmp)
     return SQ_ERR_WORKSPACE;
   cudaStream_t st = c->stream;
   unsigned long long* counters = c->dflags;      // [0] unique, [1] raw, [2] n2, [4] units
@@ -971,7 +980,7 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
   uint32_t* masks = (nunits && ntiles) ? sq_scratch<uint32_t>(c, (size_t)ntiles * 32) : nullptr;
   // a5.2 pass 1: counts per (internal row, band) -> offsets
   rc = dispatch_emit(c, bw, EM_COUNT, units, nunits, units0, nunits0, vin, vint, (uint32_t)n2, bands, S,
-                     cnt, nullptr, ubase, masks);
+                     cnt, nullptr, ubase, masks, loc);
   if (rc != SQ_OK) return rc;
   rc = sq_exclusive_scan_u32(c, cnt, cnt, total + 1, reinterpret_cast<uint32_t*>(tmp), counters);
   if (rc != SQ_OK) return rc;
@@ -982,8 +991,16 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
   if (uniq > capacity) return SQ_ERR_CAPACITY;
   if (uniq >= (1ll << 32) - 1) return SQ_ERR_UNSUPPORTED;   // 32-bit output offsets
   if (uniq == 0) return SQ_OK;
+  // a5.2 pass 2: the new partners of every sorted record into the partner scratch (unit by unit,
+  // contiguous); it also leaves loc[band][row] = (start, length) of every non-empty group
+  uint32_t* tmpJ = sq_scratch<uint32_t>(c, (size_t)uniq);
+  if (!tmpJ) return SQ_ERR_WORKSPACE;
+  SQ_CUDA(c, cudaMemsetAsync(loc, 0, (rec + 2) * 8, st));
+  rc = dispatch_emit(c, bw, EM_FILL_J, units, nunits, units0, nunits0, vin, vint, (uint32_t)n2, bands, S,
+                     cnt, tmpJ, ubase, masks, loc);
+  if (rc != SQ_OK) return rc;
   // where every EXTERNAL row starts in the output
-  SQ_TIMED(c, SQ_K_SEGMENT, row_total_kernel<<<(unsigned)((n2 + 256) / 256), 256, 0, st>>>(cnt, n2, bands, rowstart));
+  SQ_TIMED(c, SQ_K_SEGMENT, row_total_kernel<<<(unsigned)((n2 + 256) / 256), 256, 0, st>>>(cnt, loc, n2, bands, rowstart));
   SQ_LAUNCH_CHECK(c);
   SQ_TIMED(c, SQ_K_SEGMENT, ext_count_kernel<<<gb, 256, 0, st>>>(rowidx, rowstart, n, ext_off));
   SQ_LAUNCH_CHECK(c);
@@ -991,12 +1008,6 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
   if (rc != SQ_OK) return rc;
   rc = sq_exclusive_scan_u32(c, rowstart, rowstart, n2 + 1, reinterpret_cast<uint32_t*>(tmp), nullptr);
   if (rc != SQ_OK) return rc;                     // rowstart[r] = first internal position of row r
-  // a5.2 pass 2: the partners of every internal row, grouped by band, into the partner scratch
-  uint32_t* tmpJ = sq_scratch<uint32_t>(c, (size_t)uniq);
-  if (!tmpJ) return SQ_ERR_WORKSPACE;
-  rc = dispatch_emit(c, bw, EM_FILL_J, units, nunits, units0, nunits0, vin, vint, (uint32_t)n2, bands, S,
-                     cnt, tmpJ, ubase, masks);
-  if (rc != SQ_OK) return rc;
   // a5.3: every row (sorted if asked) into its slice of the output
   {
     int per_sm = 0;
@@ -1008,7 +1019,7 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
     if (g > need) g = need;
     SQ_CUDA(c, cudaMemsetAsync(counters + 6, 0, 8, st));
     SQ_TIMED(c, SQ_K_ROWSORT, row_sort_kernel<<<g, kRsWarps * 32, 0, st>>>(
-        cnt, n2, bands, vin, ext_off, flags == SQ_LSH_SORTED, tmpJ, reinterpret_cast<uint2*>(pairs_out),
+        cnt, loc, n2, bands, vin, ext_off, flags == SQ_LSH_SORTED, tmpJ, reinterpret_cast<uint2*>(pairs_out),
         counters + 6));
     SQ_LAUNCH_CHECK(c);
   }
