@@ -391,3 +391,47 @@ def test_affinity_graph_against_oracle(flags):
         sq.affinity_graph(pairs, dist, cnt, P["max_d"], sig, 0, row_ptr, col[:10], wgt[:10])
     assert ei.value.code == binding.SQ_ERR_CAPACITY and ei.value.required == (hd <= P["max_d"]).sum()
     sq.close()
+
+
+@pytest.mark.parametrize("lo,hi", [(33, 64), (65, 128), (129, 160), (200, 240)])
+def test_multiword_dp_every_word_count(lo, hi):
+    """2, 4, 5 and 8 32-bit words per DP column (up to SQ_MAX_LEN = 240 residues): pair lists,
+    the fused tile kernel (unthresholded) and the filtered thresholded path against the oracle."""
+    binding, sq = _ctx()
+    rng = np.random.default_rng(hi)
+    seeds = [rng.integers(0, 20, rng.integers(lo, hi + 1)).astype(np.uint8) for _ in range(12)]
+    seqs = []
+    for s in seeds:
+        for _ in range(25):
+            t = s.copy()
+            for _e in range(rng.integers(0, 9)):                  # substitutions keep the length in range
+                t[rng.integers(0, t.size)] = rng.integers(0, 20)
+            seqs.append(t)
+    seqs.append(np.zeros(0, np.uint8))                            # an empty sequence among long ones
+    rep = dg.from_list(seqs)
+    n = rep.n
+    npairs = n * (n - 1) // 2
+    ws = sq.workspace_bytes(binding.OP_ALL_PAIRS, n, int(rep.offsets[-1]), hi, 0, 1, 0, npairs)
+    sq.set_workspace(ws)
+    sq.pack(torch.from_numpy(rep.seqs).cuda(), torch.from_numpy(rep.offsets).cuda(), 20, hi)
+    full = torch.empty(npairs, dtype=torch.int16, device="cuda")
+    assert sq.all_pairs(-1, None, full) == npairs
+    want = oracle.all_pairs_full(rep.seqs, rep.offsets)
+    assert np.array_equal(_u16(full), want)
+    ii, jj = np.triu_indices(n, 1)
+    for md in (0, 8, 30):
+        sel = np.nonzero(want <= md)[0]
+        pairs = torch.empty((sel.size + 8, 2), dtype=torch.int32, device="cuda")
+        d2 = torch.empty(sel.size + 8, dtype=torch.int16, device="cuda")
+        cnt = sq.all_pairs(md, pairs, d2)
+        assert cnt == sel.size
+        got = _u32(pairs)[:cnt]
+        assert np.array_equal(got[:, 0], ii[sel]) and np.array_equal(got[:, 1], jj[sel])
+        assert np.array_equal(_u16(d2)[:cnt], want[sel])
+    take = rng.choice(npairs, 20_000, replace=False)
+    pl = np.stack([jj[take], ii[take]], 1).astype(np.uint32)      # (j, i): i > j is allowed in a pair list
+    for md in (-1, 12):
+        d = sq.edit_distance(torch.from_numpy(pl.view(np.int32)).cuda(), pl.shape[0], md)
+        w = want[take] if md < 0 else np.minimum(want[take], md + 1)
+        assert np.array_equal(_u16(d)[:pl.shape[0]], w)
+    sq.close()
