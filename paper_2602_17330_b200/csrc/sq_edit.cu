@@ -39,7 +39,7 @@ constexpr int kEdRuns = 8;      // Peq tables resident per warp
 // on rows of the same family, whose partners are the same few sequences -- the text gathers hit
 // L2.  The schedule only permutes the pair indices; every pair is still read from `pairs`.
 template <int STRIDE, bool SCHED>
-__global__ void __launch_bounds__(kEdWarps * 32, 8)
+__global__ void __launch_bounds__(kEdWarps * 32, 5)
 edit_pairs_w1_kernel(const uint8_t* __restrict__ packed, int64_t n, const uint2* __restrict__ pairs,
                      int64_t n_pairs, int max_d, uint16_t* __restrict__ dist,
                      const uint4* __restrict__ sched, const uint32_t* __restrict__ rowstart,
@@ -112,7 +112,9 @@ edit_pairs_w1_kernel(const uint8_t* __restrict__ packed, int64_t n, const uint2*
     else if (m == 0) d = nlen;
     else if (nlen == 0) d = m;
     else {
-      const uint32_t* pq = peq + (run - rbase) * 33;
+      // byte address of this run's table in shared memory: one multiply-add per column gives the
+      // address of Peq[residue], and (Ph << 1) | 1 is one multiply-add as well (both FMA pipe)
+      const uint32_t pq = (uint32_t)__cvta_generic_to_shared(peq + (run - rbase) * 33);
       uint32_t Pv = 0xFFFFFFFFu, Mv = 0u;
 #pragma unroll
       for (int wi = 0; wi < WORDS; ++wi) {
@@ -121,12 +123,16 @@ edit_pairs_w1_kernel(const uint8_t* __restrict__ packed, int64_t n, const uint2*
 #pragma unroll
           for (int q = 0; q < 4; ++q) {
             if (4 * wi + q < nlen) {
-              const uint32_t Eq = pq[(word >> (8 * q)) & 0xFFu];
+              uint32_t Eq;
+              // (not volatile, so the loads of a word can be issued ahead of the DP chain; the
+              // dummy input m -- read from shared memory after the warp barrier -- keeps them
+              // behind the barrier that publishes the table)
+              asm("ld.shared.u32 %0, [%1];" : "=r"(Eq) : "r"(((word >> (8 * q)) & 0xFFu) * 4u + pq), "r"(m));
               const uint32_t Xv = Eq | Mv;
               const uint32_t Xh = (((Eq & Pv) + Pv) ^ Pv) | Eq;
               uint32_t Ph = Mv | ~(Xh | Pv);
               uint32_t Mh = Pv & Xh;
-              Ph = (Ph << 1) | 1u;
+              asm("mad.lo.u32 %0, %0, 2, 1;" : "+r"(Ph));
               Mh <<= 1;
               Pv = Mh | ~(Xv | Ph);
               Mv = Ph & Xv;
