@@ -691,14 +691,18 @@ sort_one_row(const uint32_t* __restrict__ off, const uint2* __restrict__ loc, in
   }
   lo = __reduce_min_sync(kFull, lo);
   hi = __reduce_max_sync(kFull, hi);
-  const float scale = (float)kRsBins / ((float)(hi - lo) + 1.0f);
-  auto bin_of = [&](uint32_t x) -> uint32_t {     // monotone in x, < kRsBins
-    return min((uint32_t)kRsBins - 1u, (uint32_t)((float)(x - lo) * scale));
+  // 64, 256 or 1,024 bins by row size (zeroing and scanning the bins is the fixed cost of a row)
+  const int psh = T <= 64u ? 1 : T <= 256u ? 3 : 5;          // log2(bins per lane)
+  const uint32_t nbins = 32u << psh;
+  const float scale = (float)nbins / ((float)(hi - lo) + 1.0f);
+  auto bin_of = [&](uint32_t x) -> uint32_t {     // monotone in x, < nbins
+    return min(nbins - 1u, (uint32_t)((float)(x - lo) * scale));
   };
-  auto bin_at = [&](uint32_t x) -> uint32_t { const uint32_t b = bin_of(x); return b + (b >> 5); };
+  // bin b lives at word b + b/per (per = bins per lane): the lane-major walk of the scan below
+  // is then conflict-free
+  auto bin_at = [&](uint32_t x) -> uint32_t { const uint32_t b = bin_of(x); return b + (b >> psh); };
   uint32_t* Y = X + T;
-  // bin b lives at word b + b/32: lane-major walks of the scan below are then conflict-free
-  for (int q = lane; q < kRsBins + kRsBins / 32; q += 32) bins[q] = 0u;
+  for (uint32_t q = lane; q < nbins + 32u; q += 32) bins[q] = 0u;
   __syncwarp();
   // (every pass loads 4 batches of 32 before it uses them: the passes are latency-bound)
   for (uint32_t t0 = lane; t0 < T; t0 += 128) {
@@ -710,10 +714,10 @@ sort_one_row(const uint32_t* __restrict__ off, const uint2* __restrict__ loc, in
   }
   __syncwarp();
   {                                          // exclusive scan of the bin counts
-    constexpr int PER = kRsBins / 32;
-    uint32_t v[PER], s = 0;
-#pragma unroll
-    for (int q = 0; q < PER; ++q) { v[q] = bins[lane * (PER + 1) + q]; s += v[q]; }
+    const int per = 1 << psh;
+    uint32_t* mine = bins + lane * (per + 1);
+    uint32_t s = 0;
+    for (int q = 0; q < per; ++q) s += mine[q];
     uint32_t inc = s;
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) {
@@ -721,8 +725,7 @@ sort_one_row(const uint32_t* __restrict__ off, const uint2* __restrict__ loc, in
       if (lane >= d) inc += o;
     }
     uint32_t run = inc - s;
-#pragma unroll
-    for (int q = 0; q < PER; ++q) { bins[lane * (PER + 1) + q] = run; run += v[q]; }
+    for (int q = 0; q < per; ++q) { const uint32_t v = mine[q]; mine[q] = run; run += v; }
   }
   __syncwarp();
   for (uint32_t t0 = lane; t0 < T; t0 += 128) {   // group by bin (arrival order inside a bin)
@@ -741,7 +744,7 @@ sort_one_row(const uint32_t* __restrict__ off, const uint2* __restrict__ loc, in
     for (int u = 0; u < 4; ++u) {
       if (t0 + 32 * u < T) {
         const uint32_t b = bin_of(x[u]);
-        const uint32_t s = b ? bins[(b - 1) + ((b - 1) >> 5)] : 0u, e = bins[b + (b >> 5)];
+        const uint32_t s = b ? bins[(b - 1) + ((b - 1) >> psh)] : 0u, e = bins[b + (b >> psh)];
         uint32_t rk = s;
         for (uint32_t q = s; q < e; ++q) rk += Y[q] < x[u] ? 1u : 0u;
         X[rk] = x[u];
