@@ -276,3 +276,47 @@ def affinity_graph(pairs, dist, max_d: int, sig, min_matches: int, lengths, n: i
     row_ptr = np.zeros(n + 1, np.int64)
     np.cumsum(np.bincount(kp[:, 0], minlength=n), out=row_ptr[1:])
     return row_ptr, kp[:, 1].copy(), weight
+
+
+# ---- next-3 / next-4: Eq. 12 batch size and the cross-repertoire join (plain definitions) -------
+
+def batch_size(n_seqs: int, avail_bytes: int, c: int, l_max: int) -> int:
+    """PAPER.md L139-143 Eq. (12): B = min(#S, max(32, floor(sqrt(M_avail / (c * l_max))))).
+    Integer arithmetic throughout (math.isqrt of the integer quotient floor(M_avail / (c*l_max));
+    floor(sqrt(x)) == isqrt(floor(x)) for real x >= 0), so no floating-point rounding decides B.
+    c = the per-sequence memory overhead constant (bytes per sequence per unit of length); the
+    paper leaves its value open (reading 23)."""
+    import math
+    if n_seqs < 0 or avail_bytes < 0 or c < 1 or l_max < 1:
+        raise ValueError("batch_size: bad argument")
+    return min(int(n_seqs), max(32, math.isqrt(int(avail_bytes) // (int(c) * int(l_max)))))
+
+
+def join_threshold(seqs_a, offsets_a, seqs_b, offsets_b, max_d: int, upper: bool = False):
+    """Cross-repertoire join (Eq. 45: "N and M represent the sizes of the two
+    sequence batches being compared"): every (i, j), i in A, j in B, with Levenshtein distance
+    d(A_i, B_j) <= max_d, ascending by (i, j), and the distances.  `upper` keeps j > i only (the
+    self-join's upper triangle when B is A).  The definition written out: the full rectangle is
+    enumerated and every distance comes from the plain Wagner-Fischer routine."""
+    seqs_a, offsets_a = _u8(seqs_a), _off(offsets_a)
+    seqs_b, offsets_b = _u8(seqs_b), _off(offsets_b)
+    na, nb = offsets_a.shape[0] - 1, offsets_b.shape[0] - 1
+    both = np.concatenate([seqs_a, seqs_b])
+    off = np.concatenate([offsets_a, offsets_b[1:] + offsets_a[-1]])
+    out_p, out_d = [], []
+    rows_per = max(1, (1 << 22) // max(1, nb))
+    jj = np.arange(nb, dtype=np.uint32)
+    for i0 in range(0, na, rows_per):
+        i1 = min(na, i0 + rows_per)
+        ii = np.repeat(np.arange(i0, i1, dtype=np.uint32), nb)
+        jt = np.tile(jj, i1 - i0)
+        pr = np.stack([ii, jt + np.uint32(na)], axis=1)
+        d = edit_distance_pairs(both, off, pr, -1)
+        keep = d.astype(np.int64) <= max_d
+        if upper:
+            keep &= jt > ii
+        out_p.append(np.stack([ii[keep], jt[keep]], axis=1))
+        out_d.append(d[keep])
+    if not out_p:
+        return np.zeros((0, 2), np.uint32), np.zeros(0, np.uint16)
+    return np.concatenate(out_p).astype(np.uint32), np.concatenate(out_d).astype(np.uint16)

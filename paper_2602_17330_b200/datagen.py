@@ -324,3 +324,17 @@ def random_substitution_costs(sigma: int, lo: int, hi: int, seed: int) -> np.nda
     c = np.triu(c, 1)
     c = c + c.T
     return c.astype(np.uint8)
+
+
+def split(rep: Repertoire, n_a: int):
+    """Two repertoires out of one: the first n_a sequences and the rest.  The generators above end
+    with a random permutation, so every family has members on both sides -- the shape of a
+    cross-repertoire (multi-donor) comparison where clonotype families are shared between donors
+    ("pooled CDR3 sequences from ten unrelated individuals")."""
+    n_a = int(n_a)
+    cut = int(rep.offsets[n_a])
+    a = Repertoire(rep.seqs[:cut].copy(), rep.offsets[:n_a + 1].copy(), rep.family[:n_a].copy(),
+                   rep.n_edits[:n_a].copy(), rep.name + "/A")
+    b = Repertoire(rep.seqs[cut:].copy(), (rep.offsets[n_a:] - cut).copy(), rep.family[n_a:].copy(),
+                   rep.n_edits[n_a:].copy(), rep.name + "/B")
+    return a, b
