@@ -56,6 +56,9 @@ extern "C" {
 #define SQ_OP_ALL_PAIRS       4
 #define SQ_OP_PIPELINE_HOST   5
 #define SQ_OP_GRAPH           6   /* sizes->pair_capacity = number of pairs handed to the graph */
+#define SQ_OP_JOIN            7   /* sizes->n = |A| (this context's set), sizes->n_other = |B|,
+                                     sizes->pair_capacity = capacity (sq_join) or block_capacity
+                                     (sq_join_host) */
 
 /* flags of sq_lsh_candidates */
 #define SQ_LSH_SORTED     0   /* pairs_out ascending by (i, j) (default)                      */
@@ -75,6 +78,7 @@ typedef struct sq_sizes {
   int32_t bands;         /* LSH bands                                                        */
   int32_t bucket_cap;    /* LSH bucket cap                                                   */
   int64_t pair_capacity; /* capacity of the pair output (LSH / all-pairs / pipeline)         */
+  int64_t n_other;       /* SQ_OP_JOIN: number of sequences of the other set                 */
 } sq_sizes;
 
 /* Create / destroy a context bound to `device` and to `cuda_stream` (a cudaStream_t cast to
@@ -165,6 +169,41 @@ int  sq_affinity_graph(sq_ctx* ctx, const uint32_t* pairs, const uint16_t* dist,
  *             dist_out uint16[capacity]; *n_out (host) = number of hits.
  * Synchronises. */
 int  sq_all_pairs(sq_ctx* ctx, int max_d, uint32_t* pairs_out, uint16_t* dist_out,
+                  int64_t capacity, int64_t* n_out);
+
+/* next-4  Cross-repertoire join (Eq. 45: "N and M
+ * represent the sizes of the two sequence batches being compared").  A = the set packed in `a`,
+ * B = the set packed in `b` (same device, and packed with the same alphabet and the same max_len
+ * class so that both have one slot stride; `b` may be `a` itself).  Result: every (i, j) with
+ * a_begin <= i < a_end, 0 <= j < n_b and Levenshtein d(A_i, B_j) <= max_d (max_d >= 0), ascending
+ * by (i, j); with SQ_JOIN_UPPER only j > i (the self-join's upper triangle when b == a).
+ * pairs_out: DEVICE uint32[capacity][2] (i indexes A, j indexes B), dist_out: DEVICE
+ * uint16[capacity]; *n_out (host) = number of hits.  Runs on a's stream and scratch (size it with
+ * SQ_OP_JOIN); b's pack must be complete (sq_pack synchronises).  Synchronises.
+ * SQ_ERR_CAPACITY if *n_out > capacity; SQ_ERR_WORKSPACE if even one row of A against B leaves
+ * more bag-filter survivors than the scratch holds (4 * capacity + 65536). */
+#define SQ_JOIN_UPPER 1
+int  sq_join(sq_ctx* a, const sq_ctx* b, int64_t a_begin, int64_t a_end, int max_d, int flags,
+             uint32_t* pairs_out, uint16_t* dist_out, int64_t capacity, int64_t* n_out);
+
+/* next-3  Batch size of PAPER.md L139-143 Eq. (12):
+ *   B = min(n_seqs, max(32, floor(sqrt(avail_bytes / (c * l_max))))),
+ * c = "per-sequence memory overhead constant" (the paper gives no value).  Integer arithmetic
+ * (floor of the integer quotient, then the integer square root).  Host only; -1 on c == 0,
+ * l_max == 0 or n_seqs < 0. */
+int64_t sq_batch_size(int64_t n_seqs, uint64_t avail_bytes, uint32_t c, uint32_t l_max);
+
+/* next-3  Out-of-core join: sq_join over all of A in blocks of `batch_rows` rows, every block's
+ * hits copied to HOST buffers (pinned for full speed) on a second stream while the next block is
+ * computed -- the device holds one block's hits (block_capacity >= 1) and survivors only, so the
+ * hit list may exceed HBM.  batch_rows <= 0: B from Eq. (12) with c = 1 and avail_bytes = the
+ * free scratch, rows per block = B*B / n_b (a block of rows x n_b holds the cells of Eq. 12's
+ * B x B tile).  A block that overflows block_capacity or the survivor scratch is halved and
+ * redone; SQ_ERR_CAPACITY / SQ_ERR_WORKSPACE only if a single row does not fit.
+ * pairs_host: uint32[capacity][2], dist_host: uint16[capacity], ascending by (i, j) overall.
+ * SQ_ERR_CAPACITY (with the required *n_out) if the total exceeds `capacity`.  Synchronises. */
+int  sq_join_host(sq_ctx* a, const sq_ctx* b, int max_d, int flags, int64_t batch_rows,
+                  int64_t block_capacity, uint32_t* pairs_host, uint16_t* dist_host,
                   int64_t capacity, int64_t* n_out);
 
 /* The whole path from HOST buffers (the end-to-end entry point bench.py times as `e2e`):

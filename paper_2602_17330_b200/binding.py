@@ -19,12 +19,13 @@ SQ_OK = 0
 SQ_ERR_INVALID_ARG, SQ_ERR_BAD_RESIDUE, SQ_ERR_NOT_PACKED, SQ_ERR_CAPACITY = -1, -2, -3, -4
 SQ_ERR_WORKSPACE, SQ_ERR_UNSUPPORTED, SQ_ERR_CUDA = -5, -6, -7
 SQ_MAX_LEN, SQ_MAX_H, SQ_MAX_BANDS = 240, 256, 32
-OP_PACK, OP_MINHASH, OP_LSH, OP_EDIT_DISTANCE, OP_ALL_PAIRS, OP_PIPELINE_HOST, OP_GRAPH = range(7)
+OP_PACK, OP_MINHASH, OP_LSH, OP_EDIT_DISTANCE, OP_ALL_PAIRS, OP_PIPELINE_HOST, OP_GRAPH, OP_JOIN = range(8)
 LSH_SORTED, LSH_UNORDERED = 0, 1
+JOIN_UPPER = 1
 
 EXPORTS = ["sq_create", "sq_destroy", "sq_workspace_bytes", "sq_set_workspace", "sq_pack",
            "sq_minhash", "sq_lsh_candidates", "sq_edit_distance", "sq_edit_distance_weighted", "sq_affinity_graph", "sq_all_pairs",
-           "sq_pipeline_host", "sq_packed_n", "sq_packed_stride", "sq_last_raw_pairs",
+           "sq_join", "sq_join_host", "sq_batch_size", "sq_pipeline_host", "sq_packed_n", "sq_packed_stride", "sq_last_raw_pairs",
            "sq_kernel_launches", "sq_last_cuda_error", "sq_strerror", "sq_int_peak",
            "sq_profile_enable", "sq_profile_reset", "sq_profile_read", "sq_profile_name"]
 
@@ -32,7 +33,7 @@ EXPORTS = ["sq_create", "sq_destroy", "sq_workspace_bytes", "sq_set_workspace", 
 class SqSizes(C.Structure):
     _fields_ = [("n", C.c_int64), ("total_len", C.c_int64), ("max_len", C.c_int32),
                 ("H", C.c_int32), ("bands", C.c_int32), ("bucket_cap", C.c_int32),
-                ("pair_capacity", C.c_int64)]
+                ("pair_capacity", C.c_int64), ("n_other", C.c_int64)]
 
 
 class SubQuadError(RuntimeError):
@@ -78,6 +79,12 @@ def load_library():
     L.sq_affinity_graph.argtypes = [vp, vp, vp, i64, i32, vp, i32, i32, vp, vp, vp, i64, C.POINTER(i64)]
     L.sq_all_pairs.restype = i32
     L.sq_all_pairs.argtypes = [vp, i32, vp, vp, i64, C.POINTER(i64)]
+    L.sq_join.restype = i32
+    L.sq_join.argtypes = [vp, vp, i64, i64, i32, i32, vp, vp, i64, C.POINTER(i64)]
+    L.sq_join_host.restype = i32
+    L.sq_join_host.argtypes = [vp, vp, i32, i32, i64, i64, vp, vp, i64, C.POINTER(i64)]
+    L.sq_batch_size.restype = i64
+    L.sq_batch_size.argtypes = [i64, C.c_uint64, C.c_uint32, C.c_uint32]
     L.sq_pipeline_host.restype = i32
     L.sq_pipeline_host.argtypes = [vp, vp, vp, i64, i32, i32, i32, i32, C.c_uint64, i32, i32, i32,
                                    i32, vp, vp, i64, C.POINTER(i64)]
@@ -105,6 +112,11 @@ def load_library():
     L.sq_profile_name.argtypes = [i32]
     _lib = L
     return L
+
+
+def batch_size(n_seqs: int, avail_bytes: int, c: int, l_max: int) -> int:
+    """PAPER.md Eq. (12) through the library (host arithmetic in C)."""
+    return int(load_library().sq_batch_size(n_seqs, avail_bytes, c, l_max))
 
 
 def strerror(code: int) -> str:
@@ -156,8 +168,8 @@ class SubQuad:
             raise SubQuadError(rc, msg, required)
 
     def workspace_bytes(self, op, n, total_len=0, max_len=0, H=0, bands=0, bucket_cap=0,
-                        pair_capacity=0) -> int:
-        s = SqSizes(n, total_len, max_len, H, bands, bucket_cap, pair_capacity)
+                        pair_capacity=0, n_other=0) -> int:
+        s = SqSizes(n, total_len, max_len, H, bands, bucket_cap, pair_capacity, n_other)
         return int(self.lib.sq_workspace_bytes(self.h, op, C.byref(s)))
 
     def set_workspace(self, nbytes: int):
@@ -238,6 +250,31 @@ class SubQuad:
         rc = self.lib.sq_all_pairs(self.h, max_d, _dev_ptr(pairs_out, torch.int32, "pairs_out"),
                                    _dev_ptr(dist_out, torch.int16, "dist_out"),
                                    dist_out.shape[0], C.byref(cnt))
+        self._check(rc, required=cnt.value)
+        return cnt.value
+
+    def join(self, other, max_d, pairs_out, dist_out, a_begin=0, a_end=None, flags=0):
+        """Hits (i in self, j in other, d <= max_d) of rows [a_begin, a_end) into CUDA tensors."""
+        if a_end is None:
+            a_end = int(self.lib.sq_packed_n(self.h))
+        cnt = C.c_int64(0)
+        rc = self.lib.sq_join(self.h, other.h, a_begin, a_end, max_d, flags,
+                              _dev_ptr(pairs_out, torch.int32, "pairs_out"),
+                              _dev_ptr(dist_out, torch.int16, "dist_out"), dist_out.shape[0], C.byref(cnt))
+        self._check(rc, required=cnt.value)
+        return cnt.value
+
+    def join_host(self, other, max_d, pairs_out_host, dist_out_host, block_capacity, batch_rows=0,
+                  flags=0):
+        """Out-of-core join into (pinned) HOST tensors, block by block; returns the hit count."""
+        for t in (pairs_out_host, dist_out_host):
+            if t.is_cuda or not t.is_contiguous():
+                raise TypeError("join_host takes contiguous host tensors")
+        cnt = C.c_int64(0)
+        rc = self.lib.sq_join_host(self.h, other.h, max_d, flags, batch_rows, block_capacity,
+                                   C.c_void_p(pairs_out_host.data_ptr()),
+                                   C.c_void_p(dist_out_host.data_ptr()), dist_out_host.shape[0],
+                                   C.byref(cnt))
         self._check(rc, required=cnt.value)
         return cnt.value
 

@@ -188,6 +188,31 @@ inline int bits_for(int64_t n) {
 
 }  // namespace
 
+// launchers shared with sq_join.cu
+int sq_residue_hist(sq_ctx* c, const uint8_t* packed, int stride, int64_t n, uint32_t* rh, uint32_t* lens) {
+  if (n <= 0) return SQ_OK;
+  SQ_TIMED(c, SQ_K_ALLPAIRS, residue_hist_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(
+      packed, stride, n, rh, lens));
+  SQ_LAUNCH_CHECK(c);
+  return SQ_OK;
+}
+
+int sq_hit_compact(sq_ctx* c, const uint2* surv, const uint16_t* sdist, int64_t ns, int max_d,
+                   uint64_t* hit_pairs, uint32_t* hit_dist, int64_t capacity, unsigned long long* counter) {
+  if (ns <= 0) return SQ_OK;
+  SQ_TIMED(c, SQ_K_ALLPAIRS, hit_compact_kernel<<<(unsigned)((ns + 255) / 256), 256, 0, c->stream>>>(
+      surv, sdist, ns, max_d, hit_pairs, hit_dist, (unsigned long long)capacity, counter));
+  SQ_LAUNCH_CHECK(c);
+  return SQ_OK;
+}
+
+int sq_narrow_dist(sq_ctx* c, const uint32_t* in, int64_t n, uint16_t* out) {
+  if (n <= 0) return SQ_OK;
+  SQ_TIMED(c, SQ_K_MISC, narrow_dist_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(in, n, out));
+  SQ_LAUNCH_CHECK(c);
+  return SQ_OK;
+}
+
 // survivors of the bag-distance filter the scratch is sized for (more -> the fused kernel runs)
 static inline size_t sq_survivor_cap(int64_t pair_capacity) {
   return 4 * (size_t)(pair_capacity > 0 ? pair_capacity : 1) + 65536;

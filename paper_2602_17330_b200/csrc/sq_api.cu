@@ -122,6 +122,8 @@ size_t sq_workspace_bytes(const sq_ctx*, int op, const sq_sizes* s) {
       return persist + sq_allpairs_scratch_bytes(s->n, s->pair_capacity) + slack;
     case SQ_OP_GRAPH:
       return persist + sq_graph_scratch_bytes(s->n, s->pair_capacity) + slack;
+    case SQ_OP_JOIN:
+      return persist + sq_join_scratch_bytes(s->n, s->n_other, s->pair_capacity) + slack;
     case SQ_OP_PIPELINE_HOST: {
       size_t io = sq_align_up((size_t)s->total_len + 16) + sq_align_up((size_t)(s->n + 1) * 8 + 16) +
                   sq_align_up((size_t)s->n * s->H * 4 + 16) +

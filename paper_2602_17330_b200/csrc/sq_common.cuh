@@ -110,6 +110,7 @@ size_t sq_persist_bytes(int64_t n, int max_len);
 size_t sq_lsh_scratch_bytes(int64_t n, int bands, int64_t pair_capacity);
 size_t sq_allpairs_scratch_bytes(int64_t n, int64_t pair_capacity);
 size_t sq_graph_scratch_bytes(int64_t n, int64_t n_pairs);
+size_t sq_join_scratch_bytes(int64_t rows, int64_t n_b, int64_t pair_capacity);
 size_t sq_sort_scratch_bytes(int64_t n_per_batch, int nbatch);
 
 // ---- radix sort (sq_sort.cu) ----
@@ -138,3 +139,11 @@ int sq_exclusive_scan_u32(sq_ctx* c, const uint32_t* in, uint32_t* out, int64_t 
 int sq_minhash_impl(sq_ctx* c, int k, int H, uint64_t seed, uint32_t* sig_out);
 int sq_edit_distance_impl(sq_ctx* c, const uint32_t* pairs, int64_t n_pairs, int max_d,
                           uint16_t* dist_out);
+// pairs (i, j) with i in the context's own pack and j in `packedB` (same stride and alphabet)
+int sq_edit_distance_ab(sq_ctx* c, const uint8_t* packedB, int64_t nB, int max_len_b,
+                        const uint32_t* pairs, int64_t n_pairs, int max_d, uint16_t* dist_out);
+// pieces of the thresholded all-pairs path (sq_allpairs.cu) shared with the join (sq_join.cu)
+int sq_residue_hist(sq_ctx* c, const uint8_t* packed, int stride, int64_t n, uint32_t* rh, uint32_t* lens);
+int sq_hit_compact(sq_ctx* c, const uint2* surv, const uint16_t* sdist, int64_t ns, int max_d,
+                   uint64_t* hit_pairs, uint32_t* hit_dist, int64_t capacity, unsigned long long* counter);
+int sq_narrow_dist(sq_ctx* c, const uint32_t* in, int64_t n, uint16_t* out);

@@ -9,14 +9,15 @@ namespace {
 
 template <int W>
 __global__ void edit_pairs_kernel(const uint8_t* __restrict__ packed, int stride, int64_t n,
+                                  const uint8_t* __restrict__ packedB, int64_t nB,
                                   const uint2* __restrict__ pairs, int64_t n_pairs, int max_d,
                                   int alphabet, uint16_t* __restrict__ dist) {
   extern __shared__ uint32_t peq_smem[];
   const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= n_pairs) return;
   const uint2 pr = pairs[p];
-  if (pr.x >= (uint64_t)n || pr.y >= (uint64_t)n) { dist[p] = 0xFFFFu; return; }
-  const int d = sq_pair_distance<W>(packed + (int64_t)pr.x * stride, packed + (int64_t)pr.y * stride,
+  if (pr.x >= (uint64_t)n || pr.y >= (uint64_t)nB) { dist[p] = 0xFFFFu; return; }
+  const int d = sq_pair_distance<W>(packed + (int64_t)pr.x * stride, packedB + (int64_t)pr.y * stride,
                                     stride, alphabet, max_d, peq_smem + threadIdx.x, blockDim.x);
   dist[p] = (uint16_t)d;
 }
@@ -40,7 +41,8 @@ constexpr int kEdRuns = 8;      // Peq tables resident per warp
 // L2.  The schedule only permutes the pair indices; every pair is still read from `pairs`.
 template <int STRIDE, bool SCHED>
 __global__ void __launch_bounds__(kEdWarps * 32, 5)
-edit_pairs_w1_kernel(const uint8_t* __restrict__ packed, int64_t n, const uint2* __restrict__ pairs,
+edit_pairs_w1_kernel(const uint8_t* __restrict__ packed, int64_t n,
+                     const uint8_t* __restrict__ packedB, int64_t nB, const uint2* __restrict__ pairs,
                      int64_t n_pairs, int max_d, uint16_t* __restrict__ dist,
                      const uint4* __restrict__ sched, const uint32_t* __restrict__ rowstart,
                      const uint32_t* __restrict__ delta) {
@@ -63,12 +65,12 @@ edit_pairs_w1_kernel(const uint8_t* __restrict__ packed, int64_t n, const uint2*
   }
   uint2 pr = make_uint2(0xFFFFFFFFu, 0xFFFFFFFFu);
   if (valid) pr = pairs[p];
-  const bool inrange = valid && pr.x < (uint64_t)n && pr.y < (uint64_t)n;
+  const bool inrange = valid && pr.x < (uint64_t)n && pr.y < (uint64_t)nB;
   const uint32_t i = inrange ? pr.x : 0xFFFFFFFFu;
   // the text is independent of the runs: issue its load first
   uint32_t tw[WORDS];
   {
-    const uint4* rowB = reinterpret_cast<const uint4*>(packed + (int64_t)(inrange ? pr.y : 0u) * STRIDE);
+    const uint4* rowB = reinterpret_cast<const uint4*>(packedB + (int64_t)(inrange ? pr.y : 0u) * STRIDE);
 #pragma unroll
     for (int q = 0; q < WORDS / 4; ++q) {
       const uint4 v = inrange ? rowB[q] : make_uint4(0, 0, 0, 0);
@@ -151,27 +153,30 @@ edit_pairs_w1_kernel(const uint8_t* __restrict__ packed, int64_t n, const uint2*
 }
 
 template <int STRIDE>
-int launch_edit_w1(sq_ctx* c, const uint32_t* pairs, int64_t n_pairs, int max_d, uint16_t* dist_out) {
+int launch_edit_w1(sq_ctx* c, const uint8_t* packedB, int64_t nB, const uint32_t* pairs, int64_t n_pairs,
+                   int max_d, uint16_t* dist_out) {
   const int64_t per_block = kEdWarps * 32;
   // the schedule pays off only when the packed sequences do not fit the L2 anyway
   const bool big = (size_t)c->n * (size_t)c->stride > ((size_t)96 << 20);
-  if (big && c->sched && c->sched_pairs == pairs && c->sched_npairs == n_pairs && c->sched_chunks > 0) {
+  if (packedB == c->packed && big && c->sched && c->sched_pairs == pairs && c->sched_npairs == n_pairs && c->sched_chunks > 0) {
     const int64_t blocks = (c->sched_chunks + kEdWarps - 1) / kEdWarps;
     SQ_TIMED(c, SQ_K_EDIT, edit_pairs_w1_kernel<STRIDE, true><<<(unsigned)blocks, kEdWarps * 32, 0, c->stream>>>(
-        c->packed, c->n, reinterpret_cast<const uint2*>(pairs), n_pairs, max_d, dist_out, c->sched,
-        c->sched_rowstart, c->sched_delta));
+        c->packed, c->n, c->packed, c->n, reinterpret_cast<const uint2*>(pairs), n_pairs, max_d, dist_out,
+        c->sched, c->sched_rowstart, c->sched_delta));
     SQ_LAUNCH_CHECK(c);
     return SQ_OK;
   }
   const int64_t blocks = (n_pairs + per_block - 1) / per_block;
   SQ_TIMED(c, SQ_K_EDIT, edit_pairs_w1_kernel<STRIDE, false><<<(unsigned)blocks, kEdWarps * 32, 0, c->stream>>>(
-      c->packed, c->n, reinterpret_cast<const uint2*>(pairs), n_pairs, max_d, dist_out, nullptr, nullptr, nullptr));
+      c->packed, c->n, packedB, nB, reinterpret_cast<const uint2*>(pairs), n_pairs, max_d, dist_out, nullptr,
+      nullptr, nullptr));
   SQ_LAUNCH_CHECK(c);
   return SQ_OK;
 }
 
 template <int W>
-int launch_edit(sq_ctx* c, const uint32_t* pairs, int64_t n_pairs, int max_d, uint16_t* dist_out) {
+int launch_edit(sq_ctx* c, const uint8_t* packedB, int64_t nB, const uint32_t* pairs, int64_t n_pairs,
+                int max_d, uint16_t* dist_out) {
   const int threads = W <= 2 ? 256 : 128;
   const size_t smem = (size_t)c->alphabet * W * threads * sizeof(uint32_t);
   if (smem > 48 * 1024)
@@ -179,29 +184,38 @@ int launch_edit(sq_ctx* c, const uint32_t* pairs, int64_t n_pairs, int max_d, ui
                                     (int)smem));
   const int64_t blocks = (n_pairs + threads - 1) / threads;
   SQ_TIMED(c, SQ_K_EDIT, edit_pairs_kernel<W><<<(unsigned)blocks, threads, smem, c->stream>>>(
-      c->packed, c->stride, c->n, reinterpret_cast<const uint2*>(pairs), n_pairs, max_d, c->alphabet,
-      dist_out));
+      c->packed, c->stride, c->n, packedB, nB, reinterpret_cast<const uint2*>(pairs), n_pairs, max_d,
+      c->alphabet, dist_out));
   SQ_LAUNCH_CHECK(c);
   return SQ_OK;
 }
 
 }  // namespace
 
-int sq_edit_distance_impl(sq_ctx* c, const uint32_t* pairs, int64_t n_pairs, int max_d,
-                          uint16_t* dist_out) {
+// pairs (i, j): i indexes the context's own pack, j indexes `packedB` (nB slots of the same stride
+// and alphabet, at most max_len_b residues each); packedB == c->packed is the ordinary self case
+int sq_edit_distance_ab(sq_ctx* c, const uint8_t* packedB, int64_t nB, int max_len_b,
+                        const uint32_t* pairs, int64_t n_pairs, int max_d, uint16_t* dist_out) {
   if (c->n < 0) return SQ_ERR_NOT_PACKED;
   if (n_pairs < 0) return SQ_ERR_INVALID_ARG;
   if (n_pairs == 0) return SQ_OK;
-  if (!pairs || !dist_out) return SQ_ERR_INVALID_ARG;
+  if (!pairs || !dist_out || !packedB) return SQ_ERR_INVALID_ARG;
   if (n_pairs >= (1ll << 31) * 128) return SQ_ERR_UNSUPPORTED;
   if (max_d > 65534) max_d = -1;
-  if (c->stride == 16) return launch_edit_w1<16>(c, pairs, n_pairs, max_d, dist_out);
-  if (c->stride == 32) return launch_edit_w1<32>(c, pairs, n_pairs, max_d, dist_out);
-  const int words = (c->max_len + 31) / 32;
-  if (words <= 1) return launch_edit<1>(c, pairs, n_pairs, max_d, dist_out);
-  if (words <= 2) return launch_edit<2>(c, pairs, n_pairs, max_d, dist_out);
-  if (words <= 4) return launch_edit<4>(c, pairs, n_pairs, max_d, dist_out);
-  if (words <= 5) return launch_edit<5>(c, pairs, n_pairs, max_d, dist_out);
-  if (words <= 8) return launch_edit<8>(c, pairs, n_pairs, max_d, dist_out);
+  if (c->stride == 16) return launch_edit_w1<16>(c, packedB, nB, pairs, n_pairs, max_d, dist_out);
+  if (c->stride == 32) return launch_edit_w1<32>(c, packedB, nB, pairs, n_pairs, max_d, dist_out);
+  const int ml = c->max_len > max_len_b ? c->max_len : max_len_b;
+  const int words = (ml + 31) / 32;
+  if (words <= 1) return launch_edit<1>(c, packedB, nB, pairs, n_pairs, max_d, dist_out);
+  if (words <= 2) return launch_edit<2>(c, packedB, nB, pairs, n_pairs, max_d, dist_out);
+  if (words <= 4) return launch_edit<4>(c, packedB, nB, pairs, n_pairs, max_d, dist_out);
+  if (words <= 5) return launch_edit<5>(c, packedB, nB, pairs, n_pairs, max_d, dist_out);
+  if (words <= 8) return launch_edit<8>(c, packedB, nB, pairs, n_pairs, max_d, dist_out);
   return SQ_ERR_UNSUPPORTED;
+}
+
+int sq_edit_distance_impl(sq_ctx* c, const uint32_t* pairs, int64_t n_pairs, int max_d,
+                          uint16_t* dist_out) {
+  if (c->n < 0) return SQ_ERR_NOT_PACKED;
+  return sq_edit_distance_ab(c, c->packed, c->n, c->max_len, pairs, n_pairs, max_d, dist_out);
 }

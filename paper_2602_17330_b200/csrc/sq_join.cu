@@ -1,0 +1,282 @@
+// sq_join.cu -- SURVEY.md 8(f) ranks 3-4: the cross-repertoire join and its out-of-core driver.
+//
+// PAPER.md App. F.1, Eq. 45: a 2-D grid over "the two sequence batches being compared",
+// N x M.  sq_all_pairs reads it as a self-join; here the two batches are two packed sets A and B
+// (two contexts, same stride and alphabet) and the result is every (i in A, j in B) with
+// d(A_i, B_j) <= max_d.  PAPER.md L139-143, Eq. 12: the batch size that keeps a tile inside the
+// device memory -- sq_batch_size is that formula, and sq_join_host walks A in row blocks of that
+// many cells, streaming each block's hits to the host while the next block is computed, so neither
+// the hit list nor the survivor list of the whole rectangle ever has to fit in HBM.
+//
+//   join_filter_kernel   a block owns 256 columns j and kJoinRows rows i.  Each thread keeps its
+//                        column's residue histogram (32 bytes) in registers; the rows' histograms
+//                        sit in shared memory and are read as broadcasts.  Bag distance
+//                        (L1 of the histograms + |m - n|) / 2 <= d (sq_allpairs.cu) decides
+//                        whether the pair can be a hit; survivors are appended with
+//                        warp-aggregated atomics.
+//   DP                   sq_edit_distance_ab on the survivors (patterns from A, texts from B).
+//   hits                 sq_hit_compact, then one radix sort by (i, j).
+// A row range whose survivors do not fit their scratch is split in two and redone (host work
+// list), so the only hard limit is one row against all of B.
+#include "sq_common.cuh"
+
+namespace {
+
+constexpr int kJoinThreads = 256;
+constexpr int kJoinRows = 16;
+
+__global__ void __launch_bounds__(kJoinThreads)
+join_filter_kernel(const uint32_t* __restrict__ rhA, const uint32_t* __restrict__ lensA, int64_t row0,
+                   int64_t rows, int64_t a_base, const uint32_t* __restrict__ rhB,
+                   const uint32_t* __restrict__ lensB, int64_t nB, int max_d, int upper,
+                   uint2* __restrict__ surv, unsigned long long scap,
+                   unsigned long long* __restrict__ counter) {
+  __shared__ uint4 ha[kJoinRows][2];
+  __shared__ int la[kJoinRows];
+  const int64_t r0 = row0 + (int64_t)blockIdx.x * kJoinRows;          // first row (index into rhA)
+  const int nr = (int)min((int64_t)kJoinRows, row0 + rows - r0);
+  const int64_t jbase = (int64_t)blockIdx.y * kJoinThreads;
+  // `upper`: columns j <= i never count; skip the block when all of its cells are such
+  if (upper && jbase + kJoinThreads <= a_base + r0 + 1) return;
+  if (threadIdx.x < (unsigned)(2 * nr))
+    ha[threadIdx.x >> 1][threadIdx.x & 1] =
+        reinterpret_cast<const uint4*>(rhA)[(r0 + (threadIdx.x >> 1)) * 2 + (threadIdx.x & 1)];
+  if (threadIdx.x >= 64 && threadIdx.x < 64u + (unsigned)nr) la[threadIdx.x - 64] = (int)lensA[r0 + threadIdx.x - 64];
+  __syncthreads();
+  const int64_t j = jbase + threadIdx.x;
+  const bool col = j < nB;
+  uint4 b0 = make_uint4(0, 0, 0, 0), b1 = b0;
+  int nl = 0;
+  if (col) {
+    b0 = reinterpret_cast<const uint4*>(rhB)[j * 2];
+    b1 = reinterpret_cast<const uint4*>(rhB)[j * 2 + 1];
+    nl = (int)lensB[j];
+  }
+  const int lane = threadIdx.x & 31;
+  for (int r = 0; r < nr; ++r) {
+    const uint4 a0 = ha[r][0], a1 = ha[r][1];
+    const int m = la[r];
+    uint32_t l1 = __vsadu4(a0.x, b0.x);
+    l1 += __vsadu4(a0.y, b0.y); l1 += __vsadu4(a0.z, b0.z); l1 += __vsadu4(a0.w, b0.w);
+    l1 += __vsadu4(a1.x, b1.x); l1 += __vsadu4(a1.y, b1.y); l1 += __vsadu4(a1.z, b1.z);
+    l1 += __vsadu4(a1.w, b1.w);
+    const int diff = m > nl ? m - nl : nl - m;
+    const int64_t i = a_base + r0 + r;                                 // row id in A
+    const bool pass = col && (int)((l1 + (uint32_t)diff) >> 1) <= max_d && (!upper || j > i);
+    const uint32_t mask = __ballot_sync(0xFFFFFFFFu, pass);
+    if (mask) {
+      unsigned long long base = 0;
+      if (lane == __ffs(mask) - 1) base = atomicAdd(counter, (unsigned long long)__popc(mask));
+      base = __shfl_sync(0xFFFFFFFFu, base, __ffs(mask) - 1);
+      if (pass) {
+        const unsigned long long slot = base + __popc(mask & ((1u << lane) - 1u));
+        if (slot < scap) surv[slot] = make_uint2((uint32_t)i, (uint32_t)j);
+      }
+    }
+  }
+}
+
+inline int bits_for(int64_t n) {
+  int b = 1;
+  while (b < 32 && (1ll << b) < n) ++b;
+  return b;
+}
+
+inline size_t join_survivor_cap(int64_t cap) { return 4 * (size_t)(cap > 0 ? cap : 1) + 65536; }
+
+// Every hit of rows [a_begin, a_end) of A against all of B, sorted by (i, j), into device buffers.
+// Scratch is taken above the current top and given back.  Synchronises.
+int join_core(sq_ctx* a, const sq_ctx* b, int64_t a_begin, int64_t a_end, int max_d, int flags,
+              uint32_t* pairs_out, uint16_t* dist_out, int64_t capacity, int64_t* n_out) {
+  *n_out = 0;
+  const int64_t rows = a_end - a_begin, nB = b->n;
+  if (rows <= 0 || nB <= 0) return SQ_OK;
+  if ((nB + kJoinThreads - 1) / kJoinThreads > 65535) return SQ_ERR_UNSUPPORTED;
+  if (capacity >= (1ll << 32) - 1) return SQ_ERR_UNSUPPORTED;
+  cudaStream_t st = a->stream;
+  const size_t top = a->scratch_top;
+  struct Restore { sq_ctx* c; size_t t; ~Restore() { c->scratch_top = t; } } restore{a, top};
+  const size_t cap = (size_t)(capacity > 0 ? capacity : 1), scap = join_survivor_cap(capacity);
+  uint64_t* hp = sq_scratch<uint64_t>(a, cap);
+  uint64_t* hp_alt = sq_scratch<uint64_t>(a, cap);
+  uint32_t* hd = sq_scratch<uint32_t>(a, cap);
+  uint32_t* hd_alt = sq_scratch<uint32_t>(a, cap);
+  uint8_t* tmp = sq_scratch<uint8_t>(a, sq_sort_scratch_bytes(capacity, 1));
+  uint32_t* rhA = sq_scratch<uint32_t>(a, (size_t)rows * 8);
+  uint32_t* lensA = sq_scratch<uint32_t>(a, (size_t)rows);
+  uint32_t* rhB = sq_scratch<uint32_t>(a, (size_t)nB * 8);
+  uint32_t* lensB = sq_scratch<uint32_t>(a, (size_t)nB);
+  uint2* surv = sq_scratch<uint2>(a, scap);
+  uint16_t* sdist = sq_scratch<uint16_t>(a, scap);
+  if (!hp || !hp_alt || !hd || !hd_alt || !tmp || !rhA || !lensA || !rhB || !lensB || !surv || !sdist)
+    return SQ_ERR_WORKSPACE;
+  SQ_CUDA(a, cudaMemsetAsync(a->dflags, 0, 64, st));
+  int rc = sq_residue_hist(a, a->packed + a_begin * a->stride, a->stride, rows, rhA, lensA);
+  if (rc != SQ_OK) return rc;
+  rc = sq_residue_hist(a, b->packed, b->stride, nB, rhB, lensB);
+  if (rc != SQ_OK) return rc;
+  // host work list of row ranges (relative to a_begin); a range whose survivors overflow is halved
+  int64_t stack_lo[80], stack_n[80];
+  int sp = 0;
+  stack_lo[0] = 0; stack_n[0] = rows; sp = 1;
+  while (sp > 0) {
+    --sp;
+    const int64_t lo = stack_lo[sp], cnt = stack_n[sp];
+    SQ_CUDA(a, cudaMemsetAsync(a->dflags + 1, 0, 8, st));
+    dim3 grid((unsigned)((cnt + kJoinRows - 1) / kJoinRows), (unsigned)((nB + kJoinThreads - 1) / kJoinThreads));
+    SQ_TIMED(a, SQ_K_ALLPAIRS, join_filter_kernel<<<grid, kJoinThreads, 0, st>>>(
+        rhA, lensA, lo, cnt, a_begin, rhB, lensB, nB, max_d, (flags & SQ_JOIN_UPPER) ? 1 : 0, surv,
+        (unsigned long long)scap, a->dflags + 1));
+    SQ_LAUNCH_CHECK(a);
+    SQ_CUDA(a, cudaMemcpyAsync(a->pinned, a->dflags + 1, 8, cudaMemcpyDeviceToHost, st));
+    SQ_CUDA(a, cudaStreamSynchronize(st));
+    const int64_t ns = (int64_t)a->pinned[0];
+    if ((size_t)ns > scap) {
+      if (cnt == 1 || sp + 2 > 80) return SQ_ERR_WORKSPACE;    // one row against B does not fit
+      const int64_t h = cnt / 2;
+      stack_lo[sp] = lo + h; stack_n[sp] = cnt - h; ++sp;         // second half later,
+      stack_lo[sp] = lo; stack_n[sp] = h; ++sp;                   // first half next
+      continue;
+    }
+    if (ns == 0) continue;
+    rc = sq_edit_distance_ab(a, b->packed, nB, b->max_len, reinterpret_cast<const uint32_t*>(surv), ns,
+                             max_d, sdist);
+    if (rc != SQ_OK) return rc;
+    rc = sq_hit_compact(a, surv, sdist, ns, max_d, hp, hd, capacity, a->dflags);
+    if (rc != SQ_OK) return rc;
+  }
+  SQ_CUDA(a, cudaMemcpyAsync(a->pinned, a->dflags, 8, cudaMemcpyDeviceToHost, st));
+  SQ_CUDA(a, cudaStreamSynchronize(st));
+  const int64_t hits = (int64_t)a->pinned[0];
+  *n_out = hits;
+  if (hits > capacity) return SQ_ERR_CAPACITY;
+  if (hits == 0) return SQ_OK;
+  // order by (i, j): LSD passes over the j field (bits 32..) then the i field (bits 0..)
+  int shifts[8], widths[8], q = 0;
+  const int nbits[2] = {bits_for(nB), bits_for(a->n)};
+  for (int f = 0; f < 2; ++f)
+    for (int p = 0; p < (nbits[f] + 7) / 8; ++p) {
+      shifts[q] = (f == 0 ? 32 : 0) + 8 * p;
+      widths[q] = (nbits[f] - 8 * p) >= 8 ? 8 : (nbits[f] - 8 * p);
+      ++q;
+    }
+  int in_alt = 0;
+  rc = sq_radix_sort(a, hp, hp_alt, hd, hd_alt, hits, 1, shifts, widths, q, tmp, &in_alt);
+  if (rc != SQ_OK) return rc;
+  SQ_CUDA(a, cudaMemcpyAsync(pairs_out, in_alt ? hp_alt : hp, (size_t)hits * 8, cudaMemcpyDeviceToDevice, st));
+  rc = sq_narrow_dist(a, in_alt ? hd_alt : hd, hits, dist_out);
+  if (rc != SQ_OK) return rc;
+  SQ_CUDA(a, cudaStreamSynchronize(st));
+  return SQ_OK;
+}
+
+int join_check(const sq_ctx* a, const sq_ctx* b, int max_d) {
+  if (!a || !b) return SQ_ERR_INVALID_ARG;
+  if (a->n < 0 || b->n < 0) return SQ_ERR_NOT_PACKED;
+  if (a->device != b->device || a->stride != b->stride || a->alphabet != b->alphabet || a->alphabet > 32)
+    return SQ_ERR_INVALID_ARG;
+  if (max_d < 0) return SQ_ERR_INVALID_ARG;
+  return SQ_OK;
+}
+
+}  // namespace
+
+size_t sq_join_scratch_bytes(int64_t rows, int64_t n_b, int64_t pair_capacity) {
+  const size_t cap = (size_t)(pair_capacity > 0 ? pair_capacity : 1), scap = join_survivor_cap(pair_capacity);
+  const size_t r = (size_t)(rows > 0 ? rows : 1), nb = (size_t)(n_b > 0 ? n_b : 1);
+  return 2 * sq_align_up(cap * 8 + 16) + 2 * sq_align_up(cap * 4 + 16) + sq_sort_scratch_bytes(pair_capacity, 1) +
+         sq_align_up(r * 32 + 16) + sq_align_up(r * 4 + 16) + sq_align_up(nb * 32 + 16) + sq_align_up(nb * 4 + 16) +
+         sq_align_up(scap * 8 + 16) + sq_align_up(scap * 2 + 16) +
+         2 * (sq_align_up(cap * 8 + 16) + sq_align_up(cap * 2 + 16)) + 4096;   // sq_join_host staging
+}
+
+extern "C" int64_t sq_batch_size(int64_t n_seqs, uint64_t avail_bytes, uint32_t c, uint32_t l_max) {
+  if (n_seqs < 0 || c == 0 || l_max == 0) return -1;
+  const uint64_t x = avail_bytes / ((uint64_t)c * (uint64_t)l_max);
+  // integer square root: the largest s with s*s <= x
+  // (the floating-point root is only a starting guess; 128-bit products so that s near 2^32 is safe)
+  uint64_t s = (uint64_t)sqrt((double)x);
+  if (s > 0xFFFFFFFFull) s = 0xFFFFFFFFull;
+  while ((unsigned __int128)s * s > x) --s;
+  while ((unsigned __int128)(s + 1) * (s + 1) <= x) ++s;
+  const int64_t bsz = (int64_t)(s > 32 ? s : 32);
+  return n_seqs < bsz ? n_seqs : bsz;
+}
+
+extern "C" int sq_join(sq_ctx* a, const sq_ctx* b, int64_t a_begin, int64_t a_end, int max_d, int flags,
+                       uint32_t* pairs_out, uint16_t* dist_out, int64_t capacity, int64_t* n_out) {
+  if (!n_out) return SQ_ERR_INVALID_ARG;
+  *n_out = 0;
+  int rc = join_check(a, b, max_d);
+  if (rc != SQ_OK) return rc;
+  if (a_begin < 0 || a_end < a_begin || a_end > a->n || capacity < 0) return SQ_ERR_INVALID_ARG;
+  if (capacity > 0 && (!pairs_out || !dist_out)) return SQ_ERR_INVALID_ARG;
+  if (max_d > 65534) max_d = 65534;
+  sq_scratch_reset(a);
+  return join_core(a, b, a_begin, a_end, max_d, flags, pairs_out, dist_out, capacity, n_out);
+}
+
+extern "C" int sq_join_host(sq_ctx* a, const sq_ctx* b, int max_d, int flags, int64_t batch_rows,
+                            int64_t block_capacity, uint32_t* pairs_host, uint16_t* dist_host,
+                            int64_t capacity, int64_t* n_out) {
+  if (!n_out) return SQ_ERR_INVALID_ARG;
+  *n_out = 0;
+  int rc = join_check(a, b, max_d);
+  if (rc != SQ_OK) return rc;
+  if (capacity < 0 || block_capacity < 1) return SQ_ERR_INVALID_ARG;
+  if (capacity > 0 && (!pairs_host || !dist_host)) return SQ_ERR_INVALID_ARG;
+  if (max_d > 65534) max_d = 65534;
+  const int64_t nA = a->n, nB = b->n;
+  if (nA == 0 || nB == 0) return SQ_OK;
+  sq_scratch_reset(a);
+  uint32_t* dp[2]; uint16_t* dd[2];
+  for (int s = 0; s < 2; ++s) {
+    dp[s] = sq_scratch<uint32_t>(a, (size_t)block_capacity * 2);
+    dd[s] = sq_scratch<uint16_t>(a, (size_t)block_capacity);
+    if (!dp[s] || !dd[s]) return SQ_ERR_WORKSPACE;
+  }
+  if (batch_rows <= 0) {
+    // Eq. 12 with c = 1: a tile of B x B cells; a block of rows x n_b holds the same number of cells
+    const int64_t B = sq_batch_size(nA > nB ? nA : nB, (uint64_t)(a->ws_bytes - a->scratch_top), 1,
+                                    (uint32_t)(a->max_len > 0 ? a->max_len : 1));
+    batch_rows = (int64_t)(((__int128)B * B) / nB);
+  }
+  if (batch_rows < 1) batch_rows = 1;
+  if (batch_rows > nA) batch_rows = nA;
+  cudaEvent_t done[2];
+  for (int s = 0; s < 2; ++s) SQ_CUDA(a, cudaEventCreateWithFlags(&done[s], cudaEventDisableTiming));
+  struct Ev { cudaEvent_t* e; ~Ev() { cudaEventDestroy(e[0]); cudaEventDestroy(e[1]); } } ev{done};
+  bool used[2] = {false, false};
+  int64_t total = 0, lo = 0, step = batch_rows;
+  int slot = 0;
+  int result = SQ_OK;
+  while (lo < nA) {
+    const int64_t hi = lo + step < nA ? lo + step : nA;
+    if (used[slot]) SQ_CUDA(a, cudaEventSynchronize(done[slot]));      // its last copy has left
+    int64_t hits = 0;
+    rc = join_core(a, b, lo, hi, max_d, flags, dp[slot], dd[slot], block_capacity, &hits);
+    if (rc == SQ_ERR_CAPACITY || rc == SQ_ERR_WORKSPACE) {
+      if (hi - lo == 1) { result = rc; break; }
+      step = (hi - lo) / 2;                                            // smaller blocks from here on
+      continue;
+    }
+    if (rc != SQ_OK) { result = rc; break; }
+    if (hits > 0 && total + hits <= capacity) {
+      // the block is complete on a->stream (join_core synchronises): ship it beside the next block
+      SQ_CUDA(a, cudaMemcpyAsync(pairs_host + 2 * total, dp[slot], (size_t)hits * 8, cudaMemcpyDeviceToHost,
+                                 a->copy_stream));
+      SQ_CUDA(a, cudaMemcpyAsync(dist_host + total, dd[slot], (size_t)hits * 2, cudaMemcpyDeviceToHost,
+                                 a->copy_stream));
+      SQ_CUDA(a, cudaEventRecord(done[slot], a->copy_stream));
+      used[slot] = true;
+      slot ^= 1;
+    }
+    total += hits;
+    lo = hi;
+  }
+  SQ_CUDA(a, cudaStreamSynchronize(a->copy_stream));
+  sq_scratch_reset(a);
+  if (result != SQ_OK) return result;
+  *n_out = total;
+  return total > capacity ? SQ_ERR_CAPACITY : SQ_OK;
+}

@@ -68,3 +68,26 @@ def test_no_cpu_fallback_in_product_path():
         from paper_2602_17330_b200 import binding
         with pytest.raises(RuntimeError):
             binding.SubQuad(0)
+
+
+def test_batch_size_matches_oracle_eq12():
+    """sq_batch_size is host arithmetic: the library must agree with the oracle's Eq. 12 everywhere,
+    including exact squares and values near 2^64."""
+    import numpy as np
+    import oracle
+    from paper_2602_17330_b200 import binding
+    rng = np.random.default_rng(0)
+    cases = [(10**7, 10**9, 4, 25), (10**7, 10**5, 8, 130), (20, 10**9, 4, 25), (10**6, 640000, 2, 32),
+             (10**6, 639999, 2, 32), (0, 10**9, 1, 1), (10**12, 2**64 - 1, 1, 1), (10**12, (2**32 - 1)**2, 1, 1),
+             (10**12, (2**32 - 1)**2 - 1, 1, 1)]
+    for _ in range(2000):
+        s = int(rng.integers(1, 2**31))
+        cl = int(rng.integers(1, 5000))
+        delta = int(rng.integers(-2, 3))
+        cases.append((int(rng.integers(0, 2**40)), max(0, s * s * cl + delta), cl, 1))
+        cases.append((int(rng.integers(0, 2**40)), int(rng.integers(0, 2**63)), int(rng.integers(1, 2**20)),
+                      int(rng.integers(1, 241))))
+    for n, m, c, l in cases:
+        if m >= 2**64:
+            continue
+        assert binding.batch_size(n, m, c, l) == oracle.batch_size(n, m, c, l), (n, m, c, l)
