@@ -206,6 +206,53 @@ def run_reference(args):
 # ---------------------------------------------------------------------------------------------
 # our arm
 # ---------------------------------------------------------------------------------------------
+def time_cross_join(binding, dev, flush):
+    """sq_join (device output) and sq_join_host (blocks streamed to pinned host memory) on two
+    synthetic repertoires; outside the timed step, reported beside it."""
+    import torch
+    a, b = dg.split(dg.config3(1_000_000, seed=0), 100_000)
+    max_len = int(max(a.lengths.max(), b.lengths.max()))
+    cap, block_cap, max_d = 60_000_000, 8_000_000, 2
+    ctx = []
+    for rep, other in ((a, b), (b, a)):
+        sq = binding.SubQuad(dev.index or 0)
+        sq.set_workspace(sq.workspace_bytes(binding.OP_JOIN, rep.n, int(rep.offsets[-1]), max_len,
+                                            pair_capacity=cap if rep is a else 1, n_other=other.n))
+        sq.pack(torch.from_numpy(rep.seqs).to(dev), torch.from_numpy(rep.offsets).to(dev), alphabet=20,
+                max_len=max_len)
+        ctx.append(sq)
+    sa, sb = ctx
+    pairs = torch.empty((cap, 2), dtype=torch.int32, device=dev)
+    dist = torch.empty(cap, dtype=torch.int16, device=dev)
+    hits = sa.join(sb, max_d, pairs, dist)
+    ph = torch.empty((hits + 16, 2), dtype=torch.int32).pin_memory()
+    dh = torch.empty(hits + 16, dtype=torch.int16).pin_memory()
+    batch_rows = 16384
+    sa.join_host(sb, max_d, ph, dh, block_capacity=block_cap, batch_rows=batch_rows)
+    t_dev, t_host = [], []
+    for _ in range(3):
+        flush.fill_(1); torch.cuda.synchronize()
+        t0 = time.perf_counter(); sa.join(sb, max_d, pairs, dist); t_dev.append(time.perf_counter() - t0)
+        flush.fill_(1); torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        h2 = sa.join_host(sb, max_d, ph, dh, block_capacity=block_cap, batch_rows=batch_rows)
+        t_host.append(time.perf_counter() - t0)
+    assert h2 == hits
+    sa.profile_enable(True); sa.profile_reset()
+    sa.join(sb, max_d, pairs, dist)
+    prof = {k: round(v[0], 3) for k, v in sa.profile_read().items() if v[1]}
+    sa.profile_enable(False)
+    cells = a.n * b.n
+    td, th = sum(t_dev) / 3, sum(t_host) / 3
+    out = {"workload": "config3 recipe split 100,000 x 900,000, max_d=2", "cells": cells, "hits": int(hits),
+           "join_ms": td * 1e3, "cells_per_s": cells / td,
+           "join_host_ms": th * 1e3, "join_host_cells_per_s": cells / th,
+           "block_capacity": block_cap, "batch_rows": batch_rows, "d2h_bytes": int(hits) * 10, "kernel_ms": prof,
+           "timing": "host clock around the synchronising call (sq_join / sq_join_host), 3 runs"}
+    sa.close(); sb.close()
+    return out
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -368,6 +415,15 @@ def run_ours(args):
     except Exception as ex:
         graph = {"error": repr(ex)[:200]}
 
+    # ---- next-3/4: cross-repertoire join, 100,000 x 900,000 CDR3s (config-3 recipe
+    # split in two, the 1 M multi-donor pool shape of PAPER.md L647), max_d = 2
+    join = None
+    if rank == 0 and not args.no_e2e:
+        try:
+            join = time_cross_join(binding, dev, flush)
+        except Exception as ex:
+            join = {"error": repr(ex)[:200]}
+
     # ---- e2e: through the C ABI with HOST buffers -------------------------------------------
     e2e = None
     if not args.no_e2e:
@@ -474,7 +530,7 @@ def run_ours(args):
                    "edit_pairs_per_s": cnt / (st_ms[3] * 1e-3),
                    "edit_gcups": cells / (st_ms[3] * 1e-3) / 1e9,
                    "wall_s_timed_region": wall},
-        "weighted_edit_distance": weighted, "affinity_graph": graph,
+        "weighted_edit_distance": weighted, "affinity_graph": graph, "cross_join": join,
         "roofline": roof, "kernels": kernels, "int_peak_ops_per_s": int_peak,
         "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
     }

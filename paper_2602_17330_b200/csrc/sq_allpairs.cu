@@ -77,7 +77,7 @@ all_pairs_kernel(const uint8_t* __restrict__ packed, int stride, int64_t n, int 
 // with L1 the L1 distance of the residue histograms: an edit changes one count by one (indel) or
 // two counts by one each (substitution).  A pair whose bag distance exceeds max_d cannot be a hit,
 // so it is dropped before any DP.  The histograms (<= 32 residues, one byte each: 8 words) are
-// compared with 8 byte-wise sum-of-absolute-differences instructions.
+// compared with byte-wise sum-of-absolute-differences instructions (sq_join.cu: sq_bag_filter).
 __global__ void __launch_bounds__(256)
 residue_hist_kernel(const uint8_t* __restrict__ packed, int stride, int64_t n,
                     uint32_t* __restrict__ rh, uint32_t* __restrict__ lens) {
@@ -100,41 +100,6 @@ residue_hist_kernel(const uint8_t* __restrict__ packed, int stride, int64_t n,
   }
 #pragma unroll
   for (int q = 0; q < 8; ++q) rh[i * 8 + q] = h[q];
-}
-
-__global__ void __launch_bounds__(kApThreads)
-all_pairs_filter_kernel(const uint32_t* __restrict__ rh, const uint32_t* __restrict__ lens, int64_t n,
-                        int max_d, uint2* __restrict__ surv, unsigned long long scap,
-                        unsigned long long* __restrict__ counter) {
-  const int64_t i = blockIdx.x;
-  const int64_t jbase = (int64_t)blockIdx.y * kApThreads;
-  if (jbase + kApThreads <= i + 1) return;                 // whole block below / on the diagonal
-  const uint4* __restrict__ rh4 = reinterpret_cast<const uint4*>(rh);
-  const uint4 a0 = rh4[i * 2], a1 = rh4[i * 2 + 1];
-  const int m = (int)lens[i];
-  const int64_t j = jbase + threadIdx.x;
-  bool pass = false;
-  if (j > i && j < n) {
-    const uint4 b0 = rh4[j * 2], b1 = rh4[j * 2 + 1];
-    const int nl = (int)lens[j];
-    uint32_t l1 = __vsadu4(a0.x, b0.x);
-    l1 += __vsadu4(a0.y, b0.y); l1 += __vsadu4(a0.z, b0.z); l1 += __vsadu4(a0.w, b0.w);
-    l1 += __vsadu4(a1.x, b1.x); l1 += __vsadu4(a1.y, b1.y); l1 += __vsadu4(a1.z, b1.z);
-    l1 += __vsadu4(a1.w, b1.w);
-    const int diff = m > nl ? m - nl : nl - m;
-    pass = (int)((l1 + (uint32_t)diff) >> 1) <= max_d;
-  }
-  const uint32_t mask = __ballot_sync(0xFFFFFFFFu, pass);
-  if (mask) {
-    const int lane = threadIdx.x & 31;
-    unsigned long long base = 0;
-    if (lane == __ffs(mask) - 1) base = atomicAdd(counter, (unsigned long long)__popc(mask));
-    base = __shfl_sync(0xFFFFFFFFu, base, __ffs(mask) - 1);
-    if (pass) {
-      const unsigned long long slot = base + __popc(mask & ((1u << lane) - 1u));
-      if (slot < scap) surv[slot] = make_uint2((uint32_t)i, (uint32_t)j);
-    }
-  }
 }
 
 // phase 3: the survivors that are hits, as (i | j << 32, d) records for the final ordering
@@ -273,10 +238,10 @@ extern "C" int sq_all_pairs(sq_ctx* c, int max_d, uint32_t* pairs_out, uint16_t*
       SQ_TIMED(c, SQ_K_ALLPAIRS, residue_hist_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(
           c->packed, c->stride, n, rh, lens));
       SQ_LAUNCH_CHECK(c);
-      dim3 grid((unsigned)n, (unsigned)((n + kApThreads - 1) / kApThreads));
-      SQ_TIMED(c, SQ_K_ALLPAIRS, all_pairs_filter_kernel<<<grid, kApThreads, 0, st>>>(
-          rh, lens, n, max_d, surv, (unsigned long long)scap, c->dflags + 1));
-      SQ_LAUNCH_CHECK(c);
+      // (the filter kernel is the join's, sq_join.cu: the column's histogram in registers, 16 rows'
+      // histograms in shared memory; blocks below the diagonal return at once)
+      rc = sq_bag_filter(c, rh, lens, 0, n, 0, rh, lens, n, max_d, 1, surv, scap, c->dflags + 1);
+      if (rc != SQ_OK) return rc;
       SQ_CUDA(c, cudaMemcpyAsync(c->pinned, c->dflags + 1, 8, cudaMemcpyDeviceToHost, st));
       SQ_CUDA(c, cudaStreamSynchronize(st));
       const int64_t ns = (int64_t)c->pinned[0];

@@ -25,44 +25,43 @@ namespace {
 constexpr int kJoinThreads = 256;
 constexpr int kJoinRows = 16;
 
+// NW = histogram words that can be non-zero: ceil(alphabet / 4) (5 for the 20 amino acids)
+template <int NW>
 __global__ void __launch_bounds__(kJoinThreads)
 join_filter_kernel(const uint32_t* __restrict__ rhA, const uint32_t* __restrict__ lensA, int64_t row0,
                    int64_t rows, int64_t a_base, const uint32_t* __restrict__ rhB,
                    const uint32_t* __restrict__ lensB, int64_t nB, int max_d, int upper,
                    uint2* __restrict__ surv, unsigned long long scap,
                    unsigned long long* __restrict__ counter) {
-  __shared__ uint4 ha[kJoinRows][2];
+  __shared__ uint32_t ha[kJoinRows][8];
   __shared__ int la[kJoinRows];
   const int64_t r0 = row0 + (int64_t)blockIdx.x * kJoinRows;          // first row (index into rhA)
   const int nr = (int)min((int64_t)kJoinRows, row0 + rows - r0);
   const int64_t jbase = (int64_t)blockIdx.y * kJoinThreads;
   // `upper`: columns j <= i never count; skip the block when all of its cells are such
   if (upper && jbase + kJoinThreads <= a_base + r0 + 1) return;
-  if (threadIdx.x < (unsigned)(2 * nr))
-    ha[threadIdx.x >> 1][threadIdx.x & 1] =
-        reinterpret_cast<const uint4*>(rhA)[(r0 + (threadIdx.x >> 1)) * 2 + (threadIdx.x & 1)];
-  if (threadIdx.x >= 64 && threadIdx.x < 64u + (unsigned)nr) la[threadIdx.x - 64] = (int)lensA[r0 + threadIdx.x - 64];
+  if (threadIdx.x < (unsigned)(8 * nr)) ha[threadIdx.x >> 3][threadIdx.x & 7] = rhA[r0 * 8 + threadIdx.x];
+  if (threadIdx.x >= 128 && threadIdx.x < 128u + (unsigned)nr) la[threadIdx.x - 128] = (int)lensA[r0 + threadIdx.x - 128];
   __syncthreads();
   const int64_t j = jbase + threadIdx.x;
   const bool col = j < nB;
-  uint4 b0 = make_uint4(0, 0, 0, 0), b1 = b0;
+  uint32_t hb[8] = {0, 0, 0, 0, 0, 0, 0, 0};
   int nl = 0;
   if (col) {
-    b0 = reinterpret_cast<const uint4*>(rhB)[j * 2];
-    b1 = reinterpret_cast<const uint4*>(rhB)[j * 2 + 1];
+    const uint4 b0 = reinterpret_cast<const uint4*>(rhB)[j * 2];
+    const uint4 b1 = reinterpret_cast<const uint4*>(rhB)[j * 2 + 1];
+    hb[0] = b0.x; hb[1] = b0.y; hb[2] = b0.z; hb[3] = b0.w;
+    hb[4] = b1.x; hb[5] = b1.y; hb[6] = b1.z; hb[7] = b1.w;
     nl = (int)lensB[j];
   }
   const int lane = threadIdx.x & 31;
   for (int r = 0; r < nr; ++r) {
-    const uint4 a0 = ha[r][0], a1 = ha[r][1];
     const int m = la[r];
-    uint32_t l1 = __vsadu4(a0.x, b0.x);
-    l1 += __vsadu4(a0.y, b0.y); l1 += __vsadu4(a0.z, b0.z); l1 += __vsadu4(a0.w, b0.w);
-    l1 += __vsadu4(a1.x, b1.x); l1 += __vsadu4(a1.y, b1.y); l1 += __vsadu4(a1.z, b1.z);
-    l1 += __vsadu4(a1.w, b1.w);
-    const int diff = m > nl ? m - nl : nl - m;
+    uint32_t l1 = (uint32_t)(m > nl ? m - nl : nl - m);
+#pragma unroll
+    for (int q = 0; q < NW; ++q) l1 += __vsadu4(ha[r][q], hb[q]);
     const int64_t i = a_base + r0 + r;                                 // row id in A
-    const bool pass = col && (int)((l1 + (uint32_t)diff) >> 1) <= max_d && (!upper || j > i);
+    const bool pass = col && (int)(l1 >> 1) <= max_d && (!upper || j > i);
     const uint32_t mask = __ballot_sync(0xFFFFFFFFu, pass);
     if (mask) {
       unsigned long long base = 0;
@@ -123,11 +122,9 @@ int join_core(sq_ctx* a, const sq_ctx* b, int64_t a_begin, int64_t a_end, int ma
     --sp;
     const int64_t lo = stack_lo[sp], cnt = stack_n[sp];
     SQ_CUDA(a, cudaMemsetAsync(a->dflags + 1, 0, 8, st));
-    dim3 grid((unsigned)((cnt + kJoinRows - 1) / kJoinRows), (unsigned)((nB + kJoinThreads - 1) / kJoinThreads));
-    SQ_TIMED(a, SQ_K_ALLPAIRS, join_filter_kernel<<<grid, kJoinThreads, 0, st>>>(
-        rhA, lensA, lo, cnt, a_begin, rhB, lensB, nB, max_d, (flags & SQ_JOIN_UPPER) ? 1 : 0, surv,
-        (unsigned long long)scap, a->dflags + 1));
-    SQ_LAUNCH_CHECK(a);
+    rc = sq_bag_filter(a, rhA, lensA, lo, cnt, a_begin, rhB, lensB, nB, max_d, (flags & SQ_JOIN_UPPER) ? 1 : 0,
+                       surv, scap, a->dflags + 1);
+    if (rc != SQ_OK) return rc;
     SQ_CUDA(a, cudaMemcpyAsync(a->pinned, a->dflags + 1, 8, cudaMemcpyDeviceToHost, st));
     SQ_CUDA(a, cudaStreamSynchronize(st));
     const int64_t ns = (int64_t)a->pinned[0];
@@ -180,6 +177,24 @@ int join_check(const sq_ctx* a, const sq_ctx* b, int max_d) {
 }
 
 }  // namespace
+
+// rows [row0, row0 + rows) of rhA (row r is sequence a_base + r of A) against all nB columns of rhB:
+// the cells whose bag distance allows d <= max_d are appended to surv (count in *counter)
+int sq_bag_filter(sq_ctx* c, const uint32_t* rhA, const uint32_t* lensA, int64_t row0, int64_t rows,
+                  int64_t a_base, const uint32_t* rhB, const uint32_t* lensB, int64_t nB, int max_d,
+                  int upper, uint2* surv, size_t scap, unsigned long long* counter) {
+  if (rows <= 0 || nB <= 0) return SQ_OK;
+  if ((nB + kJoinThreads - 1) / kJoinThreads > 65535) return SQ_ERR_UNSUPPORTED;
+  dim3 grid((unsigned)((rows + kJoinRows - 1) / kJoinRows), (unsigned)((nB + kJoinThreads - 1) / kJoinThreads));
+  if (c->alphabet <= 20)
+    SQ_TIMED(c, SQ_K_ALLPAIRS, join_filter_kernel<5><<<grid, kJoinThreads, 0, c->stream>>>(
+        rhA, lensA, row0, rows, a_base, rhB, lensB, nB, max_d, upper, surv, (unsigned long long)scap, counter));
+  else
+    SQ_TIMED(c, SQ_K_ALLPAIRS, join_filter_kernel<8><<<grid, kJoinThreads, 0, c->stream>>>(
+        rhA, lensA, row0, rows, a_base, rhB, lensB, nB, max_d, upper, surv, (unsigned long long)scap, counter));
+  SQ_LAUNCH_CHECK(c);
+  return SQ_OK;
+}
 
 size_t sq_join_scratch_bytes(int64_t rows, int64_t n_b, int64_t pair_capacity) {
   const size_t cap = (size_t)(pair_capacity > 0 ? pair_capacity : 1), scap = join_survivor_cap(pair_capacity);
