@@ -467,9 +467,9 @@ def run_ours(args):
         "minhash": n * (stride + 4 + 4 * P["H"]),
         "band_key": n * (4 * P["H"] + 12 * B + 4),
         "sort_hist": 8 * (rec + n),                # keys read once for all digit histograms
-        "sort_scatter": 24 * (8 * rec + n),        # read + write (key 8 B, id 4 B) per pass
+        "sort_scatter": 24 * (4 * rec + n),        # read + write (key 8 B, id 4 B) per pass, 4 passes
         "scan": 12 * (rec + 4 * n),                # counts -> offsets; per-sequence scans
-        "bucket_scan": rec * (8 + 4 + 4) + rec * 12 + 8 * n,   # keys + ids in, S out; id -> internal row
+        "bucket_scan": rec * (8 + 4 + 4) + rec * 12 + 8 * n + 8 * rec,   # keys + ids in, S out; id -> internal row; mixed-run detection
         "emit": rec * (4 + 4 * sw) + 8 * rec + 4 * cnt,        # ids + S rows; counts out, offsets in; partners out
         "row_sort": 4 * cnt + 4 * rec + 8 * cnt,   # partners + offsets in, pairs out
         "misc": 16 * (cnt // 32) + 12 * n,         # chunk schedule of the edit-distance stage

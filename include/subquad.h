@@ -217,6 +217,14 @@ int  sq_pipeline_host(sq_ctx* ctx, const uint8_t* seqs_host, const int64_t* offs
                       uint32_t* pairs_out_host, uint16_t* dist_out_host, int64_t capacity,
                       int64_t* n_pairs);
 
+/* Tuning knobs; none changes any result.
+ * SQ_OPT_SORT_KEY_BYTES (1..8, default 4): the bucket sort of sq_lsh_candidates orders each band by
+ * the top `value` bytes of the 64-bit band key (that many radix passes) and then puts the few
+ * prefix runs that hold several full keys in order, so buckets are always the sets of equal
+ * 64-bit keys the spec defines; 8 = a plain sort on the whole key.  SQ_ERR_INVALID_ARG otherwise. */
+#define SQ_OPT_SORT_KEY_BYTES 1
+int  sq_set_option(sq_ctx* ctx, int option, int64_t value);
+
 /* Introspection (host values, valid after the call they describe). */
 int64_t sq_packed_n(const sq_ctx* ctx);          /* n of the current pack, -1 if none        */
 int     sq_packed_stride(const sq_ctx* ctx);     /* slot stride in bytes                     */

@@ -22,10 +22,11 @@ SQ_MAX_LEN, SQ_MAX_H, SQ_MAX_BANDS = 240, 256, 32
 OP_PACK, OP_MINHASH, OP_LSH, OP_EDIT_DISTANCE, OP_ALL_PAIRS, OP_PIPELINE_HOST, OP_GRAPH, OP_JOIN = range(8)
 LSH_SORTED, LSH_UNORDERED = 0, 1
 JOIN_UPPER = 1
+OPT_SORT_KEY_BYTES = 1
 
 EXPORTS = ["sq_create", "sq_destroy", "sq_workspace_bytes", "sq_set_workspace", "sq_pack",
            "sq_minhash", "sq_lsh_candidates", "sq_edit_distance", "sq_edit_distance_weighted", "sq_affinity_graph", "sq_all_pairs",
-           "sq_join", "sq_join_host", "sq_batch_size", "sq_pipeline_host", "sq_packed_n", "sq_packed_stride", "sq_last_raw_pairs",
+           "sq_join", "sq_join_host", "sq_batch_size", "sq_set_option", "sq_pipeline_host", "sq_packed_n", "sq_packed_stride", "sq_last_raw_pairs",
            "sq_kernel_launches", "sq_last_cuda_error", "sq_strerror", "sq_int_peak",
            "sq_profile_enable", "sq_profile_reset", "sq_profile_read", "sq_profile_name"]
 
@@ -83,6 +84,8 @@ def load_library():
     L.sq_join.argtypes = [vp, vp, i64, i64, i32, i32, vp, vp, i64, C.POINTER(i64)]
     L.sq_join_host.restype = i32
     L.sq_join_host.argtypes = [vp, vp, i32, i32, i64, i64, vp, vp, i64, C.POINTER(i64)]
+    L.sq_set_option.restype = i32
+    L.sq_set_option.argtypes = [vp, i32, i64]
     L.sq_batch_size.restype = i64
     L.sq_batch_size.argtypes = [i64, C.c_uint64, C.c_uint32, C.c_uint32]
     L.sq_pipeline_host.restype = i32
@@ -293,6 +296,9 @@ class SubQuad:
             pairs_out_host.shape[0], C.byref(cnt))
         self._check(rc, required=cnt.value)
         return cnt.value
+
+    def set_option(self, option: int, value: int):
+        self._check(self.lib.sq_set_option(self.h, option, value))
 
     # -- introspection -----------------------------------------------------------------------
     def packed_stride(self) -> int:

@@ -44,6 +44,8 @@ struct sq_ctx {
   int64_t sched_chunks = 0;
   const void* sched_pairs = nullptr;          // the pair buffer it describes
   int64_t sched_npairs = 0;
+  // tuning (sq_set_option)
+  int sort_key_bytes = 4;       // top bytes of the band key the bucket sort orders by (1..8)
   // bookkeeping
   int64_t launches = 0;
   int64_t last_raw_pairs = 0;
@@ -123,10 +125,10 @@ int sq_radix_sort(sq_ctx* c, uint64_t* keys_in, uint64_t* keys_alt, uint32_t* va
                   uint32_t* vals_alt, int64_t n, int nbatch, const int* shifts, const int* widths,
                   int npasses, void* tmp, int* result_in_alt);
 
-// The same sort for byte-wise passes 0..npasses-1 (shift 8p, width 8) in ONE kernel per pass
-// (all histograms up front, decoupled look-back between tiles).  n < 2^30 per batch.
+// The same sort on the key bytes first_pass .. first_pass+npasses-1 (width 8 each) in ONE kernel
+// per pass (all histograms up front, decoupled look-back between tiles).  n < 2^30 per batch.
 int sq_onesweep_sort(sq_ctx* c, uint64_t* keys_in, uint64_t* keys_alt, uint32_t* vals_in,
-                     uint32_t* vals_alt, int64_t n, int nbatch, int npasses, void* tmp,
+                     uint32_t* vals_alt, int64_t n, int nbatch, int first_pass, int npasses, void* tmp,
                      int* result_in_alt);
 
 // exclusive prefix sum of uint32 (offsets wrap mod 2^32; the grand total is returned in 64 bits

@@ -167,6 +167,97 @@ sched_fill_kernel(const uint32_t* __restrict__ rowstart, const uint32_t* __restr
 
 // ---------------------------------------------------------------------------------------------
 // a5.1  bucket scan
+// ---- a4 fix-up: the sort orders every band by only the top `kb` bytes of the 64-bit key --------
+// (half the radix passes for kb = 4).  A bucket is a run of equal FULL keys, so a run of equal
+// prefixes that holds more than one full key ("mixed": ~n^2 / 2^(8 kb + 1) per band) is put in order
+// afterwards: detect_mixed lists the start of every mixed prefix run (the first full-key change
+// inside the run registers it), fix_mixed gives each listed run to a warp, which copies the
+// records key by key -- smallest remaining full key first, records of one key in their current,
+// id-ascending order (ballot compaction) -- into the dead ping-pong buffers and back.  The result
+// is exactly the order of a sort on (prefix, full key), so every bucket is contiguous again.
+__device__ __forceinline__ uint64_t key_prefix(uint64_t k, int pshift) { return k >> pshift; }
+
+__global__ void __launch_bounds__(256)
+detect_mixed_kernel(const uint64_t* __restrict__ keys, int64_t n2, int64_t total, int pshift,
+                    uint32_t* __restrict__ list, unsigned long long* __restrict__ nlist) {
+  const int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= total) return;
+  const int64_t q = g % n2;
+  if (q == 0) return;
+  const uint64_t k = keys[g], kp = keys[g - 1];
+  if (k == kp || key_prefix(k, pshift) != key_prefix(kp, pshift)) return;
+  // a full-key change inside a prefix run: walk back to the run's start; an earlier change in the
+  // same run means this one is not the first
+  int64_t t = g - 1;
+  const int64_t band_lo = g - q;
+  while (t > band_lo) {
+    const uint64_t a = keys[t - 1];
+    if (key_prefix(a, pshift) != key_prefix(kp, pshift)) break;
+    if (a != kp) return;
+    --t;
+  }
+  list[atomicAdd(nlist, 1ull)] = (uint32_t)t;
+}
+
+__global__ void __launch_bounds__(256)
+fix_mixed_kernel(uint64_t* __restrict__ keys, uint32_t* __restrict__ vals, uint64_t* __restrict__ kalt,
+                 uint32_t* __restrict__ valt, int64_t n2, int pshift, const uint32_t* __restrict__ list,
+                 const unsigned long long* __restrict__ nlist) {
+  const int lane = threadIdx.x & 31;
+  const int64_t nw = ((int64_t)gridDim.x * blockDim.x) >> 5;
+  const int64_t nl = (int64_t)*nlist;
+  for (int64_t e = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5; e < nl; e += nw) {
+    const int64_t s = list[e];
+    const int64_t band_hi = (s / n2 + 1) * n2;
+    const uint64_t pre = key_prefix(keys[s], pshift);
+    // end of the prefix run
+    int64_t end = s + 1;
+    for (;;) {
+      const int64_t t = end + lane;
+      const bool same = t < band_hi && key_prefix(keys[t], pshift) == pre;
+      const uint32_t m = __ballot_sync(0xFFFFFFFFu, same);
+      if (m == 0xFFFFFFFFu) { end += 32; continue; }
+      end += __ffs(~m) - 1;
+      break;
+    }
+    // smallest remaining full key first
+    int64_t out = s;
+    bool first = true;
+    uint64_t prev = 0;
+    for (;;) {
+      uint64_t best = ~0ull;
+      bool any = false;
+      for (int64_t t = s + lane; t < end; t += 32) {
+        const uint64_t k = keys[t];
+        if ((first || k > prev) && (!any || k < best)) { best = k; any = true; }
+      }
+#pragma unroll
+      for (int d = 16; d > 0; d >>= 1) {
+        const uint64_t ob = __shfl_xor_sync(0xFFFFFFFFu, best, d);
+        const bool oa = __shfl_xor_sync(0xFFFFFFFFu, (int)any, d) != 0;
+        if (oa && (!any || ob < best)) { best = ob; any = true; }
+      }
+      if (!any) break;
+      for (int64_t t0 = s; t0 < end; t0 += 32) {
+        const int64_t t = t0 + lane;
+        const bool hit = t < end && keys[t] == best;
+        const uint32_t m = __ballot_sync(0xFFFFFFFFu, hit);
+        if (hit) {
+          const int64_t o = out + __popc(m & ((1u << lane) - 1u));
+          kalt[o] = best;
+          valt[o] = vals[t];
+        }
+        out += __popc(m);
+      }
+      prev = best;
+      first = false;
+    }
+    __syncwarp();
+    for (int64_t t = s + lane; t < end; t += 32) { keys[t] = kalt[t]; vals[t] = valt[t]; }
+    __syncwarp();
+  }
+}
+
 // ---------------------------------------------------------------------------------------------
 constexpr int kBsThreads = 256;
 constexpr int kBsItems = 4;
@@ -944,8 +1035,9 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
   // a4: stable radix sort of every band's records by the 64-bit key
   {
     int in_alt = 0;
+    const int kb = c->sort_key_bytes;            // top bytes of the key the sort looks at (1..8)
     if (n2 < (1ll << 30)) {
-      rc = sq_onesweep_sort(c, kin, kalt, vin, valt, n2, bands, 8, tmp, &in_alt);
+      rc = sq_onesweep_sort(c, kin, kalt, vin, valt, n2, bands, 8 - kb, kb, tmp, &in_alt);
     } else {
       int shifts[8], widths[8];
       for (int p = 0; p < 8; ++p) { shifts[p] = 8 * p; widths[p] = 8; }
@@ -953,6 +1045,17 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
     }
     if (rc != SQ_OK) return rc;
     if (in_alt) { uint64_t* t = kin; kin = kalt; kalt = t; uint32_t* tv = vin; vin = valt; valt = tv; }
+    if (n2 < (1ll << 30) && kb < 8) {
+      // prefix runs holding several full keys -> in full-key order (the list lives in `cnt`, which
+      // is cleared afterwards; a mixed run has >= 2 records, so rec / 2 entries always suffice)
+      const int64_t tot = n2 * bands;
+      SQ_TIMED(c, SQ_K_SEGMENT, detect_mixed_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(
+          kin, n2, tot, 64 - 8 * kb, cnt, counters + 3));
+      SQ_LAUNCH_CHECK(c);
+      SQ_TIMED(c, SQ_K_SEGMENT, fix_mixed_kernel<<<(unsigned)(c->sm_count * 4), 256, 0, st>>>(
+          kin, vin, kalt, valt, n2, 64 - 8 * kb, cnt, counters + 3));
+      SQ_LAUNCH_CHECK(c);
+    }
   }
   // internal rows: position in band 0's sorted order (band 0's records are vin[0, n2))
   const int64_t total = n2 * bands;

@@ -265,7 +265,8 @@ constexpr uint32_t kOsAgg = 1u << 30, kOsPrefix = 2u << 30, kOsValue = (1u << 30
 
 // hist[batch][pass][256]: one pass over the keys, all digits at once
 __global__ void __launch_bounds__(256)
-os_hist_kernel(const uint64_t* __restrict__ keys, int64_t n, int npasses, uint32_t* __restrict__ hist) {
+os_hist_kernel(const uint64_t* __restrict__ keys, int64_t n, int first_pass, int npasses,
+               uint32_t* __restrict__ hist) {
   __shared__ uint32_t sh[8 * 256];
   const int batch = blockIdx.y;
   for (int t = threadIdx.x; t < npasses * 256; t += 256) sh[t] = 0u;
@@ -273,7 +274,8 @@ os_hist_kernel(const uint64_t* __restrict__ keys, int64_t n, int npasses, uint32
   const uint64_t* __restrict__ k = keys + (int64_t)batch * n;
   for (int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x; i < n; i += (int64_t)gridDim.x * 256) {
     const uint64_t key = k[i];
-    for (int p = 0; p < npasses; ++p) atomicAdd(&sh[p * 256 + (uint32_t)((key >> (8 * p)) & 255u)], 1u);
+    for (int p = 0; p < npasses; ++p)
+      atomicAdd(&sh[p * 256 + (uint32_t)((key >> (8 * (first_pass + p))) & 255u)], 1u);
   }
   __syncthreads();
   for (int t = threadIdx.x; t < npasses * 256; t += 256)
@@ -303,7 +305,7 @@ template <bool HAS_VALS>
 __global__ void __launch_bounds__(kOsThreads, 2)
 os_pass_kernel(const uint64_t* __restrict__ keys_in, uint64_t* __restrict__ keys_out,
                const uint32_t* __restrict__ vals_in, uint32_t* __restrict__ vals_out, int64_t n,
-               int pass, const uint32_t* __restrict__ hist, uint32_t* desc, uint32_t* tile_ctr,
+               int pass, int shift, const uint32_t* __restrict__ hist, uint32_t* desc, uint32_t* tile_ctr,
                int ntiles) {
   extern __shared__ __align__(16) uint8_t os_smem[];
   uint64_t* skey = reinterpret_cast<uint64_t*>(os_smem);                       // [kOsTile]
@@ -316,7 +318,6 @@ os_pass_kernel(const uint64_t* __restrict__ keys_in, uint64_t* __restrict__ keys
   const int batch = blockIdx.y;
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const uint32_t lt = (1u << lane) - 1u;
-  const int shift = 8 * pass;
   if (threadIdx.x == 0) sh_tile = atomicAdd(&tile_ctr[batch], 1u);
 #pragma unroll
   for (int q = threadIdx.x; q < (kOsThreads / 32) * 256; q += kOsThreads) cnt[q] = 0u;
@@ -431,13 +432,14 @@ size_t sq_onesweep_scratch_bytes(int64_t n, int nbatch) {
          sq_align_up((size_t)nbatch * 8 * 4 + 16);                    // tile counters, per pass
 }
 
-// Byte-wise LSD sort on passes [0, npasses) of 8 bits each; same contract as sq_radix_sort.
+// Byte-wise LSD sort on the key bytes [first_pass, first_pass + npasses); same contract as
+// sq_radix_sort.
 int sq_onesweep_sort(sq_ctx* c, uint64_t* keys_in, uint64_t* keys_alt, uint32_t* vals_in,
-                     uint32_t* vals_alt, int64_t n, int nbatch, int npasses, void* tmp,
+                     uint32_t* vals_alt, int64_t n, int nbatch, int first_pass, int npasses, void* tmp,
                      int* result_in_alt) {
   *result_in_alt = 0;
   if (n <= 0 || nbatch <= 0 || npasses <= 0) return SQ_OK;
-  if (n >= (1ll << 30) || nbatch > 65535 || npasses > 8) return SQ_ERR_UNSUPPORTED;
+  if (n >= (1ll << 30) || nbatch > 65535 || first_pass < 0 || first_pass + npasses > 8) return SQ_ERR_UNSUPPORTED;
   const int64_t ntiles = (n + kOsTile - 1) / kOsTile;
   uint8_t* p = static_cast<uint8_t*>(tmp);
   uint32_t* hist = reinterpret_cast<uint32_t*>(p);      p += sq_align_up((size_t)nbatch * 8 * 256 * 4 + 16);
@@ -451,7 +453,7 @@ int sq_onesweep_sort(sq_ctx* c, uint64_t* keys_in, uint64_t* keys_alt, uint32_t*
     const int64_t cap = (int64_t)c->sm_count * 8 / nbatch + 1;
     if (gx > cap) gx = cap;
     dim3 grid((unsigned)gx, (unsigned)nbatch);
-    SQ_TIMED(c, SQ_K_SORT_HIST, os_hist_kernel<<<grid, 256, 0, st>>>(keys_in, n, npasses, hist));
+    SQ_TIMED(c, SQ_K_SORT_HIST, os_hist_kernel<<<grid, 256, 0, st>>>(keys_in, n, first_pass, npasses, hist));
     SQ_LAUNCH_CHECK(c);
     SQ_TIMED(c, SQ_K_SORT_HIST, os_hist_scan_kernel<<<(unsigned)(nbatch * 8), 32, 0, st>>>(hist));
     SQ_LAUNCH_CHECK(c);
@@ -469,10 +471,12 @@ int sq_onesweep_sort(sq_ctx* c, uint64_t* keys_in, uint64_t* keys_alt, uint32_t*
     SQ_CUDA(c, cudaMemsetAsync(desc, 0, (size_t)nbatch * ntiles * 256 * 4, st));
     if (vals_in)
       SQ_TIMED(c, SQ_K_SORT_SCATTER, os_pass_kernel<true><<<grid, kOsThreads, kOsSmem, st>>>(
-          kin, kout, vin, vout, n, pass, hist, desc, ctr + (size_t)pass * nbatch, (int)ntiles));
+          kin, kout, vin, vout, n, pass, 8 * (first_pass + pass), hist, desc, ctr + (size_t)pass * nbatch,
+          (int)ntiles));
     else
       SQ_TIMED(c, SQ_K_SORT_SCATTER, os_pass_kernel<false><<<grid, kOsThreads, kOsSmem, st>>>(
-          kin, kout, nullptr, nullptr, n, pass, hist, desc, ctr + (size_t)pass * nbatch, (int)ntiles));
+          kin, kout, nullptr, nullptr, n, pass, 8 * (first_pass + pass), hist, desc,
+          ctr + (size_t)pass * nbatch, (int)ntiles));
     SQ_LAUNCH_CHECK(c);
     uint64_t* tk = kin; kin = kout; kout = tk;
     uint32_t* tv = vin; vin = vout; vout = tv;

@@ -90,8 +90,10 @@ def test_minhash_shapes(k, H):
 # ---------------------------------------------------------------------------------------------
 # configs 2-4 shapes: minhash -> lsh -> edit distance
 # ---------------------------------------------------------------------------------------------
-def _run_path(rep, P, capacity, flags=0):
+def _run_path(rep, P, capacity, flags=0, sort_key_bytes=None):
     binding, sq = _ctx()
+    if sort_key_bytes is not None:
+        sq.set_option(binding.OPT_SORT_KEY_BYTES, sort_key_bytes)
     _pack(sq, binding, rep, bands=P["bands"], cap=P["cap"], pair_capacity=capacity, H=P["H"])
     sig = sq.minhash(P["k"], P["H"], SEED)
     pairs = torch.empty((capacity, 2), dtype=torch.int32, device="cuda")
@@ -125,6 +127,24 @@ def test_path_against_oracle(cfg, n, cap_override):
     assert raw == want_raw
     want_d = oracle.edit_distance_pairs(rep.seqs, rep.offsets, want_pairs, P["max_d"])
     assert np.array_equal(dist, want_d)
+
+
+@pytest.mark.parametrize("kb", [1, 2, 3, 8])
+def test_bucket_sort_prefix_bytes_do_not_change_buckets(kb):
+    """The bucket sort orders by the top `kb` key bytes and repairs prefix runs that hold several
+    full keys; with 1-2 bytes nearly every run is mixed, so the repair does the real work."""
+    P = dict(dg.PARAMS["config2"])
+    rep = dg.config2(40_009, seed=8)
+    want_sig = oracle.minhash(rep.seqs, rep.offsets, P["k"], P["H"], SEED)
+    want_pairs, want_raw, _ = oracle.lsh_sorted(want_sig, P["bands"], P["rows"], P["cap"])
+    for flags in (0, 1):
+        _, pairs, dist, raw = _run_path(rep, P, want_pairs.shape[0] + 10, flags=flags, sort_key_bytes=kb)
+        assert raw == want_raw
+        if flags == 0:
+            assert np.array_equal(pairs, want_pairs)
+        else:
+            key = np.sort(pairs[:, 0].astype(np.int64) << 32 | pairs[:, 1])
+            assert np.array_equal(key, want_pairs[:, 0].astype(np.int64) << 32 | want_pairs[:, 1])
 
 
 def test_lsh_unordered_is_the_same_set_and_capacity_protocol():
