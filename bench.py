@@ -425,32 +425,51 @@ def run_ours(args):
             join = {"error": repr(ex)[:200]}
 
     # ---- e2e: through the C ABI with HOST buffers -------------------------------------------
-    e2e = None
+    # headline: sq_pipeline_host_csr (row offsets + partner + byte distance: 5 B per candidate over
+    # PCIe); beside it the pair-list form sq_pipeline_host (10 B per candidate)
+    e2e, e2e_pairs = None, None
     if not args.no_e2e:
-        try:
-            pairs_h = torch.empty((capacity, 2), dtype=torch.int32).pin_memory()
-            dist_h = torch.empty(capacity, dtype=torch.int16).pin_memory()
-            e2e_steps = max(1, min(args.steps, 3))
-            sq.pipeline_host(seqs_h, offs_h, 20, max_len, P["k"], P["H"], dg.DEFAULT_SEED64,
-                             P["bands"], P["rows"], P["cap"], P["max_d"], pairs_h, dist_h)
+        e2e_steps = max(1, min(args.steps, 3))
+
+        def time_host_api(call):
+            call()
             torch.cuda.synchronize()
             t0 = time.perf_counter()
             for _ in range(e2e_steps):
-                c3 = sq.pipeline_host(seqs_h, offs_h, 20, max_len, P["k"], P["H"],
-                                      dg.DEFAULT_SEED64, P["bands"], P["rows"], P["cap"],
-                                      P["max_d"], pairs_h, dist_h)
+                c3 = call()
             torch.cuda.synchronize()
-            t_e2e = (time.perf_counter() - t0) / e2e_steps
+            t = (time.perf_counter() - t0) / e2e_steps
             assert c3 == cnt
-            t_e2e_ms, _ = shard.aggregate(1e3 * t_e2e, {}, dev)
-            te = torch.tensor([t_e2e_ms * 1e-3], dtype=torch.float64)
-            e2e = {"value": cnt_all / te.item(), "unit": UNIT,
+            t_ms, _ = shard.aggregate(1e3 * t, {}, dev)
+            return t_ms * 1e-3
+        try:
+            row_ptr_h = torch.empty(n + 1, dtype=torch.int64).pin_memory()
+            col_h = torch.empty(capacity, dtype=torch.int32).pin_memory()
+            d8_h = torch.empty(capacity, dtype=torch.uint8).pin_memory()
+            te = time_host_api(lambda: sq.pipeline_host_csr(
+                seqs_h, offs_h, 20, max_len, P["k"], P["H"], dg.DEFAULT_SEED64, P["bands"], P["rows"],
+                P["cap"], P["max_d"], row_ptr_h, col_h, d8_h))
+            e2e = {"value": cnt_all / te, "unit": UNIT,
                    "h2d_bytes_per_step": total_len + 8 * (n + 1),
-                   "d2h_bytes_per_step": 10 * cnt, "ms_per_step": 1e3 * te.item(),
-                   "steps": e2e_steps, "api": "sq_pipeline_host (pinned host buffers)"}
-            del pairs_h, dist_h
+                   "d2h_bytes_per_step": 5 * cnt + 8 * (n + 1), "ms_per_step": 1e3 * te,
+                   "steps": e2e_steps,
+                   "api": "sq_pipeline_host_csr (pinned host buffers; row_ptr int64, col uint32, dist uint8)"}
+            del row_ptr_h, col_h, d8_h
         except Exception as ex:               # e.g. not enough pinned host memory
             e2e = {"value": None, "unit": UNIT, "error": repr(ex)[:200]}
+        try:
+            pairs_h = torch.empty((capacity, 2), dtype=torch.int32).pin_memory()
+            dist_h = torch.empty(capacity, dtype=torch.int16).pin_memory()
+            te = time_host_api(lambda: sq.pipeline_host(
+                seqs_h, offs_h, 20, max_len, P["k"], P["H"], dg.DEFAULT_SEED64, P["bands"], P["rows"],
+                P["cap"], P["max_d"], pairs_h, dist_h))
+            e2e_pairs = {"value": cnt_all / te, "unit": UNIT,
+                         "h2d_bytes_per_step": total_len + 8 * (n + 1),
+                         "d2h_bytes_per_step": 10 * cnt, "ms_per_step": 1e3 * te, "steps": e2e_steps,
+                         "api": "sq_pipeline_host (pinned host buffers; pairs uint32[.][2], dist uint16)"}
+            del pairs_h, dist_h
+        except Exception as ex:
+            e2e_pairs = {"value": None, "unit": UNIT, "error": repr(ex)[:200]}
 
     if rank != 0:
         return
@@ -532,7 +551,7 @@ def run_ours(args):
                    "wall_s_timed_region": wall},
         "weighted_edit_distance": weighted, "affinity_graph": graph, "cross_join": join,
         "roofline": roof, "kernels": kernels, "int_peak_ops_per_s": int_peak,
-        "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+        "cpu_baseline": cpu, "e2e": e2e, "e2e_pair_list": e2e_pairs, "gpu_launches": launches, "clocks": clocks,
     }
     print(json.dumps(line))
 

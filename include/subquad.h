@@ -217,6 +217,18 @@ int  sq_pipeline_host(sq_ctx* ctx, const uint8_t* seqs_host, const int64_t* offs
                       uint32_t* pairs_out_host, uint16_t* dist_out_host, int64_t capacity,
                       int64_t* n_pairs);
 
+/* The same path, results as a compressed sparse row structure: the pair list is ascending in
+ * (i, j), so i is carried by row offsets and a thresholded distance fits a byte -- 5 bytes per
+ * candidate cross PCIe instead of 10.  Row i's partners j > i are
+ * col_host[row_ptr_host[i] .. row_ptr_host[i+1]) (ascending), dist_host[...] = min(d, max_d + 1).
+ * row_ptr_host: int64[n+1], col_host: uint32[capacity], dist_host: uint8[capacity].
+ * 0 <= max_d <= 254 (else SQ_ERR_UNSUPPORTED).  Workspace: SQ_OP_PIPELINE_HOST.  Synchronises. */
+int  sq_pipeline_host_csr(sq_ctx* ctx, const uint8_t* seqs_host, const int64_t* offsets_host,
+                          int64_t n, int alphabet, int max_len, int k, int H, uint64_t seed,
+                          int bands, int rows, int bucket_cap, int max_d,
+                          int64_t* row_ptr_host, uint32_t* col_host, uint8_t* dist_host,
+                          int64_t capacity, int64_t* n_pairs);
+
 /* Tuning knobs; none changes any result.
  * SQ_OPT_SORT_KEY_BYTES (1..8, default 4): the bucket sort of sq_lsh_candidates orders each band by
  * the top `value` bytes of the 64-bit band key (that many radix passes) and then puts the few

@@ -26,7 +26,7 @@ OPT_SORT_KEY_BYTES = 1
 
 EXPORTS = ["sq_create", "sq_destroy", "sq_workspace_bytes", "sq_set_workspace", "sq_pack",
            "sq_minhash", "sq_lsh_candidates", "sq_edit_distance", "sq_edit_distance_weighted", "sq_affinity_graph", "sq_all_pairs",
-           "sq_join", "sq_join_host", "sq_batch_size", "sq_set_option", "sq_pipeline_host", "sq_packed_n", "sq_packed_stride", "sq_last_raw_pairs",
+           "sq_join", "sq_join_host", "sq_batch_size", "sq_set_option", "sq_pipeline_host", "sq_pipeline_host_csr", "sq_packed_n", "sq_packed_stride", "sq_last_raw_pairs",
            "sq_kernel_launches", "sq_last_cuda_error", "sq_strerror", "sq_int_peak",
            "sq_profile_enable", "sq_profile_reset", "sq_profile_read", "sq_profile_name"]
 
@@ -91,6 +91,9 @@ def load_library():
     L.sq_pipeline_host.restype = i32
     L.sq_pipeline_host.argtypes = [vp, vp, vp, i64, i32, i32, i32, i32, C.c_uint64, i32, i32, i32,
                                    i32, vp, vp, i64, C.POINTER(i64)]
+    L.sq_pipeline_host_csr.restype = i32
+    L.sq_pipeline_host_csr.argtypes = [vp, vp, vp, i64, i32, i32, i32, i32, C.c_uint64, i32, i32, i32,
+                                       i32, vp, vp, vp, i64, C.POINTER(i64)]
     L.sq_packed_n.restype = i64
     L.sq_packed_n.argtypes = [vp]
     L.sq_packed_stride.restype = i32
@@ -294,6 +297,23 @@ class SubQuad:
             alphabet, max_len, k, H, C.c_uint64(seed), bands, rows, bucket_cap, max_d,
             C.c_void_p(pairs_out_host.data_ptr()), C.c_void_p(dist_out_host.data_ptr()),
             pairs_out_host.shape[0], C.byref(cnt))
+        self._check(rc, required=cnt.value)
+        return cnt.value
+
+    def pipeline_host_csr(self, seqs_host, offsets_host, alphabet, max_len, k, H, seed, bands, rows,
+                          bucket_cap, max_d, row_ptr_host, col_host, dist_host):
+        """Whole path from (pinned) HOST tensors, CSR results (int64 row_ptr[n+1], int32 col,
+        uint8 dist); returns the number of candidate pairs."""
+        for t in (seqs_host, offsets_host, row_ptr_host, col_host, dist_host):
+            if t.is_cuda or not t.is_contiguous():
+                raise TypeError("pipeline_host_csr takes contiguous host tensors")
+        n = offsets_host.numel() - 1
+        cnt = C.c_int64(0)
+        rc = self.lib.sq_pipeline_host_csr(
+            self.h, C.c_void_p(seqs_host.data_ptr()), C.c_void_p(offsets_host.data_ptr()), n,
+            alphabet, max_len, k, H, C.c_uint64(seed), bands, rows, bucket_cap, max_d,
+            C.c_void_p(row_ptr_host.data_ptr()), C.c_void_p(col_host.data_ptr()),
+            C.c_void_p(dist_host.data_ptr()), col_host.shape[0], C.byref(cnt))
         self._check(rc, required=cnt.value)
         return cnt.value
 

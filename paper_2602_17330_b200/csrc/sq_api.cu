@@ -128,7 +128,10 @@ size_t sq_workspace_bytes(const sq_ctx*, int op, const sq_sizes* s) {
       size_t io = sq_align_up((size_t)s->total_len + 16) + sq_align_up((size_t)(s->n + 1) * 8 + 16) +
                   sq_align_up((size_t)s->n * s->H * 4 + 16) +
                   sq_align_up((size_t)s->pair_capacity * 8 + 16) +
-                  sq_align_up((size_t)s->pair_capacity * 2 + 16);
+                  sq_align_up((size_t)s->pair_capacity * 2 + 16) +
+                  sq_align_up((size_t)s->pair_capacity * 4 + 16) +      // sq_pipeline_host_csr: col,
+                  sq_align_up((size_t)s->pair_capacity + 16) +          // byte distances,
+                  sq_align_up((size_t)(s->n + 1) * 8 + 16);             // row offsets
       return persist + io + sq_lsh_scratch_bytes(s->n, s->bands, s->pair_capacity) + slack;
     }
     default: return 0;
@@ -152,13 +155,17 @@ int sq_edit_distance(sq_ctx* c, const uint32_t* pairs, int64_t n_pairs, int max_
   return sq_edit_distance_impl(c, pairs, n_pairs, max_d, dist_out);
 }
 
-int sq_pipeline_host(sq_ctx* c, const uint8_t* seqs_host, const int64_t* offsets_host, int64_t n,
-                     int alphabet, int max_len, int k, int H, uint64_t seed, int bands, int rows,
-                     int bucket_cap, int max_d, uint32_t* pairs_out_host, uint16_t* dist_out_host,
-                     int64_t capacity, int64_t* n_pairs) {
+// shared body of sq_pipeline_host / sq_pipeline_host_csr
+static int pipeline_host_impl(sq_ctx* c, const uint8_t* seqs_host, const int64_t* offsets_host, int64_t n,
+                              int alphabet, int max_len, int k, int H, uint64_t seed, int bands, int rows,
+                              int bucket_cap, int max_d, uint32_t* pairs_out_host, uint16_t* dist_out_host,
+                              int64_t* row_ptr_host, uint32_t* col_host, uint8_t* dist8_host,
+                              int64_t capacity, int64_t* n_pairs) {
+  const bool csr = row_ptr_host != nullptr;
   if (!c || !offsets_host || !n_pairs || n < 0 || capacity < 0) return SQ_ERR_INVALID_ARG;
   if (!c->ws) return SQ_ERR_WORKSPACE;
   if (max_len < 0 || max_len > SQ_MAX_LEN) return SQ_ERR_UNSUPPORTED;
+  if (csr && (max_d < 0 || max_d > 254)) return SQ_ERR_UNSUPPORTED;      // min(d, max_d+1) in a byte
   *n_pairs = 0;
   int64_t total = offsets_host[n];
   // Device I/O buffers sit at the END of the workspace so that sq_pack's persistent region
@@ -166,6 +173,8 @@ int sq_pipeline_host(sq_ctx* c, const uint8_t* seqs_host, const int64_t* offsets
   size_t io = sq_align_up((size_t)total + 16) + sq_align_up((size_t)(n + 1) * 8 + 16) +
               sq_align_up((size_t)n * H * 4 + 16) + sq_align_up((size_t)capacity * 8 + 16) +
               sq_align_up((size_t)capacity * 2 + 16);
+  if (csr) io += sq_align_up((size_t)capacity * 4 + 16) + sq_align_up((size_t)capacity + 16) +
+                 sq_align_up((size_t)(n + 1) * 8 + 16);
   if (io + 4096 > c->ws_bytes) return SQ_ERR_WORKSPACE;
   size_t full = c->ws_bytes;
   uint8_t* p = c->ws + (full - io) / 256 * 256;
@@ -173,7 +182,13 @@ int sq_pipeline_host(sq_ctx* c, const uint8_t* seqs_host, const int64_t* offsets
   int64_t* d_off = (int64_t*)p;   p += sq_align_up((size_t)(n + 1) * 8 + 16);
   uint32_t* d_sig = (uint32_t*)p; p += sq_align_up((size_t)n * H * 4 + 16);
   uint32_t* d_pairs = (uint32_t*)p; p += sq_align_up((size_t)capacity * 8 + 16);
-  uint16_t* d_dist = (uint16_t*)p;
+  uint16_t* d_dist = (uint16_t*)p;  p += sq_align_up((size_t)capacity * 2 + 16);
+  uint32_t* d_col = nullptr; uint8_t* d_dist8 = nullptr; int64_t* d_rowptr = nullptr;
+  if (csr) {
+    d_col = (uint32_t*)p;   p += sq_align_up((size_t)capacity * 4 + 16);
+    d_dist8 = p;            p += sq_align_up((size_t)capacity + 16);
+    d_rowptr = (int64_t*)p;
+  }
   // shrink the arena seen by the ops to the part in front of the I/O buffers
   size_t saved = c->ws_bytes;
   c->ws_bytes = (size_t)((c->ws + (full - io) / 256 * 256) - c->ws);
@@ -193,19 +208,73 @@ int sq_pipeline_host(sq_ctx* c, const uint8_t* seqs_host, const int64_t* offsets
         cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) != cudaSuccess) {
       rc = SQ_ERR_CUDA; break;
     }
-    if (*n_pairs > 0 &&
-        cudaMemcpyAsync(pairs_out_host, d_pairs, (size_t)*n_pairs * 8, cudaMemcpyDeviceToHost,
-                        c->copy_stream) != cudaSuccess) { rc = SQ_ERR_CUDA; break; }
-    if ((rc = sq_edit_distance(c, d_pairs, *n_pairs, max_d, d_dist)) != SQ_OK) break;
-    if (*n_pairs > 0 &&
-        cudaMemcpyAsync(dist_out_host, d_dist, (size_t)*n_pairs * 2, cudaMemcpyDeviceToHost,
-                        c->stream) != cudaSuccess) { rc = SQ_ERR_CUDA; break; }
+    const int64_t np = *n_pairs;
+    if (!csr) {
+      if (np > 0 &&
+          cudaMemcpyAsync(pairs_out_host, d_pairs, (size_t)np * 8, cudaMemcpyDeviceToHost,
+                          c->copy_stream) != cudaSuccess) { rc = SQ_ERR_CUDA; break; }
+    } else if (np == 0) {
+      if ((rc = sq_csr_fill(c, c->copy_stream, d_rowptr, 0)) != SQ_OK) break;
+    } else {
+      // col + row offsets: the first chunk is split and sent at once on the copy stream; the rest
+      // is split on the main stream AHEAD of the DP kernel (behind it the split would wait for
+      // SMs and starve the copy engine -- PCIe is the critical path, the DP has slack)
+      const int64_t first = np < (1ll << 24) ? np : (1ll << 24);
+      rc = sq_csr_split(c, c->copy_stream, d_pairs, 0, first, np, d_col, d_rowptr);
+      if (rc == SQ_OK && cudaMemcpyAsync(col_host, d_col, (size_t)first * 4, cudaMemcpyDeviceToHost,
+                                         c->copy_stream) != cudaSuccess) rc = SQ_ERR_CUDA;
+      if (rc == SQ_OK && first < np) {
+        rc = sq_csr_split(c, c->stream, d_pairs, first, np, np, d_col, d_rowptr);
+        cudaEvent_t ev;
+        if (rc == SQ_OK && cudaEventCreateWithFlags(&ev, cudaEventDisableTiming) != cudaSuccess) rc = SQ_ERR_CUDA;
+        if (rc == SQ_OK) {
+          if (cudaEventRecord(ev, c->stream) != cudaSuccess ||
+              cudaStreamWaitEvent(c->copy_stream, ev, 0) != cudaSuccess ||
+              cudaMemcpyAsync(col_host + first, d_col + first, (size_t)(np - first) * 4,
+                              cudaMemcpyDeviceToHost, c->copy_stream) != cudaSuccess) rc = SQ_ERR_CUDA;
+          cudaEventDestroy(ev);
+        }
+      }
+      if (rc != SQ_OK) break;
+    }
+    if (csr && cudaMemcpyAsync(row_ptr_host, d_rowptr, (size_t)(n + 1) * 8, cudaMemcpyDeviceToHost,
+                               c->copy_stream) != cudaSuccess) { rc = SQ_ERR_CUDA; break; }
+    if ((rc = sq_edit_distance(c, d_pairs, np, max_d, d_dist)) != SQ_OK) break;
+    if (!csr) {
+      if (np > 0 &&
+          cudaMemcpyAsync(dist_out_host, d_dist, (size_t)np * 2, cudaMemcpyDeviceToHost,
+                          c->stream) != cudaSuccess) { rc = SQ_ERR_CUDA; break; }
+    } else if (np > 0) {
+      if ((rc = sq_csr_narrow(c, d_dist, np, d_dist8)) != SQ_OK) break;
+      if (cudaMemcpyAsync(dist8_host, d_dist8, (size_t)np, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess) {
+        rc = SQ_ERR_CUDA; break;
+      }
+    }
     if (cudaStreamSynchronize(c->copy_stream) != cudaSuccess) { rc = SQ_ERR_CUDA; break; }
     if (cudaStreamSynchronize(c->stream) != cudaSuccess) { rc = SQ_ERR_CUDA; break; }
   } while (0);
   if (rc == SQ_ERR_CUDA) c->last_err = cudaGetLastError();
   c->ws_bytes = saved;
   return rc;
+}
+
+int sq_pipeline_host(sq_ctx* c, const uint8_t* seqs_host, const int64_t* offsets_host, int64_t n,
+                     int alphabet, int max_len, int k, int H, uint64_t seed, int bands, int rows,
+                     int bucket_cap, int max_d, uint32_t* pairs_out_host, uint16_t* dist_out_host,
+                     int64_t capacity, int64_t* n_pairs) {
+  return pipeline_host_impl(c, seqs_host, offsets_host, n, alphabet, max_len, k, H, seed, bands, rows,
+                            bucket_cap, max_d, pairs_out_host, dist_out_host, nullptr, nullptr, nullptr,
+                            capacity, n_pairs);
+}
+
+int sq_pipeline_host_csr(sq_ctx* c, const uint8_t* seqs_host, const int64_t* offsets_host, int64_t n,
+                         int alphabet, int max_len, int k, int H, uint64_t seed, int bands, int rows,
+                         int bucket_cap, int max_d, int64_t* row_ptr_host, uint32_t* col_host,
+                         uint8_t* dist_host, int64_t capacity, int64_t* n_pairs) {
+  if (!row_ptr_host || (capacity > 0 && (!col_host || !dist_host))) return SQ_ERR_INVALID_ARG;
+  return pipeline_host_impl(c, seqs_host, offsets_host, n, alphabet, max_len, k, H, seed, bands, rows,
+                            bucket_cap, max_d, nullptr, nullptr, row_ptr_host, col_host, dist_host,
+                            capacity, n_pairs);
 }
 
 }  // extern "C"

@@ -149,6 +149,11 @@ int sq_residue_hist(sq_ctx* c, const uint8_t* packed, int stride, int64_t n, uin
 int sq_hit_compact(sq_ctx* c, const uint2* surv, const uint16_t* sdist, int64_t ns, int max_d,
                    uint64_t* hit_pairs, uint32_t* hit_dist, int64_t capacity, unsigned long long* counter);
 int sq_narrow_dist(sq_ctx* c, const uint32_t* in, int64_t n, uint16_t* out);
+// CSR form of an (i, j)-ascending pair list (sq_csr.cu)
+int sq_csr_split(sq_ctx* c, cudaStream_t st, const uint32_t* pairs, int64_t p0, int64_t p1,
+                 int64_t n_pairs, uint32_t* col, int64_t* row_ptr);
+int sq_csr_fill(sq_ctx* c, cudaStream_t st, int64_t* row_ptr, int64_t v);
+int sq_csr_narrow(sq_ctx* c, const uint16_t* dist, int64_t n_pairs, uint8_t* out);
 // the bag-distance filter over a block of rows x all columns (sq_join.cu)
 int sq_bag_filter(sq_ctx* c, const uint32_t* rhA, const uint32_t* lensA, int64_t row0, int64_t rows,
                   int64_t a_base, const uint32_t* rhB, const uint32_t* lensB, int64_t nB, int max_d,

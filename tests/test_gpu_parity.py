@@ -455,3 +455,65 @@ def test_multiword_dp_every_word_count(lo, hi):
         w = want[take] if md < 0 else np.minimum(want[take], md + 1)
         assert np.array_equal(_u16(d)[:pl.shape[0]], w)
     sq.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# the whole path from host buffers (the e2e entry points)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cfg,n", [("config2", 30_011), ("config4", 50_003)])
+def test_pipeline_host_pairs_and_csr(cfg, n):
+    binding, sq = _ctx()
+    P = dict(dg.PARAMS[cfg])
+    rep = dg.GENERATORS[cfg](n, seed=6)
+    want_sig = oracle.minhash(rep.seqs, rep.offsets, P["k"], P["H"], SEED)
+    want_pairs, _, _ = oracle.lsh_sorted(want_sig, P["bands"], P["rows"], P["cap"])
+    want_d = oracle.edit_distance_pairs(rep.seqs, rep.offsets, want_pairs, P["max_d"])
+    cap = want_pairs.shape[0] + 100
+    max_len = int(rep.lengths.max())
+    sq.set_workspace(sq.workspace_bytes(binding.OP_PIPELINE_HOST, rep.n, int(rep.offsets[-1]), max_len,
+                                        P["H"], P["bands"], P["cap"], cap))
+    seqs_h = torch.from_numpy(rep.seqs).pin_memory()
+    offs_h = torch.from_numpy(rep.offsets).pin_memory()
+    pairs_h = torch.empty((cap, 2), dtype=torch.int32).pin_memory()
+    dist_h = torch.empty(cap, dtype=torch.int16).pin_memory()
+    cnt = sq.pipeline_host(seqs_h, offs_h, 20, max_len, P["k"], P["H"], SEED, P["bands"], P["rows"],
+                           P["cap"], P["max_d"], pairs_h, dist_h)
+    assert cnt == want_pairs.shape[0]
+    assert np.array_equal(pairs_h.numpy().view(np.uint32)[:cnt], want_pairs)
+    assert np.array_equal(dist_h.numpy().view(np.uint16)[:cnt], want_d)
+    # CSR form: same content, 5 bytes per candidate
+    row_ptr = torch.full((rep.n + 1,), -1, dtype=torch.int64).pin_memory()
+    col = torch.empty(cap, dtype=torch.int32).pin_memory()
+    d8 = torch.empty(cap, dtype=torch.uint8).pin_memory()
+    cnt2 = sq.pipeline_host_csr(seqs_h, offs_h, 20, max_len, P["k"], P["H"], SEED, P["bands"], P["rows"],
+                                P["cap"], P["max_d"], row_ptr, col, d8)
+    assert cnt2 == cnt
+    want_rp = np.searchsorted(want_pairs[:, 0], np.arange(rep.n + 1), side="left")
+    assert np.array_equal(row_ptr.numpy(), want_rp)
+    assert np.array_equal(col.numpy().view(np.uint32)[:cnt], want_pairs[:, 1])
+    assert np.array_equal(d8.numpy()[:cnt], want_d.astype(np.uint8))
+    sq.close()
+
+
+def test_pipeline_host_csr_no_candidates_and_limits():
+    from paper_2602_17330_b200.binding import SubQuadError, SQ_ERR_UNSUPPORTED
+    binding, sq = _ctx()
+    rep = dg.config1(300, seed=2)                  # iid random sequences: k=5 sketches share no band
+    max_len = int(rep.lengths.max())
+    sq.set_workspace(sq.workspace_bytes(binding.OP_PIPELINE_HOST, rep.n, int(rep.offsets[-1]), max_len,
+                                        64, 16, 8, 1000))
+    seqs_h = torch.from_numpy(rep.seqs).pin_memory()
+    offs_h = torch.from_numpy(rep.offsets).pin_memory()
+    row_ptr = torch.full((rep.n + 1,), -1, dtype=torch.int64).pin_memory()
+    col = torch.empty(1000, dtype=torch.int32).pin_memory()
+    d8 = torch.empty(1000, dtype=torch.uint8).pin_memory()
+    sig = oracle.minhash(rep.seqs, rep.offsets, 5, 64, SEED)
+    want_pairs, _, _ = oracle.lsh_sorted(sig, 16, 4, 8)
+    cnt = sq.pipeline_host_csr(seqs_h, offs_h, 20, max_len, 5, 64, SEED, 16, 4, 8, 3, row_ptr, col, d8)
+    assert cnt == want_pairs.shape[0]
+    want_rp = np.searchsorted(want_pairs[:, 0], np.arange(rep.n + 1), side="left")
+    assert np.array_equal(row_ptr.numpy(), want_rp)
+    with pytest.raises(SubQuadError) as e:
+        sq.pipeline_host_csr(seqs_h, offs_h, 20, max_len, 5, 64, SEED, 16, 4, 8, 255, row_ptr, col, d8)
+    assert e.value.code == SQ_ERR_UNSUPPORTED
+    sq.close()
