@@ -517,3 +517,47 @@ def test_pipeline_host_csr_no_candidates_and_limits():
         sq.pipeline_host_csr(seqs_h, offs_h, 20, max_len, 5, 64, SEED, 16, 4, 8, 255, row_ptr, col, d8)
     assert e.value.code == SQ_ERR_UNSUPPORTED
     sq.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# long sequences under a threshold: look-ahead filter + banded multi-word column
+# ---------------------------------------------------------------------------------------------
+def _edited_families(rng, n_fam, members, L_lo, L_hi, max_edits):
+    seqs = []
+    for _ in range(n_fam):
+        base = rng.integers(0, 20, rng.integers(L_lo, L_hi + 1)).astype(np.uint8)
+        for _ in range(members):
+            s = list(base)
+            for _ in range(rng.integers(0, max_edits + 1)):
+                op = rng.integers(0, 3)
+                pos = rng.integers(0, len(s) + (op == 1))
+                if op == 0 and len(s):
+                    s[min(pos, len(s) - 1)] = rng.integers(0, 20)
+                elif op == 1:
+                    s.insert(pos, rng.integers(0, 20))
+                elif len(s) > 1:
+                    del s[min(pos, len(s) - 1)]
+            seqs.append(np.asarray(s, np.uint8))
+    order = rng.permutation(len(seqs))
+    return dg.from_list([seqs[q] for q in order])
+
+
+@pytest.mark.parametrize("L_lo,L_hi,max_edits,max_d", [
+    (66, 80, 6, 3), (66, 80, 12, 8), (100, 130, 20, 15), (100, 130, 40, 31), (100, 130, 40, 32),
+    (150, 160, 24, 20), (200, 225, 30, 25), (33, 70, 10, 7), (120, 125, 3, 0)])
+def test_all_pairs_long_thresholded_band(L_lo, L_hi, max_edits, max_d):
+    """Distances straddle max_d (edits up to ~1.3 max_d per member), lengths span 2-8 words."""
+    rng = np.random.default_rng(L_lo * 1000 + max_d)
+    rep = _edited_families(rng, 12, 40, L_lo, L_hi, max_edits)
+    want_p, want_d = oracle.all_pairs_threshold(rep.seqs, rep.offsets, max_d)
+    assert want_p.shape[0] > 100
+    binding, sq = _ctx()
+    cap = want_p.shape[0] + 64
+    _pack(sq, binding, rep, op=binding.OP_ALL_PAIRS, pair_capacity=cap)
+    pairs = torch.empty((cap, 2), dtype=torch.int32, device="cuda")
+    dist = torch.empty(cap, dtype=torch.int16, device="cuda")
+    cnt = sq.all_pairs(max_d, pairs, dist)
+    assert cnt == want_p.shape[0]
+    assert np.array_equal(_u32(pairs)[:cnt], want_p)
+    assert np.array_equal(_u16(dist)[:cnt], want_d)
+    sq.close()
