@@ -189,7 +189,8 @@ size_t sq_allpairs_scratch_bytes(int64_t n, int64_t pair_capacity) {
   return 2 * sq_align_up(cap * 8 + 16) + 2 * sq_align_up(cap * 4 + 16) +
          sq_sort_scratch_bytes(pair_capacity, 1) +
          sq_align_up(nn * 32 + 16) + sq_align_up(nn * 4 + 16) +          // histograms, lengths
-         2 * sq_align_up(scap * 8 + 16) + sq_align_up(scap * 2 + 16) + 4096;   // survivors (x2), distances
+         2 * sq_align_up(scap * 8 + 16) + sq_align_up(scap * 2 + 16) +        // survivors (x2), distances
+         sq_sort_scratch_bytes((int64_t)scap, 1) + 4096;
 }
 
 extern "C" int sq_all_pairs(sq_ctx* c, int max_d, uint32_t* pairs_out, uint16_t* dist_out,
@@ -235,7 +236,8 @@ extern "C" int sq_all_pairs(sq_ctx* c, int max_d, uint32_t* pairs_out, uint16_t*
     uint2* surv = sq_scratch<uint2>(c, scap);
     uint16_t* sdist = sq_scratch<uint16_t>(c, scap);
     uint2* surv2 = sq_scratch<uint2>(c, scap);
-    if (rh && lens && surv && sdist && surv2 && c->alphabet <= 32) {
+    uint8_t* tmp2 = sq_scratch<uint8_t>(c, sq_sort_scratch_bytes((int64_t)scap, 1));
+    if (rh && lens && surv && sdist && surv2 && tmp2 && c->alphabet <= 32) {
       SQ_TIMED(c, SQ_K_ALLPAIRS, residue_hist_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(
           c->packed, c->stride, n, rh, lens));
       SQ_LAUNCH_CHECK(c);
@@ -249,22 +251,13 @@ extern "C" int sq_all_pairs(sq_ctx* c, int max_d, uint32_t* pairs_out, uint16_t*
       if ((size_t)ns <= scap) {
         filtered = true;
         if (ns > 0) {
-          // long sequences: drop the survivors whose first columns already rule a hit out
+          // (long sequences: grouping by i and the banded shared-Peq kernel -- sq_edit.cu)
           const uint2* live = surv;
           int64_t nlive = ns;
-          int applied = 0;
-          SQ_CUDA(c, cudaMemsetAsync(c->dflags + 2, 0, 8, st));
-          rc = sq_dp_prefilter(c, c->packed, n, c->max_len, surv, ns, max_d, surv2, c->dflags + 2, &applied);
+          rc = sq_survivor_distances(c, c->packed, n, c->max_len, surv, ns, max_d, surv2, tmp2, sdist, &live,
+                                     &nlive);
           if (rc != SQ_OK) return rc;
-          if (applied) {
-            SQ_CUDA(c, cudaMemcpyAsync(c->pinned, c->dflags + 2, 8, cudaMemcpyDeviceToHost, st));
-            SQ_CUDA(c, cudaStreamSynchronize(st));
-            live = surv2; nlive = (int64_t)c->pinned[0];
-          }
           if (nlive > 0) {
-            rc = sq_edit_distance_ab(c, c->packed, n, c->max_len, reinterpret_cast<const uint32_t*>(live), nlive,
-                                     max_d, sdist, applied != 0);
-            if (rc != SQ_OK) return rc;
             SQ_TIMED(c, SQ_K_ALLPAIRS, hit_compact_kernel<<<(unsigned)((nlive + 255) / 256), 256, 0, st>>>(
                 live, sdist, nlive, max_d, hp, hd, (unsigned long long)capacity, c->dflags));
             SQ_LAUNCH_CHECK(c);

@@ -142,14 +142,15 @@ int sq_minhash_impl(sq_ctx* c, int k, int H, uint64_t seed, uint32_t* sig_out);
 int sq_edit_distance_impl(sq_ctx* c, const uint32_t* pairs, int64_t n_pairs, int max_d,
                           uint16_t* dist_out);
 // pairs (i, j) with i in the context's own pack and j in `packedB` (same stride and alphabet)
-// banded: most pairs are expected within max_d (they passed a filter) -- multi-word pairs then
-// take the banded column without early exit (sq_dp.cuh)
+// banded: the pairs passed a filter (most are within max_d) and come grouped by i -- sequences
+// longer than 64 then take the banded shared-Peq kernel (no early exit)
 int sq_edit_distance_ab(sq_ctx* c, const uint8_t* packedB, int64_t nB, int max_len_b,
                         const uint32_t* pairs, int64_t n_pairs, int max_d, uint16_t* dist_out,
                         bool banded);
-// long sequences: survivors that can still be within max_d after a look at the first columns
-int sq_dp_prefilter(sq_ctx* c, const uint8_t* packedB, int64_t nB, int max_len_b, const uint2* surv,
-                    int64_t ns, int max_d, uint2* alive_out, unsigned long long* counter, int* applied);
+// survivors of a coarse filter -> distances (grouping by i, banded shared-Peq kernel; sq_edit.cu)
+int sq_survivor_distances(sq_ctx* c, const uint8_t* packedB, int64_t nB, int max_len_b, uint2* surv,
+                          int64_t ns, int max_d, uint2* surv2, void* sort_tmp, uint16_t* sdist,
+                          const uint2** live_out, int64_t* nlive_out);
 // pieces of the thresholded all-pairs path (sq_allpairs.cu) shared with the join (sq_join.cu)
 int sq_residue_hist(sq_ctx* c, const uint8_t* packed, int stride, int64_t n, uint32_t* rh, uint32_t* lens);
 int sq_hit_compact(sq_ctx* c, const uint2* surv, const uint16_t* sdist, int64_t ns, int max_d,

@@ -94,75 +94,8 @@ __device__ __forceinline__ int sq_myers(const uint32_t* peq, int cstride, int ts
   return score;
 }
 
-// The same column step restricted to the words that meet the diagonal band |x - y| <= max_d
-// (Ukkonen's cut-off on the word grid).  Text index y produces DP column y + 1, whose band rows
-// y + 1 - max_d .. y + 1 + max_d live in words (y - max_d) >> 5 .. (y + max_d) >> 5.
-//  * words below the band are not touched until the band reaches them; their stale state (all
-//    vertical deltas +1) is then an OVERESTIMATE of the column they join -- a true vertical delta
-//    is at most +1;
-//  * words above the band are dropped; the first active word takes the boundary inputs of word 0
-//    (horizontal delta +1, no carry) -- again an overestimate, a true horizontal delta is <= +1.
-// The DP is monotone, so every computed value is >= the true one, and a cell whose true value is
-// <= max_d is exact (its optimal path never leaves the band, and a minimum over one exact and
-// other overestimated candidates is exact).  Hence min(result, max_d + 1) is exact.  The tracked
-// score is the cell at the bottom of the highest active word.  No early exit (an overestimate
-// proves nothing about columns to come).  Needs |m - n| <= max_d, m, n >= 1.
-template <int W>
-__device__ __forceinline__ int sq_myers_banded(const uint32_t* peq, int cstride, int tstride, int m,
-                                               const uint8_t* __restrict__ b, int n, int max_d) {
-  uint32_t Pv[W], Mv[W];
-#pragma unroll
-  for (int w = 0; w < W; ++w) { Pv[w] = 0xFFFFFFFFu; Mv[w] = 0u; }
-  const int last = (m - 1) >> 5;
-  const int topbit = (m - 1) & 31;
-  int whi = (max_d >> 5) < last ? (max_d >> 5) : last;
-  int score = whi == last ? m : 32 * (whi + 1);
-  const uint32_t* b32 = reinterpret_cast<const uint32_t*>(b);
-  for (int y0 = 0; y0 < n; y0 += 4) {
-    const uint32_t word = b32[y0 >> 2];
-#pragma unroll
-    for (int q = 0; q < 4; ++q) {
-      const int y = y0 + q;
-      if (y >= n) break;
-      const uint32_t ch = (word >> (8 * q)) & 0xFFu;
-      int nwhi = (y + max_d) >> 5;
-      nwhi = nwhi < last ? nwhi : last;
-      if (nwhi > whi) { whi = nwhi; score += whi == last ? m - 32 * last : 32; }
-      const int wlo = y >= max_d ? (y - max_d) >> 5 : 0;
-      uint32_t carry = 0u, ph_in = 1u, mh_in = 0u;
-#pragma unroll
-      for (int w = 0; w < W; ++w) {
-        if (w < wlo || w > whi) continue;
-        const uint32_t Eq = peq[(ch * cstride + w) * tstride];
-        const uint32_t pv = Pv[w], mv = Mv[w];
-        const uint32_t Xv = Eq | mv;
-        const uint64_t s64 = (uint64_t)(Eq & pv) + (uint64_t)pv + (uint64_t)carry;
-        const uint32_t sum = (uint32_t)s64;
-        carry = (uint32_t)(s64 >> 32);
-        const uint32_t Xh = (sum ^ pv) | Eq;
-        uint32_t Ph = mv | ~(Xh | pv);
-        uint32_t Mh = pv & Xh;
-        if (w == whi) {
-          const int tb = w == last ? topbit : 31;
-          score += (int)((Ph >> tb) & 1u) - (int)((Mh >> tb) & 1u);
-        }
-        const uint32_t ph_out = Ph >> 31, mh_out = Mh >> 31;
-        Ph = (Ph << 1) | ph_in;
-        Mh = (Mh << 1) | mh_in;
-        ph_in = ph_out;
-        mh_in = mh_out;
-        Pv[w] = Mh | ~(Xv | Ph);
-        Mv[w] = Ph & Xv;
-      }
-    }
-  }
-  return score;
-}
-
 // Whole distance for one pair of packed slots, with the trivial cases and the length filter.
-// BANDED: the caller expects most pairs to be within max_d (candidates that passed a filter), so
-// the banded column (no early exit) beats the full column with its early exit.
-template <int W, bool BANDED = false>
+template <int W>
 __device__ __forceinline__ int sq_pair_distance(const uint8_t* __restrict__ rowA,
                                                 const uint8_t* __restrict__ rowB, int stride,
                                                 int alphabet, int max_d, uint32_t* peq,
@@ -175,8 +108,7 @@ __device__ __forceinline__ int sq_pair_distance(const uint8_t* __restrict__ rowA
   else if (n == 0) d = m;
   else {
     sq_peq_build<W>(rowA, m, alphabet, peq, tstride);
-    if (BANDED && W > 1 && max_d >= 0) d = sq_myers_banded<W>(peq, W, tstride, m, rowB, n, max_d);
-    else d = sq_myers<W>(peq, W, tstride, m, rowB, n, max_d);
+    d = sq_myers<W>(peq, W, tstride, m, rowB, n, max_d);
   }
   if (max_d >= 0 && d > max_d) d = max_d + 1;
   return d;

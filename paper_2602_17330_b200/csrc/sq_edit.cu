@@ -7,7 +7,7 @@
 
 namespace {
 
-template <int W, bool BANDED>
+template <int W>
 __global__ void edit_pairs_kernel(const uint8_t* __restrict__ packed, int stride, int64_t n,
                                   const uint8_t* __restrict__ packedB, int64_t nB,
                                   const uint2* __restrict__ pairs, int64_t n_pairs, int max_d,
@@ -17,7 +17,7 @@ __global__ void edit_pairs_kernel(const uint8_t* __restrict__ packed, int stride
   if (p >= n_pairs) return;
   const uint2 pr = pairs[p];
   if (pr.x >= (uint64_t)n || pr.y >= (uint64_t)nB) { dist[p] = 0xFFFFu; return; }
-  const int d = sq_pair_distance<W, BANDED>(packed + (int64_t)pr.x * stride, packedB + (int64_t)pr.y * stride,
+  const int d = sq_pair_distance<W>(packed + (int64_t)pr.x * stride, packedB + (int64_t)pr.y * stride,
                                     stride, alphabet, max_d, peq_smem + threadIdx.x, blockDim.x);
   dist[p] = (uint16_t)d;
 }
@@ -174,112 +174,172 @@ int launch_edit_w1(sq_ctx* c, const uint8_t* packedB, int64_t nB, const uint32_t
   return SQ_OK;
 }
 
-template <int W, bool BANDED>
-int launch_edit_wb(sq_ctx* c, const uint8_t* packedB, int64_t nB, const uint32_t* pairs, int64_t n_pairs,
-                   int max_d, uint16_t* dist_out) {
+template <int W>
+int launch_edit(sq_ctx* c, const uint8_t* packedB, int64_t nB, const uint32_t* pairs, int64_t n_pairs,
+                int max_d, uint16_t* dist_out) {
   const int threads = W <= 2 ? 256 : 128;
   const size_t smem = (size_t)c->alphabet * W * threads * sizeof(uint32_t);
   if (smem > 48 * 1024)
-    SQ_CUDA(c, cudaFuncSetAttribute(edit_pairs_kernel<W, BANDED>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    SQ_CUDA(c, cudaFuncSetAttribute(edit_pairs_kernel<W>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     (int)smem));
   const int64_t blocks = (n_pairs + threads - 1) / threads;
-  SQ_TIMED(c, SQ_K_EDIT, edit_pairs_kernel<W, BANDED><<<(unsigned)blocks, threads, smem, c->stream>>>(
+  SQ_TIMED(c, SQ_K_EDIT, edit_pairs_kernel<W><<<(unsigned)blocks, threads, smem, c->stream>>>(
       c->packed, c->stride, c->n, packedB, nB, reinterpret_cast<const uint2*>(pairs), n_pairs, max_d,
       c->alphabet, dist_out));
   SQ_LAUNCH_CHECK(c);
   return SQ_OK;
 }
 
-template <int W>
-int launch_edit(sq_ctx* c, const uint8_t* packedB, int64_t nB, const uint32_t* pairs, int64_t n_pairs,
-                int max_d, uint16_t* dist_out, bool banded) {
-  // the band only pays when it is narrower than the words
-  if (banded && W > 1 && max_d >= 0 && 2 * max_d + 1 < 32 * (W - 1))
-    return launch_edit_wb<W, true>(c, packedB, nB, pairs, n_pairs, max_d, dist_out);
-  return launch_edit_wb<W, false>(c, packedB, nB, pairs, n_pairs, max_d, dist_out);
-}
+// ---- long sequences, banded, Peq shared per run of equal i --------------------------------------
+// For pairs that passed a filter (most are within max_d) and come grouped by i: a warp takes 32
+// consecutive pairs, builds the Peq table of every distinct pattern once (match.any per 32
+// pattern positions, as in the single-word kernel) in shared memory [run][residue][word], and each
+// lane runs the column step of sq_dp.cuh restricted to the diagonal band |x - y| <= max_d
+// (Ukkonen's cut-off on the word grid) as a SLIDING WINDOW of NWIN words.  Text index y produces
+// DP column y + 1, whose band rows y + 1 - max_d .. y + 1 + max_d lie in words (y - max_d) >> 5
+// .. (y + max_d) >> 5; the window's first word is (y - max_d) >> 5 and 32 NWIN >= 2 max_d + 32
+// makes it cover the band and, in the last column, row m (|m - n| <= max_d is checked first).
+//  * when the window moves down, a fresh word (all vertical deltas +1) enters at the bottom: an
+//    OVERESTIMATE of the column it joins, a true vertical delta being at most +1;
+//  * the word that leaves at the top is dropped, and the window's first word takes the boundary
+//    inputs of word 0 (horizontal delta +1, no carry): again an overestimate.
+// The DP is monotone, so every computed value is >= the true one, and a cell whose true value is
+// <= max_d is exact (its optimal path never leaves the band; a minimum over one exact and other
+// overestimated candidates is exact).  Hence min(result, max_d + 1) is exact.  The tracked value
+// is the cell at the bottom of the window; D[m][n] is read off it through the vertical deltas
+// below row m.  No early exit (an overestimate proves nothing about columns to come).
+constexpr int kLgWarps = 8;
+constexpr int kLgRuns = 2;
 
-// ---- long sequences under a threshold: a cheap look at the first columns ----------------------
-// Every alignment path leaves column C through some cell (x, C), and from there to (m, n) it
-// costs at least |(m - x) - (n - C)|, so  D[m][n] >= min_x ( D[x][C] + |(m - x) - (n - C)| ).
-// Rows x > 64 of column C have D >= x - C > max_d when C < 64 - max_d, so the minimum over the
-// rows of the first two words decides: if it exceeds max_d the pair cannot be a hit and the full
-// multi-word DP (4-8 words x 100+ columns) is never run for it.  One thread per pair, a two-word
-// Myers/Hyyro column for C columns, then one walk down the column.  Pairs that may still be hits
-// are compacted (warp-aggregated append) for the full kernel.
-constexpr int kPfThreads = 256;
-
-__global__ void __launch_bounds__(kPfThreads)
-dp_prefilter_kernel(const uint8_t* __restrict__ packedA, const uint8_t* __restrict__ packedB, int stride,
-                    int64_t nA, int64_t nB, const uint2* __restrict__ surv, int64_t ns, int max_d,
-                    int alphabet, int C, uint2* __restrict__ alive_out,
-                    unsigned long long* __restrict__ counter) {
-  extern __shared__ uint32_t peq_smem[];               // [alphabet][2][kPfThreads]
-  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  const bool valid = p < ns;
-  bool alive = valid;
-  uint2 pr = make_uint2(0u, 0u);
-  if (valid) {
-    pr = surv[p];
-    if (pr.x < (uint64_t)nA && pr.y < (uint64_t)nB) {
-      const uint8_t* rowA = packedA + (int64_t)pr.x * stride;
-      const uint8_t* rowB = packedB + (int64_t)pr.y * stride;
-      const int m = rowA[stride - 1], n = rowB[stride - 1];
-      if (n >= C && m >= 1) {
-        const int mr = m < 64 ? m : 64;                // pattern rows held in the two words
-        uint32_t* peq = peq_smem + threadIdx.x;
-        sq_peq_build<2>(rowA, mr, alphabet, peq, kPfThreads);
-        uint32_t Pv0 = 0xFFFFFFFFu, Pv1 = 0xFFFFFFFFu, Mv0 = 0u, Mv1 = 0u;
-        const uint32_t* b32 = reinterpret_cast<const uint32_t*>(rowB);
-        for (int y0 = 0; y0 < C; y0 += 4) {
-          const uint32_t word = b32[y0 >> 2];
+template <int NWIN>
+__global__ void __launch_bounds__(kLgWarps * 32)
+edit_long_shared_kernel(const uint8_t* __restrict__ packedA, int64_t nA, const uint8_t* __restrict__ packedB,
+                        int64_t nB, int stride, int alphabet, int W, const uint2* __restrict__ pairs,
+                        int64_t n_pairs, int max_d, uint16_t* __restrict__ dist) {
+  extern __shared__ uint32_t lg_smem[];                 // [kLgWarps][kLgRuns][alphabet * WP] + lengths
+  const int WP = W | 1;                                 // odd word stride per residue
+  const int tsz = alphabet * WP;
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  uint32_t* peq = lg_smem + (size_t)w * kLgRuns * tsz;
+  uint32_t* mlen = lg_smem + (size_t)kLgWarps * kLgRuns * tsz + w * kLgRuns;
+  const int64_t p = ((int64_t)blockIdx.x * kLgWarps + w) * 32 + lane;
+  const bool valid = p < n_pairs;
+  uint2 pr = make_uint2(0xFFFFFFFFu, 0xFFFFFFFFu);
+  if (valid) pr = pairs[p];
+  const bool inrange = valid && pr.x < (uint64_t)nA && pr.y < (uint64_t)nB;
+  const uint32_t i = inrange ? pr.x : 0xFFFFFFFFu;
+  const uint8_t* rowB = packedB + (int64_t)(inrange ? pr.y : 0u) * stride;
+  const int n = inrange ? (int)rowB[stride - 1] : 0;
+  const uint32_t prev = __shfl_up_sync(0xFFFFFFFFu, i, 1);
+  const uint32_t hm = __ballot_sync(0xFFFFFFFFu, lane == 0 || i != prev);
+  const int run = __popc(hm & (0xFFFFFFFFu >> (31 - lane))) - 1;
+  const int nruns = __popc(hm);
+  uint32_t rem = hm;
+  int d = 0;
+#pragma unroll 1
+  for (int rbase = 0; rbase < nruns; rbase += kLgRuns) {
+    const int nr = min(kLgRuns, nruns - rbase);
+    __syncwarp();
+#pragma unroll 1
+    for (int r = 0; r < nr; ++r) {
+      const int hl = __ffs(rem) - 1;
+      rem &= rem - 1;
+      const uint32_t ir = __shfl_sync(0xFFFFFFFFu, i, hl);
+      uint32_t* t = peq + r * tsz;
+      for (int q = lane; q < tsz; q += 32) t[q] = 0u;
+      int m = 0;
+      if (ir != 0xFFFFFFFFu) m = packedA[(int64_t)ir * stride + stride - 1];
+      __syncwarp();
+      for (int k = 0; 32 * k < m; ++k) {
+        const int x = 32 * k + lane;
+        const uint32_t ch = x < m ? packedA[(int64_t)ir * stride + x] : 0xFFu;
+        const uint32_t mm = __match_any_sync(0xFFFFFFFFu, ch);
+        if (x < m && lane == __ffs(mm) - 1) t[ch * WP + k] = mm;
+      }
+      if (lane == 0) mlen[r] = (uint32_t)m;
+    }
+    __syncwarp();
+    if (!inrange || run < rbase || run >= rbase + nr) continue;
+    const int m = (int)mlen[run - rbase];
+    const uint32_t* t = peq + (run - rbase) * tsz;
+    const int diff = m > n ? m - n : n - m;
+    if (diff > max_d) { d = max_d + 1; continue; }
+    if (m == 0) { d = n; continue; }
+    if (n == 0) { d = m; continue; }
+    const int last = (m - 1) >> 5, topbit = (m - 1) & 31;
+    uint32_t Pw[NWIN], Mw[NWIN];
 #pragma unroll
-          for (int q = 0; q < 4; ++q) {
-            if (y0 + q < C) {
-              const uint32_t ch = (word >> (8 * q)) & 0xFFu;
-              const uint32_t Eq0 = peq[(ch * 2) * kPfThreads], Eq1 = peq[(ch * 2 + 1) * kPfThreads];
-              // word 0
-              const uint32_t Xv0 = Eq0 | Mv0;
-              const uint64_t s0 = (uint64_t)(Eq0 & Pv0) + (uint64_t)Pv0;
-              const uint32_t Xh0 = ((uint32_t)s0 ^ Pv0) | Eq0;
-              uint32_t Ph0 = Mv0 | ~(Xh0 | Pv0), Mh0 = Pv0 & Xh0;
-              const uint32_t pc = Ph0 >> 31, mc = Mh0 >> 31;
-              Ph0 = (Ph0 << 1) | 1u; Mh0 <<= 1;
-              Pv0 = Mh0 | ~(Xv0 | Ph0); Mv0 = Ph0 & Xv0;
-              // word 1 (carry of the addition and of the two shifts comes from word 0)
-              const uint32_t Xv1 = Eq1 | Mv1;
-              const uint32_t s1 = (Eq1 & Pv1) + Pv1 + (uint32_t)(s0 >> 32);
-              const uint32_t Xh1 = (s1 ^ Pv1) | Eq1;
-              uint32_t Ph1 = Mv1 | ~(Xh1 | Pv1), Mh1 = Pv1 & Xh1;
-              Ph1 = (Ph1 << 1) | pc; Mh1 = (Mh1 << 1) | mc;
-              Pv1 = Mh1 | ~(Xv1 | Ph1); Mv1 = Ph1 & Xv1;
-            }
-          }
+    for (int k = 0; k < NWIN; ++k) { Pw[k] = 0xFFFFFFFFu; Mw[k] = 0u; }
+    int wlo = 0;
+    int sb = 32 * NWIN;                                  // D at the bottom row of the window
+    const uint32_t* b32 = reinterpret_cast<const uint32_t*>(rowB);
+    for (int y0 = 0; y0 < n; y0 += 4) {
+      const uint32_t word = b32[y0 >> 2];
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        const int y = y0 + q;
+        if (y >= n) break;
+        if (y >= max_d && ((y - max_d) >> 5) > wlo) {    // the band has left the top word
+#pragma unroll
+          for (int k = 0; k + 1 < NWIN; ++k) { Pw[k] = Pw[k + 1]; Mw[k] = Mw[k + 1]; }
+          Pw[NWIN - 1] = 0xFFFFFFFFu; Mw[NWIN - 1] = 0u;
+          ++wlo;
+          sb += 32;
         }
-        // walk down column C: D[0][C] = C
-        const int rem_n = n - C;
-        int D = C;
-        int best = D + (m > rem_n ? m - rem_n : rem_n - m);
-        const int xmax = mr < C + max_d ? mr : C + max_d;      // deeper rows have D > max_d
-        const uint64_t Pv = (uint64_t)Pv0 | ((uint64_t)Pv1 << 32), Mv = (uint64_t)Mv0 | ((uint64_t)Mv1 << 32);
-        for (int x = 1; x <= xmax; ++x) {
-          D += (int)((Pv >> (x - 1)) & 1ull) - (int)((Mv >> (x - 1)) & 1ull);
-          const int rm = m - x;
-          const int cand = D + (rm > rem_n ? rm - rem_n : rem_n - rm);
-          best = cand < best ? cand : best;
+        const uint32_t* te = t + ((word >> (8 * q)) & 0xFFu) * WP + wlo;
+        uint32_t carry = 0u, ph_in = 1u, mh_in = 0u;
+#pragma unroll
+        for (int k = 0; k < NWIN; ++k) {
+          const uint32_t Eq = wlo + k < W ? te[k] : 0u;
+          const uint32_t pv = Pw[k], mv = Mw[k];
+          const uint32_t Xv = Eq | mv;
+          const uint64_t s64 = (uint64_t)(Eq & pv) + (uint64_t)pv + (uint64_t)carry;
+          carry = (uint32_t)(s64 >> 32);
+          const uint32_t Xh = ((uint32_t)s64 ^ pv) | Eq;
+          uint32_t Ph = mv | ~(Xh | pv);
+          uint32_t Mh = pv & Xh;
+          const uint32_t ph_out = Ph >> 31, mh_out = Mh >> 31;
+          if (k == NWIN - 1) sb += (int)ph_out - (int)mh_out;
+          Ph = (Ph << 1) | ph_in;
+          Mh = (Mh << 1) | mh_in;
+          ph_in = ph_out;
+          mh_in = mh_out;
+          Pw[k] = Mh | ~(Xv | Ph);
+          Mw[k] = Ph & Xv;
         }
-        alive = best <= max_d;
       }
     }
+    // from the window's bottom row up to row m
+    const int kl = last - wlo;                           // 0 <= kl < NWIN (see the header comment)
+#pragma unroll
+    for (int k = 0; k < NWIN; ++k) {
+      if (k > kl) sb -= __popc(Pw[k]) - __popc(Mw[k]);
+      else if (k == kl) {
+        const uint32_t above = topbit == 31 ? 0u : (0xFFFFFFFFu << (topbit + 1));
+        sb -= __popc(Pw[k] & above) - __popc(Mw[k] & above);
+      }
+    }
+    d = sb;
   }
-  const uint32_t mask = __ballot_sync(0xFFFFFFFFu, alive);
-  if (mask) {
-    const int lane = threadIdx.x & 31;
-    unsigned long long base = 0;
-    if (lane == __ffs(mask) - 1) base = atomicAdd(counter, (unsigned long long)__popc(mask));
-    base = __shfl_sync(0xFFFFFFFFu, base, __ffs(mask) - 1);
-    if (alive) alive_out[base + __popc(mask & ((1u << lane) - 1u))] = pr;
-  }
+  if (!valid) return;
+  if (!inrange) { dist[p] = 0xFFFFu; return; }
+  if (d > max_d) d = max_d + 1;
+  dist[p] = (uint16_t)d;
+}
+
+template <int NWIN>
+int launch_edit_long(sq_ctx* c, const uint8_t* packedB, int64_t nB, int words, const uint32_t* pairs,
+                     int64_t n_pairs, int max_d, uint16_t* dist_out) {
+  const int WP = words | 1;
+  const size_t smem = ((size_t)kLgWarps * kLgRuns * c->alphabet * WP + kLgWarps * kLgRuns) * sizeof(uint32_t);
+  if (smem > 48 * 1024)
+    SQ_CUDA(c, cudaFuncSetAttribute(edit_long_shared_kernel<NWIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  const int64_t blocks = (n_pairs + kLgWarps * 32 - 1) / (kLgWarps * 32);
+  SQ_TIMED(c, SQ_K_EDIT, edit_long_shared_kernel<NWIN><<<(unsigned)blocks, kLgWarps * 32, smem, c->stream>>>(
+      c->packed, c->n, packedB, nB, c->stride, c->alphabet, words, reinterpret_cast<const uint2*>(pairs),
+      n_pairs, max_d, dist_out));
+  SQ_LAUNCH_CHECK(c);
+  return SQ_OK;
 }
 
 }  // namespace
@@ -299,31 +359,48 @@ int sq_edit_distance_ab(sq_ctx* c, const uint8_t* packedB, int64_t nB, int max_l
   if (c->stride == 32) return launch_edit_w1<32>(c, packedB, nB, pairs, n_pairs, max_d, dist_out);
   const int ml = c->max_len > max_len_b ? c->max_len : max_len_b;
   const int words = (ml + 31) / 32;
-  if (words <= 1) return launch_edit<1>(c, packedB, nB, pairs, n_pairs, max_d, dist_out, banded);
-  if (words <= 2) return launch_edit<2>(c, packedB, nB, pairs, n_pairs, max_d, dist_out, banded);
-  if (words <= 4) return launch_edit<4>(c, packedB, nB, pairs, n_pairs, max_d, dist_out, banded);
-  if (words <= 5) return launch_edit<5>(c, packedB, nB, pairs, n_pairs, max_d, dist_out, banded);
-  if (words <= 8) return launch_edit<8>(c, packedB, nB, pairs, n_pairs, max_d, dist_out, banded);
+  if (banded && words >= 3 && words <= 8 && max_d >= 0 && max_d <= 32 && c->alphabet <= 32) {
+    // filtered pairs grouped by i: shared Peq tables, sliding band window
+    if (max_d <= 16) return launch_edit_long<2>(c, packedB, nB, words, pairs, n_pairs, max_d, dist_out);
+    return launch_edit_long<3>(c, packedB, nB, words, pairs, n_pairs, max_d, dist_out);
+  }
+  if (words <= 1) return launch_edit<1>(c, packedB, nB, pairs, n_pairs, max_d, dist_out);
+  if (words <= 2) return launch_edit<2>(c, packedB, nB, pairs, n_pairs, max_d, dist_out);
+  if (words <= 4) return launch_edit<4>(c, packedB, nB, pairs, n_pairs, max_d, dist_out);
+  if (words <= 5) return launch_edit<5>(c, packedB, nB, pairs, n_pairs, max_d, dist_out);
+  if (words <= 8) return launch_edit<8>(c, packedB, nB, pairs, n_pairs, max_d, dist_out);
   return SQ_ERR_UNSUPPORTED;
 }
 
-// Survivors of a coarse filter -> those that can still be within max_d (see dp_prefilter_kernel).
-// Returns 1 through *applied when the look-ahead ran (alive pairs in alive_out, their number in
-// *counter on the device), 0 when it does not apply (short sequences, large max_d).
-int sq_dp_prefilter(sq_ctx* c, const uint8_t* packedB, int64_t nB, int max_len_b, const uint2* surv,
-                    int64_t ns, int max_d, uint2* alive_out, unsigned long long* counter, int* applied) {
-  *applied = 0;
+// Distances of the survivors of a coarse filter (sq_all_pairs, sq_join).  Long sequences: the
+// survivors are grouped by i (radix sort on the i field, ping-pong between surv and surv2) and
+// take the shared-Peq banded kernel.  *live_out = the list sdist refers to (surv or surv2).
+int sq_survivor_distances(sq_ctx* c, const uint8_t* packedB, int64_t nB, int max_len_b, uint2* surv,
+                          int64_t ns, int max_d, uint2* surv2, void* sort_tmp, uint16_t* sdist,
+                          const uint2** live_out, int64_t* nlive_out) {
+  *live_out = surv; *nlive_out = ns;
+  if (ns <= 0) return SQ_OK;
   const int ml = c->max_len > max_len_b ? c->max_len : max_len_b;
-  if (ml <= 64 || max_d < 0 || max_d > 31 || ns <= 0) return SQ_OK;
-  const int C = 64 - max_d - 1 < 48 ? 64 - max_d - 1 : 48;
-  const size_t smem = (size_t)c->alphabet * 2 * kPfThreads * sizeof(uint32_t);
-  if (smem > 48 * 1024)
-    SQ_CUDA(c, cudaFuncSetAttribute(dp_prefilter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  SQ_TIMED(c, SQ_K_EDIT, dp_prefilter_kernel<<<(unsigned)((ns + kPfThreads - 1) / kPfThreads), kPfThreads, smem, c->stream>>>(
-      c->packed, packedB, c->stride, c->n, nB, surv, ns, max_d, c->alphabet, C, alive_out, counter));
-  SQ_LAUNCH_CHECK(c);
-  *applied = 1;
-  return SQ_OK;
+  const int applied = (ml > 64 && max_d >= 0 && max_d <= 32 && c->alphabet <= 32) ? 1 : 0;
+  uint2* live = surv;
+  int64_t nlive = ns;
+  int rc = SQ_OK;
+  if (applied && nlive > 1) {
+    // group by i: LSD passes over the low word (a uint2 (i, j) is the 64-bit key i | j << 32)
+    int nb = 1;
+    while (nb < 32 && (1ll << nb) < c->n) ++nb;
+    int shifts[4], widths[4], q = 0;
+    for (int b = 0; b < nb; b += 8) { shifts[q] = b; widths[q] = nb - b >= 8 ? 8 : nb - b; ++q; }
+    int in_alt = 0;
+    rc = sq_radix_sort(c, reinterpret_cast<uint64_t*>(surv), reinterpret_cast<uint64_t*>(surv2), nullptr,
+                       nullptr, nlive, 1, shifts, widths, q, sort_tmp, &in_alt);
+    if (rc != SQ_OK) return rc;
+    if (in_alt) live = surv2;
+  }
+  *live_out = live; *nlive_out = nlive;
+  if (nlive == 0) return SQ_OK;
+  return sq_edit_distance_ab(c, packedB, nB, max_len_b, reinterpret_cast<const uint32_t*>(live), nlive, max_d,
+                             sdist, applied != 0);
 }
 
 int sq_edit_distance_impl(sq_ctx* c, const uint32_t* pairs, int64_t n_pairs, int max_d,

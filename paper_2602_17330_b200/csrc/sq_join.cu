@@ -108,7 +108,8 @@ int join_core(sq_ctx* a, const sq_ctx* b, int64_t a_begin, int64_t a_end, int ma
   uint2* surv = sq_scratch<uint2>(a, scap);
   uint16_t* sdist = sq_scratch<uint16_t>(a, scap);
   uint2* surv2 = sq_scratch<uint2>(a, scap);
-  if (!surv2 || !hp || !hp_alt || !hd || !hd_alt || !tmp || !rhA || !lensA || !rhB || !lensB || !surv || !sdist)
+  uint8_t* tmp2 = sq_scratch<uint8_t>(a, sq_sort_scratch_bytes((int64_t)scap, 1));
+  if (!surv2 || !tmp2 || !hp || !hp_alt || !hd || !hd_alt || !tmp || !rhA || !lensA || !rhB || !lensB || !surv || !sdist)
     return SQ_ERR_WORKSPACE;
   SQ_CUDA(a, cudaMemsetAsync(a->dflags, 0, 64, st));
   int rc = sq_residue_hist(a, a->packed + a_begin * a->stride, a->stride, rows, rhA, lensA);
@@ -137,22 +138,12 @@ int join_core(sq_ctx* a, const sq_ctx* b, int64_t a_begin, int64_t a_end, int ma
       continue;
     }
     if (ns == 0) continue;
-    // long sequences: drop the survivors whose first columns already rule a hit out
+    // (long sequences: grouping by i and the banded shared-Peq kernel -- sq_edit.cu)
     const uint2* live = surv;
     int64_t nlive = ns;
-    int applied = 0;
-    SQ_CUDA(a, cudaMemsetAsync(a->dflags + 2, 0, 8, st));
-    rc = sq_dp_prefilter(a, b->packed, nB, b->max_len, surv, ns, max_d, surv2, a->dflags + 2, &applied);
+    rc = sq_survivor_distances(a, b->packed, nB, b->max_len, surv, ns, max_d, surv2, tmp2, sdist, &live, &nlive);
     if (rc != SQ_OK) return rc;
-    if (applied) {
-      SQ_CUDA(a, cudaMemcpyAsync(a->pinned, a->dflags + 2, 8, cudaMemcpyDeviceToHost, st));
-      SQ_CUDA(a, cudaStreamSynchronize(st));
-      live = surv2; nlive = (int64_t)a->pinned[0];
-    }
     if (nlive == 0) continue;
-    rc = sq_edit_distance_ab(a, b->packed, nB, b->max_len, reinterpret_cast<const uint32_t*>(live), nlive,
-                             max_d, sdist, applied != 0);
-    if (rc != SQ_OK) return rc;
     rc = sq_hit_compact(a, live, sdist, nlive, max_d, hp, hd, capacity, a->dflags);
     if (rc != SQ_OK) return rc;
   }
@@ -215,7 +206,7 @@ size_t sq_join_scratch_bytes(int64_t rows, int64_t n_b, int64_t pair_capacity) {
   const size_t r = (size_t)(rows > 0 ? rows : 1), nb = (size_t)(n_b > 0 ? n_b : 1);
   return 2 * sq_align_up(cap * 8 + 16) + 2 * sq_align_up(cap * 4 + 16) + sq_sort_scratch_bytes(pair_capacity, 1) +
          sq_align_up(r * 32 + 16) + sq_align_up(r * 4 + 16) + sq_align_up(nb * 32 + 16) + sq_align_up(nb * 4 + 16) +
-         2 * sq_align_up(scap * 8 + 16) + sq_align_up(scap * 2 + 16) +
+         2 * sq_align_up(scap * 8 + 16) + sq_align_up(scap * 2 + 16) + sq_sort_scratch_bytes((int64_t)scap, 1) +
          2 * (sq_align_up(cap * 8 + 16) + sq_align_up(cap * 2 + 16)) + 4096;   // sq_join_host staging
 }
 
