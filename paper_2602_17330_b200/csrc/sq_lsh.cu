@@ -178,12 +178,11 @@ sched_fill_kernel(const uint32_t* __restrict__ rowstart, const uint32_t* __restr
 __device__ __forceinline__ uint64_t key_prefix(uint64_t k, int pshift) { return k >> pshift; }
 
 __global__ void __launch_bounds__(256)
-detect_mixed_kernel(const uint64_t* __restrict__ keys, int64_t n2, int64_t total, int pshift,
+detect_mixed_kernel(const uint64_t* __restrict__ keys, int64_t n2, int pshift,
                     uint32_t* __restrict__ list, unsigned long long* __restrict__ nlist) {
-  const int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (g >= total) return;
-  const int64_t q = g % n2;
-  if (q == 0) return;
+  const int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;     // position inside the band
+  if (q == 0 || q >= n2) return;
+  const int64_t g = (int64_t)blockIdx.y * n2 + q;
   const uint64_t k = keys[g], kp = keys[g - 1];
   if (k == kp || key_prefix(k, pshift) != key_prefix(kp, pshift)) return;
   // a full-key change inside a prefix run: walk back to the run's start; an earlier change in the
@@ -1048,9 +1047,9 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
     if (n2 < (1ll << 30) && kb < 8) {
       // prefix runs holding several full keys -> in full-key order (the list lives in `cnt`, which
       // is cleared afterwards; a mixed run has >= 2 records, so rec / 2 entries always suffice)
-      const int64_t tot = n2 * bands;
-      SQ_TIMED(c, SQ_K_SEGMENT, detect_mixed_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(
-          kin, n2, tot, 64 - 8 * kb, cnt, counters + 3));
+      dim3 gd((unsigned)((n2 + 255) / 256), (unsigned)bands);
+      SQ_TIMED(c, SQ_K_SEGMENT, detect_mixed_kernel<<<gd, 256, 0, st>>>(
+          kin, n2, 64 - 8 * kb, cnt, counters + 3));
       SQ_LAUNCH_CHECK(c);
       SQ_TIMED(c, SQ_K_SEGMENT, fix_mixed_kernel<<<(unsigned)(c->sm_count * 4), 256, 0, st>>>(
           kin, vin, kalt, valt, n2, 64 - 8 * kb, cnt, counters + 3));
