@@ -43,16 +43,17 @@ join_filter_kernel(const uint32_t* __restrict__ rhA, const uint32_t* __restrict_
   if (threadIdx.x < (unsigned)(8 * nr)) ha[threadIdx.x >> 3][threadIdx.x & 7] = rhA[r0 * 8 + threadIdx.x];
   if (threadIdx.x >= 128 && threadIdx.x < 128u + (unsigned)nr) la[threadIdx.x - 128] = (int)lensA[r0 + threadIdx.x - 128];
   __syncthreads();
-  const int64_t j = jbase + threadIdx.x;
-  const bool col = j < nB;
+  const int64_t cidx = jbase + threadIdx.x;
+  const bool col = cidx < nB;
   uint32_t hb[8] = {0, 0, 0, 0, 0, 0, 0, 0};
   int nl = 0;
+  const int64_t j = cidx;
   if (col) {
-    const uint4 b0 = reinterpret_cast<const uint4*>(rhB)[j * 2];
-    const uint4 b1 = reinterpret_cast<const uint4*>(rhB)[j * 2 + 1];
+    const uint4 b0 = reinterpret_cast<const uint4*>(rhB)[cidx * 2];
+    const uint4 b1 = reinterpret_cast<const uint4*>(rhB)[cidx * 2 + 1];
     hb[0] = b0.x; hb[1] = b0.y; hb[2] = b0.z; hb[3] = b0.w;
     hb[4] = b1.x; hb[5] = b1.y; hb[6] = b1.z; hb[7] = b1.w;
-    nl = (int)lensB[j];
+    nl = (int)lensB[cidx];
   }
   const int lane = threadIdx.x & 31;
   for (int r = 0; r < nr; ++r) {
@@ -75,6 +76,101 @@ join_filter_kernel(const uint32_t* __restrict__ rhA, const uint32_t* __restrict_
   }
 }
 
+// Both sides in order of length (row r is sequence a_base + permA[r] of A, column c is sequence
+// permB[c] of B): since |m - n| <= d, a tile of 16 rows only meets the columns whose length lies in
+// [min length of the tile - max_d, max length + max_d] -- a contiguous range of the sorted columns,
+// found by two binary searches.  Block (x, y) takes row tile x and every gridDim.y-th column block
+// of that range; the rest is the kernel above.
+template <int NW>
+__global__ void __launch_bounds__(kJoinThreads)
+join_filter_ranged_kernel(const uint32_t* __restrict__ rhA, const uint32_t* __restrict__ lensA,
+                          const uint32_t* __restrict__ permA, int64_t row0, int64_t rows, int64_t a_base,
+                          const uint32_t* __restrict__ rhB, const uint32_t* __restrict__ lensB,
+                          const uint32_t* __restrict__ permB, int64_t nB, int max_d,
+                          uint2* __restrict__ surv, unsigned long long scap,
+                          unsigned long long* __restrict__ counter) {
+  __shared__ uint32_t ha[kJoinRows][8];
+  __shared__ int la[kJoinRows];
+  __shared__ uint32_t ia[kJoinRows];
+  __shared__ int64_t crange[2];
+  const int64_t r0 = row0 + (int64_t)blockIdx.x * kJoinRows;
+  const int nr = (int)min((int64_t)kJoinRows, row0 + rows - r0);
+  if (threadIdx.x < (unsigned)(8 * nr)) ha[threadIdx.x >> 3][threadIdx.x & 7] = rhA[r0 * 8 + threadIdx.x];
+  if (threadIdx.x >= 128 && threadIdx.x < 128u + (unsigned)nr) {
+    la[threadIdx.x - 128] = (int)lensA[r0 + threadIdx.x - 128];
+    ia[threadIdx.x - 128] = permA[r0 + threadIdx.x - 128];
+  }
+  if (threadIdx.x == 255) {
+    // rows ascend in length: first column with length >= lo, first with length > hi
+    const int lo = (int)lensA[r0] - max_d, hi = (int)lensA[r0 + nr - 1] + max_d;
+    int64_t a = 0, b = nB;
+    while (a < b) { const int64_t mid = (a + b) >> 1; if ((int)lensB[mid] < lo) a = mid + 1; else b = mid; }
+    crange[0] = a;
+    b = nB;
+    while (a < b) { const int64_t mid = (a + b) >> 1; if ((int)lensB[mid] <= hi) a = mid + 1; else b = mid; }
+    crange[1] = a;
+  }
+  __syncthreads();
+  const int64_t c_lo = crange[0] / kJoinThreads * kJoinThreads, c_hi = crange[1];
+  const int lane = threadIdx.x & 31;
+  for (int64_t jbase = c_lo + (int64_t)blockIdx.y * kJoinThreads; jbase < c_hi;
+       jbase += (int64_t)gridDim.y * kJoinThreads) {
+    const int64_t cidx = jbase + threadIdx.x;
+    const bool col = cidx < c_hi;
+    uint32_t hb[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    int nl = 0;
+    uint32_t j = 0;
+    if (col) {
+      const uint4 b0 = reinterpret_cast<const uint4*>(rhB)[cidx * 2];
+      const uint4 b1 = reinterpret_cast<const uint4*>(rhB)[cidx * 2 + 1];
+      hb[0] = b0.x; hb[1] = b0.y; hb[2] = b0.z; hb[3] = b0.w;
+      hb[4] = b1.x; hb[5] = b1.y; hb[6] = b1.z; hb[7] = b1.w;
+      nl = (int)lensB[cidx];
+      j = permB[cidx];
+    }
+    for (int r = 0; r < nr; ++r) {
+      const int m = la[r];
+      uint32_t l1 = (uint32_t)(m > nl ? m - nl : nl - m);
+#pragma unroll
+      for (int q = 0; q < NW; ++q) l1 += __vsadu4(ha[r][q], hb[q]);
+      const bool pass = col && (int)(l1 >> 1) <= max_d;
+      const uint32_t mask = __ballot_sync(0xFFFFFFFFu, pass);
+      if (mask) {
+        unsigned long long base = 0;
+        if (lane == __ffs(mask) - 1) base = atomicAdd(counter, (unsigned long long)__popc(mask));
+        base = __shfl_sync(0xFFFFFFFFu, base, __ffs(mask) - 1);
+        if (pass) {
+          const unsigned long long slot = base + __popc(mask & ((1u << lane) - 1u));
+          if (slot < scap) surv[slot] = make_uint2((uint32_t)a_base + ia[r], j);
+        }
+      }
+    }
+  }
+}
+
+// columns in order of length: histogram + length of column c = those of sequence perm[c]
+__global__ void __launch_bounds__(256)
+join_gather_cols_kernel(const uint32_t* __restrict__ rh, const uint32_t* __restrict__ lens,
+                        const uint32_t* __restrict__ perm, int64_t n, uint32_t* __restrict__ rh_s,
+                        uint32_t* __restrict__ lens_s) {
+  const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= n) return;
+  const uint32_t src = perm[c];
+  const uint4* in = reinterpret_cast<const uint4*>(rh) + (int64_t)src * 2;
+  uint4* out = reinterpret_cast<uint4*>(rh_s) + c * 2;
+  out[0] = in[0]; out[1] = in[1];
+  lens_s[c] = lens[src];
+}
+
+__global__ void __launch_bounds__(256)
+join_len_keys_kernel(const uint32_t* __restrict__ lens, int64_t n, uint64_t* __restrict__ keys,
+                     uint32_t* __restrict__ vals) {
+  const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= n) return;
+  keys[c] = lens[c];
+  vals[c] = (uint32_t)c;
+}
+
 inline int bits_for(int64_t n) {
   int b = 1;
   while (b < 32 && (1ll << b) < n) ++b;
@@ -82,6 +178,57 @@ inline int bits_for(int64_t n) {
 }
 
 inline size_t join_survivor_cap(int64_t cap) { return 4 * (size_t)(cap > 0 ? cap : 1) + 65536; }
+
+// (rh, lens) of n sequences -> the same in order of length + the permutation, in scratch above the
+// current top.  *ok = 0 when the scratch does not hold it (the caller then stays unsorted).
+int join_sort_by_length(sq_ctx* c, const uint32_t* rh, const uint32_t* lens, int64_t n,
+                        const uint32_t** perm, const uint32_t** rh_s, const uint32_t** lens_s, int* ok) {
+  *ok = 0;
+  uint64_t* lk = sq_scratch<uint64_t>(c, (size_t)n);
+  uint64_t* lk_alt = sq_scratch<uint64_t>(c, (size_t)n);
+  uint32_t* lv = sq_scratch<uint32_t>(c, (size_t)n);
+  uint32_t* lv_alt = sq_scratch<uint32_t>(c, (size_t)n);
+  uint8_t* ltmp = sq_scratch<uint8_t>(c, sq_sort_scratch_bytes(n, 1));
+  uint32_t* rhS = sq_scratch<uint32_t>(c, (size_t)n * 8);
+  uint32_t* lensS = sq_scratch<uint32_t>(c, (size_t)n);
+  if (!lk || !lk_alt || !lv || !lv_alt || !ltmp || !rhS || !lensS) return SQ_OK;
+  const unsigned gb = (unsigned)((n + 255) / 256);
+  SQ_TIMED(c, SQ_K_ALLPAIRS, join_len_keys_kernel<<<gb, 256, 0, c->stream>>>(lens, n, lk, lv));
+  SQ_LAUNCH_CHECK(c);
+  const int shifts[1] = {0}, widths[1] = {8};
+  int in_alt = 0;
+  int rc = sq_radix_sort(c, lk, lk_alt, lv, lv_alt, n, 1, shifts, widths, 1, ltmp, &in_alt);
+  if (rc != SQ_OK) return rc;
+  const uint32_t* pv = in_alt ? lv_alt : lv;
+  SQ_TIMED(c, SQ_K_ALLPAIRS, join_gather_cols_kernel<<<gb, 256, 0, c->stream>>>(rh, lens, pv, n, rhS, lensS));
+  SQ_LAUNCH_CHECK(c);
+  *perm = pv; *rh_s = rhS; *lens_s = lensS; *ok = 1;
+  return SQ_OK;
+}
+
+int join_filter_ranged(sq_ctx* c, const uint32_t* rhA, const uint32_t* lensA, const uint32_t* permA, int64_t row0,
+                       int64_t rows, int64_t a_base, const uint32_t* rhB, const uint32_t* lensB,
+                       const uint32_t* permB, int64_t nB, int max_d, uint2* surv, size_t scap,
+                       unsigned long long* counter) {
+  if (rows <= 0 || nB <= 0) return SQ_OK;
+  const int64_t tiles = (rows + kJoinRows - 1) / kJoinRows;
+  // enough blocks to fill the machine, at most one per column block
+  int64_t gy = ((int64_t)c->sm_count * 32 + tiles - 1) / tiles;
+  const int64_t cblocks = (nB + kJoinThreads - 1) / kJoinThreads;
+  if (gy > cblocks) gy = cblocks;
+  if (gy > 65535) gy = 65535;
+  if (gy < 1) gy = 1;
+  dim3 grid((unsigned)tiles, (unsigned)gy);
+  const unsigned long long sc = (unsigned long long)scap;
+  if (c->alphabet <= 20)
+    SQ_TIMED(c, SQ_K_ALLPAIRS, join_filter_ranged_kernel<5><<<grid, kJoinThreads, 0, c->stream>>>(
+        rhA, lensA, permA, row0, rows, a_base, rhB, lensB, permB, nB, max_d, surv, sc, counter));
+  else
+    SQ_TIMED(c, SQ_K_ALLPAIRS, join_filter_ranged_kernel<8><<<grid, kJoinThreads, 0, c->stream>>>(
+        rhA, lensA, permA, row0, rows, a_base, rhB, lensB, permB, nB, max_d, surv, sc, counter));
+  SQ_LAUNCH_CHECK(c);
+  return SQ_OK;
+}
 
 // Every hit of rows [a_begin, a_end) of A against all of B, sorted by (i, j), into device buffers.
 // Scratch is taken above the current top and given back.  Synchronises.
@@ -116,6 +263,23 @@ int join_core(sq_ctx* a, const sq_ctx* b, int64_t a_begin, int64_t a_end, int ma
   if (rc != SQ_OK) return rc;
   rc = sq_residue_hist(a, b->packed, b->stride, nB, rhB, lensB);
   if (rc != SQ_OK) return rc;
+  // both sides in order of length (stable radix sort of (length, index), one 8-bit pass): a tile of
+  // rows then only meets the columns within max_d of its lengths.  Not for SQ_JOIN_UPPER, whose
+  // blocks below the diagonal are skipped by index instead; without the scratch: unsorted.
+  const uint32_t* permA = nullptr; const uint32_t* permB = nullptr;
+  const uint32_t* rhR = rhA; const uint32_t* lensR = lensA;
+  const uint32_t* rhC = rhB; const uint32_t* lensC = lensB;
+  if (!(flags & SQ_JOIN_UPPER) && nB >= 4096) {
+    const uint32_t *pa = nullptr, *ra = nullptr, *la_ = nullptr, *pb = nullptr, *rb = nullptr, *lb_ = nullptr;
+    int ok = 0;
+    rc = join_sort_by_length(a, rhA, lensA, rows, &pa, &ra, &la_, &ok);
+    if (rc != SQ_OK) return rc;
+    if (ok) {
+      rc = join_sort_by_length(a, rhB, lensB, nB, &pb, &rb, &lb_, &ok);
+      if (rc != SQ_OK) return rc;
+    }
+    if (ok) { permA = pa; rhR = ra; lensR = la_; permB = pb; rhC = rb; lensC = lb_; }
+  }
   // host work list of row ranges (relative to a_begin); a range whose survivors overflow is halved
   int64_t stack_lo[80], stack_n[80];
   int sp = 0;
@@ -124,8 +288,12 @@ int join_core(sq_ctx* a, const sq_ctx* b, int64_t a_begin, int64_t a_end, int ma
     --sp;
     const int64_t lo = stack_lo[sp], cnt = stack_n[sp];
     SQ_CUDA(a, cudaMemsetAsync(a->dflags + 1, 0, 8, st));
-    rc = sq_bag_filter(a, rhA, lensA, lo, cnt, a_begin, rhB, lensB, nB, max_d, (flags & SQ_JOIN_UPPER) ? 1 : 0,
-                       surv, scap, a->dflags + 1);
+    if (permA)
+      rc = join_filter_ranged(a, rhR, lensR, permA, lo, cnt, a_begin, rhC, lensC, permB, nB, max_d, surv, scap,
+                              a->dflags + 1);
+    else
+      rc = sq_bag_filter(a, rhA, lensA, lo, cnt, a_begin, rhB, lensB, nB, max_d, (flags & SQ_JOIN_UPPER) ? 1 : 0,
+                         surv, scap, a->dflags + 1);
     if (rc != SQ_OK) return rc;
     SQ_CUDA(a, cudaMemcpyAsync(a->pinned, a->dflags + 1, 8, cudaMemcpyDeviceToHost, st));
     SQ_CUDA(a, cudaStreamSynchronize(st));
@@ -191,12 +359,13 @@ int sq_bag_filter(sq_ctx* c, const uint32_t* rhA, const uint32_t* lensA, int64_t
   if (rows <= 0 || nB <= 0) return SQ_OK;
   if ((nB + kJoinThreads - 1) / kJoinThreads > 65535) return SQ_ERR_UNSUPPORTED;
   dim3 grid((unsigned)((rows + kJoinRows - 1) / kJoinRows), (unsigned)((nB + kJoinThreads - 1) / kJoinThreads));
+  const unsigned long long sc = (unsigned long long)scap;
   if (c->alphabet <= 20)
     SQ_TIMED(c, SQ_K_ALLPAIRS, join_filter_kernel<5><<<grid, kJoinThreads, 0, c->stream>>>(
-        rhA, lensA, row0, rows, a_base, rhB, lensB, nB, max_d, upper, surv, (unsigned long long)scap, counter));
+        rhA, lensA, row0, rows, a_base, rhB, lensB, nB, max_d, upper, surv, sc, counter));
   else
     SQ_TIMED(c, SQ_K_ALLPAIRS, join_filter_kernel<8><<<grid, kJoinThreads, 0, c->stream>>>(
-        rhA, lensA, row0, rows, a_base, rhB, lensB, nB, max_d, upper, surv, (unsigned long long)scap, counter));
+        rhA, lensA, row0, rows, a_base, rhB, lensB, nB, max_d, upper, surv, sc, counter));
   SQ_LAUNCH_CHECK(c);
   return SQ_OK;
 }
@@ -207,7 +376,11 @@ size_t sq_join_scratch_bytes(int64_t rows, int64_t n_b, int64_t pair_capacity) {
   return 2 * sq_align_up(cap * 8 + 16) + 2 * sq_align_up(cap * 4 + 16) + sq_sort_scratch_bytes(pair_capacity, 1) +
          sq_align_up(r * 32 + 16) + sq_align_up(r * 4 + 16) + sq_align_up(nb * 32 + 16) + sq_align_up(nb * 4 + 16) +
          2 * sq_align_up(scap * 8 + 16) + sq_align_up(scap * 2 + 16) + sq_sort_scratch_bytes((int64_t)scap, 1) +
-         2 * (sq_align_up(cap * 8 + 16) + sq_align_up(cap * 2 + 16)) + 4096;   // sq_join_host staging
+         2 * (sq_align_up(cap * 8 + 16) + sq_align_up(cap * 2 + 16)) +          // sq_join_host staging
+         2 * sq_align_up(nb * 8 + 16) + 3 * sq_align_up(nb * 4 + 16) + sq_align_up(nb * 32 + 16) +
+         sq_sort_scratch_bytes(n_b, 1) +                                         // columns by length
+         2 * sq_align_up(r * 8 + 16) + 3 * sq_align_up(r * 4 + 16) + sq_align_up(r * 32 + 16) +
+         sq_sort_scratch_bytes(rows, 1) + 4096;                                  // rows by length
 }
 
 extern "C" int64_t sq_batch_size(int64_t n_seqs, uint64_t avail_bytes, uint32_t c, uint32_t l_max) {

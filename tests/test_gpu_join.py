@@ -170,3 +170,18 @@ def test_join_full_size_sampled_rows():
         m = wp[:, 0] == t
         assert np.array_equal(P[lo:hi, 1], wp[m, 1]) and np.array_equal(D[lo:hi], wd[m])
     sa.close(); sb.close()
+
+
+@pytest.mark.parametrize("cfg,n_total,n_a,max_d", [("config2", 7300, 1100, 3), ("config3", 9000, 1500, 2),
+                                                   ("config5", 4400, 150, 15)])
+def test_join_columns_sorted_by_length(cfg, n_total, n_a, max_d):
+    """With >= 4,096 columns the filter walks B in order of length (blocks skip rows whose length is
+    out of reach); the result must not change."""
+    a, b = dg.split(dg.GENERATORS[cfg](n_total, seed=13), n_a)
+    assert b.n >= 4096
+    want_p, want_d = oracle.join_threshold(a.seqs, a.offsets, b.seqs, b.offsets, max_d)
+    assert want_p.shape[0] > 200
+    binding, sa, sb = _two(a, b, want_p.shape[0] + 64)
+    got_p, got_d = _run_join(sa, sb, max_d, want_p.shape[0] + 64)
+    assert np.array_equal(got_p, want_p) and np.array_equal(got_d, want_d)
+    sa.close(); sb.close()
