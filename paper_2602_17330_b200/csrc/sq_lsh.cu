@@ -292,6 +292,17 @@ __device__ int64_t run_end(const uint64_t* __restrict__ k, int64_t at, uint64_t 
   return hi;
 }
 
+// every S entry starts as the row's own sentinel (coalesced); bucket_scan_kernel then scatters bucket
+// ids only into the entries of rows that share a bucket with someone
+__global__ void __launch_bounds__(256)
+s_prefill_kernel(uint32_t* __restrict__ S, int64_t n2, int SW) {
+  const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;     // one uint4 of S
+  const int per_row = SW >> 2;
+  if (t >= n2 * per_row) return;
+  const uint32_t v = 0x80000000u | (uint32_t)(t / per_row);
+  reinterpret_cast<uint4*>(S)[t] = make_uint4(v, v, v, v);
+}
+
 // S layout: [n][SW] uint32, SW = 4 * BW (rows are 16-byte aligned for vector loads).
 // units: (global sorted position of the unit's first row, kept members from there to the end
 // of the bucket); band 0's units go to their own list units0 (they need no compares).
@@ -398,7 +409,9 @@ bucket_scan_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict
     const int size = epos[t] - hpos[t];
     const int m = min(size, cap);
     const bool kept = r < m;
-    S[(int64_t)id * SW + band] = kept ? (uint32_t)hpos[t] : (0x80000000u | id);
+    // (rows outside any shared bucket keep the sentinel 0x80000000 | row written by s_prefill_kernel:
+    // it equals no bucket id and no other row's sentinel)
+    if (kept && m >= 2) S[(int64_t)id * SW + band] = (uint32_t)hpos[t];
     if (kept) {
       raw += (unsigned long long)(m - 1 - r);
       if ((r & 31) == 0 && r + 1 < m) {
@@ -1069,6 +1082,8 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
   uint2* units = reinterpret_cast<uint2*>(kalt);
   uint2* units0 = units + rec / 2 + 1;           // <= n2/2 units of band 0, <= rec/2 in all
   SQ_CUDA(c, cudaMemsetAsync(cnt, 0, (rec + 2) * 4, st));
+  SQ_TIMED(c, SQ_K_SEGMENT, s_prefill_kernel<<<(unsigned)((n2 * (sw / 4) + 255) / 256), 256, 0, st>>>(S, n2, sw));
+  SQ_LAUNCH_CHECK(c);
   {
     dim3 grid((unsigned)((n2 + kBsTile - 1) / kBsTile), (unsigned)bands);
     SQ_TIMED(c, SQ_K_SEGMENT, bucket_scan_kernel<<<grid, kBsThreads, 0, st>>>(
