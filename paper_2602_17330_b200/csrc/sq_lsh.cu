@@ -143,28 +143,6 @@ ext_count_kernel(const uint32_t* __restrict__ rowidx, const uint32_t* __restrict
   ext_cnt[i] = r == 0xFFFFFFFFu ? 0u : row_tot[r];
 }
 
-// delta[r] = (first pair of row r in the caller's buffer) - rowstart[r], rowstart = scan of row_tot
-__global__ void __launch_bounds__(256)
-delta_kernel(const uint32_t* __restrict__ rowstart, const uint32_t* __restrict__ ids0,
-             const uint32_t* __restrict__ ext_off, int64_t n2, uint32_t* __restrict__ delta) {
-  const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (r < n2) delta[r] = ext_off[ids0[r]] - rowstart[r];
-}
-
-// sched[k] for every chunk k whose first position 32k falls into row r (one warp per row)
-__global__ void __launch_bounds__(256)
-sched_fill_kernel(const uint32_t* __restrict__ rowstart, const uint32_t* __restrict__ delta,
-                  int64_t n2, uint4* __restrict__ sched) {
-  const int lane = threadIdx.x & 31;
-  const int64_t r = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  if (r >= n2) return;
-  const uint32_t b = rowstart[r], e = rowstart[r + 1];
-  if (e == b) return;
-  const uint32_t d = delta[r];
-  for (uint32_t k = (b + 31) / 32 + lane; (uint64_t)k * 32 < e; k += 32)
-    sched[k] = make_uint4((uint32_t)r, d, e, 0u);
-}
-
 // ---------------------------------------------------------------------------------------------
 // a5.1  bucket scan
 // ---- a4 fix-up: the sort orders every band by only the top `kb` bytes of the 64-bit key --------
@@ -874,7 +852,8 @@ __global__ void __launch_bounds__(kRsWarps * 32, 6)
 row_sort_kernel(const uint32_t* __restrict__ off, const uint2* __restrict__ loc, int64_t n2, int bands,
                 const uint32_t* __restrict__ ids0, const uint32_t* __restrict__ ext_off,
                 bool do_sort, const uint32_t* __restrict__ inJ, uint2* out,
-                unsigned long long* __restrict__ next_row) {
+                unsigned long long* __restrict__ next_row, const uint32_t* __restrict__ rowstart,
+                uint32_t* __restrict__ delta, uint4* __restrict__ sched) {
   __shared__ __align__(16) uint32_t bins_sh[kRsWarps][kRsBins + kRsBins / 32];
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   // Rows differ by four orders of magnitude in size: persistent warps fetch rows kRsChunk at a
@@ -887,7 +866,18 @@ row_sort_kernel(const uint32_t* __restrict__ off, const uint2* __restrict__ loc,
     const int64_t last = min(n2, (int64_t)first + kRsChunk);
     for (int64_t r = (int64_t)first; r < last; ++r) {
       const uint32_t i = ids0[r];            // external id of internal row r
-      sort_one_row(off, loc, n2, bands, inJ, out, r, i, ext_off[i], do_sort, bins_sh[w], lane);
+      const uint32_t eo = ext_off[i];
+      if (sched) {
+        // the family-ordered chunk schedule of the edit-distance stage (sq_common.cuh): delta[r] =
+        // (first pair of row r in the caller's buffer) - rowstart[r]; sched[k] for every chunk k
+        // whose first position 32k falls into row r
+        const uint32_t b = rowstart[r], e = rowstart[r + 1];
+        const uint32_t d = eo - b;
+        if (lane == 0) delta[r] = d;
+        for (uint32_t k = (b + 31) / 32 + lane; (uint64_t)k * 32 < e; k += 32)
+          sched[k] = make_uint4((uint32_t)r, d, e, 0u);
+      }
+      sort_one_row(off, loc, n2, bands, inJ, out, r, i, eo, do_sort, bins_sh[w], lane);
       __syncwarp();
     }
   }
@@ -1138,23 +1128,17 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
     const unsigned need = (unsigned)((n2 + kRsWarps * kRsChunk - 1) / (kRsWarps * kRsChunk));
     if (g > need) g = need;
     SQ_CUDA(c, cudaMemsetAsync(counters + 6, 0, 8, st));
-    SQ_TIMED(c, SQ_K_ROWSORT, row_sort_kernel<<<g, kRsWarps * 32, 0, st>>>(
-        cnt, loc, n2, bands, vin, ext_off, flags == SQ_LSH_SORTED, tmpJ, reinterpret_cast<uint2*>(pairs_out),
-        counters + 6));
-    SQ_LAUNCH_CHECK(c);
-  }
-  // family-ordered chunk schedule for sq_edit_distance (a hint; skipped if it does not fit)
-  {
+    // family-ordered chunk schedule for sq_edit_distance (a hint; skipped if it does not fit),
+    // written by the row kernel on its way
     const size_t nchunks = ((size_t)uniq + 31) / 32;
     uint4* sched = sq_scratch<uint4>(c, nchunks);
     uint32_t* delta = sq_scratch<uint32_t>(c, (size_t)n2 + 1);
-    if (sched && delta) {
-      SQ_TIMED(c, SQ_K_MISC, delta_kernel<<<(unsigned)((n2 + 255) / 256), 256, 0, st>>>(
-          rowstart, vin, ext_off, n2, delta));
-      SQ_LAUNCH_CHECK(c);
-      SQ_TIMED(c, SQ_K_MISC, sched_fill_kernel<<<(unsigned)((n2 * 32 + 255) / 256), 256, 0, st>>>(
-          rowstart, delta, n2, sched));
-      SQ_LAUNCH_CHECK(c);
+    if (!sched || !delta) { sched = nullptr; delta = nullptr; }
+    SQ_TIMED(c, SQ_K_ROWSORT, row_sort_kernel<<<g, kRsWarps * 32, 0, st>>>(
+        cnt, loc, n2, bands, vin, ext_off, flags == SQ_LSH_SORTED, tmpJ, reinterpret_cast<uint2*>(pairs_out),
+        counters + 6, rowstart, delta, sched));
+    SQ_LAUNCH_CHECK(c);
+    if (sched) {
       c->sched = sched;
       c->sched_rowstart = rowstart;
       c->sched_delta = delta;
