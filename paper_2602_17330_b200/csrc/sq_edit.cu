@@ -117,6 +117,9 @@ edit_pairs_w1_kernel(const uint8_t* __restrict__ packed, int64_t n,
       // byte address of this run's table in shared memory: one multiply-add per column gives the
       // address of Peq[residue], and (Ph << 1) | 1 is one multiply-add as well (both FMA pipe)
       const uint32_t pq = (uint32_t)__cvta_generic_to_shared(peq + (run - rbase) * 33);
+      // 2 and 1 as run-time values (the block has 256 threads): with literals the assembler turns
+      // the multiply-add into a shift-add on the ALU pipe, which is the pipe that bounds this loop
+      const uint32_t two = blockDim.x >> 7, one = blockDim.x >> 8;
       uint32_t Pv = 0xFFFFFFFFu, Mv = 0u;
 #pragma unroll
       for (int wi = 0; wi < WORDS; ++wi) {
@@ -134,7 +137,7 @@ edit_pairs_w1_kernel(const uint8_t* __restrict__ packed, int64_t n,
               const uint32_t Xh = (((Eq & Pv) + Pv) ^ Pv) | Eq;
               uint32_t Ph = Mv | ~(Xh | Pv);
               uint32_t Mh = Pv & Xh;
-              asm("mad.lo.u32 %0, %0, 2, 1;" : "+r"(Ph));
+              asm("mad.lo.u32 %0, %0, %1, %2;" : "+r"(Ph) : "r"(two), "r"(one));
               Mh <<= 1;
               Pv = Mh | ~(Xv | Ph);
               Mv = Ph & Xv;
