@@ -544,7 +544,8 @@ def _edited_families(rng, n_fam, members, L_lo, L_hi, max_edits):
 
 @pytest.mark.parametrize("L_lo,L_hi,max_edits,max_d", [
     (66, 80, 6, 3), (66, 80, 12, 8), (100, 130, 20, 15), (100, 130, 40, 31), (100, 130, 40, 32),
-    (150, 160, 24, 20), (200, 225, 30, 25), (33, 70, 10, 7), (120, 125, 3, 0)])
+    (150, 160, 24, 20), (200, 225, 30, 25), (33, 70, 10, 7), (120, 125, 3, 0), (100, 130, 50, 40), (70, 96, 20, 16),
+    (70, 96, 20, 17)])
 def test_all_pairs_long_thresholded_band(L_lo, L_hi, max_edits, max_d):
     """Distances straddle max_d (edits up to ~1.3 max_d per member), lengths span 2-8 words."""
     rng = np.random.default_rng(L_lo * 1000 + max_d)
