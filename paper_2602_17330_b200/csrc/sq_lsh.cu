@@ -629,7 +629,9 @@ emit_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint32_t* __
 // of the tile and the id of column `lane`; every round each lane with a bit left takes its next
 // column's id from the owning lane (SHFL) and appends it to its row's group.  A unit is a chain
 // of three dependent loads (descriptor -> ids + first mask -> output offset); the warp keeps the
-// chains of its next three units in flight while it works on the current one.
+// chains of its next kFillDepth units in flight while it works on the current one.
+constexpr int kFillDepth = 5;
+
 __global__ void __launch_bounds__(kEmWarps * 32)
 emit_fill_masks_kernel(const uint2* __restrict__ units, uint32_t nunits,
                        const uint32_t* __restrict__ ubase, const uint32_t* __restrict__ masks,
@@ -660,11 +662,19 @@ emit_fill_masks_kernel(const uint2* __restrict__ units, uint32_t nunits,
     }
     return r;
   };
-  L1 a0 = load1(u), a1 = load1(u + nw), a2 = load1(u + 2 * nw);
-  L2 b0 = load2(a0), b1 = load2(a1);
+  // kFillDepth units in flight per warp: descriptors kFillDepth ahead, their ids / masks / offsets
+  // kFillDepth - 1 ahead
+  L1 a[kFillDepth];
+  L2 b[kFillDepth - 1];
+#pragma unroll
+  for (int q = 0; q < kFillDepth; ++q) a[q] = load1(u + q * nw);
+#pragma unroll
+  for (int q = 0; q < kFillDepth - 1; ++q) b[q] = load2(a[q]);
   for (; u < nunits; u += nw) {
-    const L2 b2 = load2(a2);                         // chains of the next units advance one level
-    const L1 a3 = load1(u + 3 * nw);
+    const L2 bn = load2(a[kFillDepth - 1]);          // chains of the next units advance one level
+    const L1 an = load1(u + kFillDepth * nw);
+    const L1 a0 = a[0];
+    const L2 b0 = b[0];
     // ---- the current unit
     const uint32_t g0 = a0.un.x, mrem = a0.un.y;
     const uint32_t* __restrict__ idp = ids + g0;
@@ -689,7 +699,12 @@ emit_fill_masks_kernel(const uint2* __restrict__ units, uint32_t nunits,
       }
       mask = mask_n; idc = idc_n;
     }
-    a0 = a1; a1 = a2; a2 = a3; b0 = b1; b1 = b2;
+#pragma unroll
+    for (int q = 0; q + 1 < kFillDepth; ++q) a[q] = a[q + 1];
+    a[kFillDepth - 1] = an;
+#pragma unroll
+    for (int q = 0; q + 2 < kFillDepth; ++q) b[q] = b[q + 1];
+    b[kFillDepth - 2] = bn;
   }
 }
 
