@@ -726,14 +726,9 @@ constexpr int kRsWarps = 8;
 constexpr int kRsBins = 1024;
 
 __device__ __forceinline__ void
-sort_one_row(const uint32_t* __restrict__ off, const uint2* __restrict__ loc, int64_t n2, int bands,
-             const uint32_t* __restrict__ inJ,
-             uint2* out, int64_t r, uint32_t row, uint32_t obase, bool do_sort, uint32_t* bins,
-             int lane) {
-  // lane b holds group b
-  uint32_t gs = 0, len = 0;
-  if (lane == 0) { gs = off[r]; len = off[r + 1] - gs; }
-  else if (lane < bands) { const uint2 l = loc[(int64_t)lane * n2 + r]; gs = l.x; len = l.y; }
+sort_one_row(const uint32_t* __restrict__ inJ, uint2* out, uint32_t gs, uint32_t len, uint32_t row,
+             uint32_t obase, bool do_sort, uint32_t* bins, int lane) {
+  // lane b holds group b: (gs, len) = its start in inJ and its length (row_group below)
   uint32_t pre = len;                        // inclusive -> exclusive prefix of the group lengths
 #pragma unroll
   for (int d = 1; d < 32; d <<= 1) {
@@ -863,7 +858,7 @@ sort_one_row(const uint32_t* __restrict__ off, const uint2* __restrict__ loc, in
 
 constexpr int kRsChunk = 8;
 
-__global__ void __launch_bounds__(kRsWarps * 32, 6)
+__global__ void __launch_bounds__(kRsWarps * 32, 5)
 row_sort_kernel(const uint32_t* __restrict__ off, const uint2* __restrict__ loc, int64_t n2, int bands,
                 const uint32_t* __restrict__ ids0, const uint32_t* __restrict__ ext_off,
                 bool do_sort, const uint32_t* __restrict__ inJ, uint2* out,
@@ -879,9 +874,27 @@ row_sort_kernel(const uint32_t* __restrict__ off, const uint2* __restrict__ loc,
     first = __shfl_sync(kFull, first, 0);
     if ((int64_t)first >= n2) return;
     const int64_t last = min(n2, (int64_t)first + kRsChunk);
+    // the loads of row r + 1 (its external id one row earlier still) are issued before row r is
+    // worked on: the chain id -> output offset and the group table never stall the sort
+    auto row_group = [&](int64_t r) -> uint2 {           // lane b: group b of row r
+      uint2 g = make_uint2(0u, 0u);
+      if (lane == 0) { g.x = off[r]; g.y = off[r + 1] - g.x; }
+      else if (lane < bands) g = loc[(int64_t)lane * n2 + r];
+      return g;
+    };
+    uint32_t i_c = ids0[first];
+    uint32_t i_n = (int64_t)first + 1 < last ? ids0[first + 1] : 0u;
+    uint2 g_c = row_group((int64_t)first);
+    uint32_t eo_c = ext_off[i_c];
     for (int64_t r = (int64_t)first; r < last; ++r) {
-      const uint32_t i = ids0[r];            // external id of internal row r
-      const uint32_t eo = ext_off[i];
+      const uint32_t i = i_c, eo = eo_c;     // external id of internal row r, its output offset
+      const uint2 g = g_c;
+      if (r + 1 < last) {
+        i_c = i_n;
+        eo_c = ext_off[i_n];
+        g_c = row_group(r + 1);
+        if (r + 2 < last) i_n = ids0[r + 2];
+      }
       if (sched) {
         // the family-ordered chunk schedule of the edit-distance stage (sq_common.cuh): delta[r] =
         // (first pair of row r in the caller's buffer) - rowstart[r]; sched[k] for every chunk k
@@ -892,7 +905,7 @@ row_sort_kernel(const uint32_t* __restrict__ off, const uint2* __restrict__ loc,
         for (uint32_t k = (b + 31) / 32 + lane; (uint64_t)k * 32 < e; k += 32)
           sched[k] = make_uint4((uint32_t)r, d, e, 0u);
       }
-      sort_one_row(off, loc, n2, bands, inJ, out, r, i, eo, do_sort, bins_sh[w], lane);
+      sort_one_row(inJ, out, g.x, g.y, i, eo, do_sort, bins_sh[w], lane);
       __syncwarp();
     }
   }
