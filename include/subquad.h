@@ -110,7 +110,8 @@ int  sq_pack(sq_ctx* ctx, const uint8_t* seqs, const int64_t* offsets, int64_t n
  * g(x): x^=x>>16; x*=0x6A09E667; x^=x>>15; x*=0xBB67AE85; x^=x>>16   (mod 2^32)
  * a_j = g(lo ^ g(2j+1)) | 1,  b_j = g(hi ^ g(2j+2))   (lo/hi = 32-bit halves of seed)
  * sig_out[i][j] = min_p ( a_j * g(x_p) + b_j mod 2^32 );  all 0xFFFFFFFF if len_i < k.
- * sig_out: uint32[n][H] row-major, H a multiple of 32, 32 <= H <= SQ_MAX_H.  Asynchronous. */
+ * sig_out: uint32[n][H] row-major, 32-byte aligned (else SQ_ERR_INVALID_ARG), H a multiple of 32,
+ * 32 <= H <= SQ_MAX_H.  Asynchronous. */
 int  sq_minhash(sq_ctx* ctx, int k, int H, uint64_t seed, uint32_t* sig_out);
 
 /* a3-a5  LSH banding -> capped buckets -> unique candidate pairs (Alg. 1

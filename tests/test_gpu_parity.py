@@ -281,6 +281,10 @@ def test_error_codes():
     with pytest.raises(binding.SubQuadError) as ei:
         sq.minhash(7, 32, SEED)                                  # 5k > 32
     assert ei.value.code == binding.SQ_ERR_INVALID_ARG
+    buf = torch.empty(2 * 32 + 4, dtype=torch.int32, device="cuda")
+    with pytest.raises(binding.SubQuadError) as ei:              # signature rows are written by
+        sq.minhash(2, 32, SEED, sig_out=buf[4:].view(2, 32))     # 32-byte stores: 16-byte offset
+    assert ei.value.code == binding.SQ_ERR_INVALID_ARG
     sig = sq.minhash(2, 32, SEED)
     pairs = torch.empty((8, 2), dtype=torch.int32, device="cuda")
     with pytest.raises(binding.SubQuadError) as ei:
