@@ -71,10 +71,21 @@ edit_pairs_w1_kernel(const uint8_t* __restrict__ packed, int64_t n,
   uint32_t tw[WORDS];
   {
     const uint4* rowB = reinterpret_cast<const uint4*>(packedB + (int64_t)(inrange ? pr.y : 0u) * STRIDE);
+    if (WORDS == 8) {
+      // a CDR3 slot is one 32-byte sector: one 256-bit load (LDG.E.256) instead of two 128-bit ones
 #pragma unroll
-    for (int q = 0; q < WORDS / 4; ++q) {
-      const uint4 v = inrange ? rowB[q] : make_uint4(0, 0, 0, 0);
-      tw[4 * q] = v.x; tw[4 * q + 1] = v.y; tw[4 * q + 2] = v.z; tw[4 * q + 3] = v.w;
+      for (int q = 0; q < WORDS; ++q) tw[q] = 0u;
+      if (inrange)
+        asm("ld.global.nc.v8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+            : "=r"(tw[0]), "=r"(tw[1]), "=r"(tw[2]), "=r"(tw[3]), "=r"(tw[WORDS - 4]), "=r"(tw[WORDS - 3]),
+              "=r"(tw[WORDS - 2]), "=r"(tw[WORDS - 1])
+            : "l"(rowB));
+    } else {
+#pragma unroll
+      for (int q = 0; q < WORDS / 4; ++q) {
+        const uint4 v = inrange ? rowB[q] : make_uint4(0, 0, 0, 0);
+        tw[4 * q] = v.x; tw[4 * q + 1] = v.y; tw[4 * q + 2] = v.z; tw[4 * q + 3] = v.w;
+      }
     }
   }
   // runs of equal i
