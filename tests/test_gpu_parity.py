@@ -87,6 +87,23 @@ def test_minhash_shapes(k, H):
     sq.close()
 
 
+def test_minhash_long_slots_and_single_sequence():
+    """Slots longer than one 32-byte sector (stride 144: the word pipeline of the sketch kernel
+    walks 36 words) and a one-sequence input (every other thread of the block idles)."""
+    binding, sq = _ctx()
+    rep = dg.config5(1_003, seed=5)          # lengths 100-140
+    _pack(sq, binding, rep, op=binding.OP_MINHASH)
+    sig = sq.minhash(4, 64, SEED)
+    assert np.array_equal(_u32(sig), oracle.minhash(rep.seqs, rep.offsets, 4, 64, SEED))
+    sq.close()
+    binding, sq = _ctx()
+    one = dg.config2(1, seed=9)
+    _pack(sq, binding, one, op=binding.OP_MINHASH)
+    sig = sq.minhash(3, 64, SEED)
+    assert np.array_equal(_u32(sig), oracle.minhash(one.seqs, one.offsets, 3, 64, SEED))
+    sq.close()
+
+
 # ---------------------------------------------------------------------------------------------
 # configs 2-4 shapes: minhash -> lsh -> edit distance
 # ---------------------------------------------------------------------------------------------
