@@ -32,7 +32,8 @@ __global__ void edit_pairs_kernel(const uint8_t* __restrict__ packed, int stride
 // Each lane then streams its own text j (one or two 16-byte loads, held in registers) through
 // the Myers/Hyyro column step; the distance is read off the final vertical deltas:
 // D[m][n] = n + popc(Pv) - popc(Mv) over the m pattern bits, so no score is tracked per column.
-constexpr int kEdWarps = 8;
+constexpr int kEdWarps = 2;     // small blocks: a warp's time varies (runs, text lengths, load chain), and a
+                                // block holds its slot until its slowest warp is done (8 -> 2 warps: -5 %)
 constexpr int kEdRuns = 8;      // Peq tables resident per warp
 
 // SCHED: warp k takes positions [32k, 32k+32) of the family-ordered schedule left by
@@ -40,7 +41,7 @@ constexpr int kEdRuns = 8;      // Peq tables resident per warp
 // on rows of the same family, whose partners are the same few sequences -- the text gathers hit
 // L2.  The schedule only permutes the pair indices; every pair is still read from `pairs`.
 template <int STRIDE, bool SCHED>
-__global__ void __launch_bounds__(kEdWarps * 32, 5)
+__global__ void __launch_bounds__(kEdWarps * 32, 40 / kEdWarps)
 edit_pairs_w1_kernel(const uint8_t* __restrict__ packed, int64_t n,
                      const uint8_t* __restrict__ packedB, int64_t nB, const uint2* __restrict__ pairs,
                      int64_t n_pairs, int max_d, uint16_t* __restrict__ dist,
@@ -130,7 +131,7 @@ edit_pairs_w1_kernel(const uint8_t* __restrict__ packed, int64_t n,
       const uint32_t pq = (uint32_t)__cvta_generic_to_shared(peq + (run - rbase) * 33);
       // 2 and 1 as run-time values (the block has 256 threads): with literals the assembler turns
       // the multiply-add into a shift-add on the ALU pipe, which is the pipe that bounds this loop
-      const uint32_t two = blockDim.x >> 7, one = blockDim.x >> 8;
+      const uint32_t two = blockDim.x / (kEdWarps * 16), one = blockDim.x / (kEdWarps * 32);
       uint32_t Pv = 0xFFFFFFFFu, Mv = 0u;
 #pragma unroll
       for (int wi = 0; wi < WORDS; ++wi) {

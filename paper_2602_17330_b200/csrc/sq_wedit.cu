@@ -17,7 +17,7 @@
 
 namespace {
 
-constexpr int kWeWarps = 8;
+constexpr int kWeWarps = 2;
 constexpr int kWeRuns = 4;               // query profiles resident per warp (1 KB each)
 
 // one text column against MR pattern rows; D[x] = D(x+1, y) on entry for column y, updated in place
