@@ -30,8 +30,8 @@ METRIC = "candidate_pairs_verified_per_s"
 UNIT = "pairs/s"
 ALU_OPS_PER_COLUMN_WORD = 7         # ALU-pipe logic ops of one Myers/Hyyro column step
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
-# committed `ncu --set full` capture of this very command line (profiles/r1_v41_top_config4.md)
-NCU_TRAFFIC_BYTES = {("config4", 10_000_000, "edit_distance"): 54.55e9 + 3.50e9}
+# committed `ncu --set full` capture of this very command line (profiles/r1_v42_top_config4.md)
+NCU_TRAFFIC_BYTES = {("config4", 10_000_000, "edit_distance"): 54.67e9 + 3.49e9}
 # bounded oracle samples (first n_s sequences of the same workload)
 ORACLE_SAMPLE = {"config1": 2000, "config2": 100_000, "config3": 300_000, "config4": 300_000}
 CAP_PER_SEQ = {"config2": 40, "config3": 60, "config4": 200}
@@ -526,7 +526,7 @@ def run_ours(args):
     roof["avg_launch_ms"] = kd["ms_per_step"] / max(kd["launches_per_step"], 1)
     roof["traffic"] = NCU_TRAFFIC_BYTES.get((workload, n, dom))
     if roof["traffic"] is not None:
-        roof["traffic_source"] = "profiles/r1_v41_top_config4.md (ncu --set full, bytes per launch)"
+        roof["traffic_source"] = "profiles/r1_v42_top_config4.md (ncu --set full, bytes per launch)"
 
     cpu = None if args.no_cpu_baseline else cpu_baseline(rep, workload, P)
     line = {
