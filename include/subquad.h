@@ -143,7 +143,8 @@ int  sq_edit_distance(sq_ctx* ctx, const uint32_t* pairs, int64_t n_pairs, int m
  * one insertion/deletion cost; boundary D[x][0] = x*indel, D[0][y] = y*indel.
  * sub_cost: DEVICE uint8[alphabet][alphabet] row-major (alphabet = the one given to sq_pack),
  * entry [a][b] = cost of substituting residue a of sequence pairs[p][0] by residue b of sequence
- * pairs[p][1]; the diagonal is normally 0 but is used as given.  1 <= indel <= 255.
+ * pairs[p][1]; Eq. 46 multiplies the cost by the indicator I(a != b), so the table's diagonal is
+ * never read: equal residues cost 0.  1 <= indel <= 255.
  * dist_out[p] = min(d, max_d + 1) for max_d >= 0, else min(d, 65535).  Asynchronous. */
 int  sq_edit_distance_weighted(sq_ctx* ctx, const uint32_t* pairs, int64_t n_pairs,
                                const uint8_t* sub_cost, int indel, int max_d, uint16_t* dist_out);
@@ -236,6 +237,11 @@ int  sq_pipeline_host_csr(sq_ctx* ctx, const uint8_t* seqs_host, const int64_t* 
  * prefix runs that hold several full keys in order, so buckets are always the sets of equal
  * 64-bit keys the spec defines; 8 = a plain sort on the whole key.  SQ_ERR_INVALID_ARG otherwise. */
 #define SQ_OPT_SORT_KEY_BYTES 1
+/* SQ_OPT_SCHED_MIN_BYTES (>= 0, default 96 MiB): sq_edit_distance (and the weighted / graph steps)
+ * visits the pairs sq_lsh_candidates just wrote in the family order of its internal schedule when the
+ * packed sequences exceed this many bytes (they then do not fit the L2); 0 = always, so tests can
+ * force that path on small inputs.  The schedule only permutes the order of the work. */
+#define SQ_OPT_SCHED_MIN_BYTES 2
 int  sq_set_option(sq_ctx* ctx, int option, int64_t value);
 
 /* Introspection (host values, valid after the call they describe). */

@@ -158,7 +158,9 @@ int orc_wagner_fischer_weighted(const uint8_t* a, int la, const uint8_t* b, int 
     for (int y = 1; y <= lb; ++y) {
       int del = prev[y] + indel;
       int ins = cur[y - 1] + indel;
-      int sb = prev[y - 1] + (int)sub[(int)a[x - 1] * sigma + (int)b[y - 1]];
+      /* Eq. 46: I(s_i[x] != s_j[y]) * substitution_cost -- equal residues cost 0, whatever the
+       * table's diagonal holds (reading 22b) */
+      int sb = prev[y - 1] + (a[x - 1] != b[y - 1] ? (int)sub[(int)a[x - 1] * sigma + (int)b[y - 1]] : 0);
       int m = del < ins ? del : ins;
       cur[y] = m < sb ? m : sb;
     }

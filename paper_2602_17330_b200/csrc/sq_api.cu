@@ -141,6 +141,7 @@ size_t sq_workspace_bytes(const sq_ctx*, int op, const sq_sizes* s) {
 int sq_set_option(sq_ctx* c, int option, int64_t value) {
   if (!c) return SQ_ERR_INVALID_ARG;
   if (option == SQ_OPT_SORT_KEY_BYTES && value >= 1 && value <= 8) { c->sort_key_bytes = (int)value; return SQ_OK; }
+  if (option == SQ_OPT_SCHED_MIN_BYTES && value >= 0) { c->sched_min_bytes = value; return SQ_OK; }
   return SQ_ERR_INVALID_ARG;
 }
 

@@ -46,6 +46,7 @@ struct sq_ctx {
   int64_t sched_npairs = 0;
   // tuning (sq_set_option)
   int sort_key_bytes = 4;       // top bytes of the band key the bucket sort orders by (1..8)
+  int64_t sched_min_bytes = (int64_t)96 << 20;   // packed bytes above which the DP follows the schedule
   // bookkeeping
   int64_t launches = 0;
   int64_t last_raw_pairs = 0;

@@ -129,7 +129,7 @@ edit_pairs_w1_kernel(const uint8_t* __restrict__ packed, int64_t n,
       // byte address of this run's table in shared memory: one multiply-add per column gives the
       // address of Peq[residue], and (Ph << 1) | 1 is one multiply-add as well (both FMA pipe)
       const uint32_t pq = (uint32_t)__cvta_generic_to_shared(peq + (run - rbase) * 33);
-      // 2 and 1 as run-time values (the block has 256 threads): with literals the assembler turns
+      // 2 and 1 as run-time values (the block has kEdWarps * 32 threads): with literals the assembler turns
       // the multiply-add into a shift-add on the ALU pipe, which is the pipe that bounds this loop
       const uint32_t two = blockDim.x / (kEdWarps * 16), one = blockDim.x / (kEdWarps * 32);
       uint32_t Pv = 0xFFFFFFFFu, Mv = 0u;
@@ -172,8 +172,10 @@ int launch_edit_w1(sq_ctx* c, const uint8_t* packedB, int64_t nB, const uint32_t
                    int max_d, uint16_t* dist_out) {
   const int64_t per_block = kEdWarps * 32;
   // the schedule pays off only when the packed sequences do not fit the L2 anyway
-  const bool big = (size_t)c->n * (size_t)c->stride > ((size_t)96 << 20);
-  if (packedB == c->packed && big && c->sched && c->sched_pairs == pairs && c->sched_npairs == n_pairs && c->sched_chunks > 0) {
+  const bool big = (size_t)c->n * (size_t)c->stride > (size_t)c->sched_min_bytes;
+  const bool use_sched = packedB == c->packed && big && c->sched && c->sched_pairs == pairs &&
+                         c->sched_npairs == n_pairs && c->sched_chunks > 0;
+  if (use_sched) {
     const int64_t blocks = (c->sched_chunks + kEdWarps - 1) / kEdWarps;
     SQ_TIMED(c, SQ_K_EDIT, edit_pairs_w1_kernel<STRIDE, true><<<(unsigned)blocks, kEdWarps * 32, 0, c->stream>>>(
         c->packed, c->n, c->packed, c->n, reinterpret_cast<const uint2*>(pairs), n_pairs, max_d, dist_out,

@@ -126,7 +126,7 @@ extern "C" int sq_affinity_graph(sq_ctx* c, const uint32_t* pairs, const uint16_
   // the schedule of sq_lsh_candidates lives in the scratch: keep it (and allocate above it) when
   // it describes these very pairs and the signatures do not fit the L2
   bool use_sched = c->sched && c->sched_pairs == pairs && c->sched_npairs == n_pairs &&
-                   min_matches > 0 && (size_t)n * H * 4 > ((size_t)96 << 20);
+                   min_matches > 0 && (size_t)n * H * 4 > (size_t)c->sched_min_bytes;
   const uint4* sched = c->sched; const uint32_t* srow = c->sched_rowstart; const uint32_t* sdel = c->sched_delta;
   const size_t top_before = c->scratch_top;
   uint32_t* keep = nullptr; uint32_t* row_cnt = nullptr; uint32_t* tmp = nullptr;

@@ -903,7 +903,7 @@ row_sort_kernel(const uint32_t* __restrict__ off, const uint2* __restrict__ loc,
         const uint32_t d = eo - b;
         if (lane == 0) delta[r] = d;
         for (uint32_t k = (b + 31) / 32 + lane; (uint64_t)k * 32 < e; k += 32)
-          sched[k] = make_uint4((uint32_t)r, d, e, 0u);
+          sched[k] = make_uint4((uint32_t)r, d, e, b);
       }
       sort_one_row(inJ, out, g.x, g.y, i, eo, do_sort, bins_sh[w], lane);
       __syncwarp();

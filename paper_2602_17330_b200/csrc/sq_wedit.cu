@@ -125,7 +125,7 @@ wedit_short_kernel(const uint8_t* __restrict__ packed, int64_t n, const uint2* _
       const uint32_t m = ir != 0xFFFFFFFFu ? __shfl_sync(0xFFFFFFFFu, ax, STRIDE - 1) : 0u;
       uint8_t* pb = reinterpret_cast<uint8_t*>(prof + r * 256);
       for (int c = 0; c < sigma; ++c)
-        pb[c * 32 + lane] = lane < m ? sub[ax * sigma + c] : (uint8_t)0;
+        pb[c * 32 + lane] = (lane < m && ax != (uint32_t)c) ? sub[ax * sigma + c] : (uint8_t)0;   // Eq. 46: I(a != b) * cost
       if (lane == 0) mlen_sm[w][r] = m;
     }
     __syncwarp();
@@ -157,7 +157,8 @@ wedit_long_kernel(const uint8_t* __restrict__ packed, int stride, int64_t n,
                   int sigma, int indel, int max_d, int max_len, uint16_t* __restrict__ dist) {
   extern __shared__ int col_sm[];           // [max_len][kWlThreads]
   __shared__ uint8_t sub_sm[32 * 32];
-  for (int t = threadIdx.x; t < sigma * sigma; t += kWlThreads) sub_sm[t] = sub[t];
+  // Eq. 46 multiplies the cost by I(a != b): the table's diagonal is never used
+  for (int t = threadIdx.x; t < sigma * sigma; t += kWlThreads) sub_sm[t] = (t / sigma == t % sigma) ? (uint8_t)0 : sub[t];
   __syncthreads();
   const int64_t p = (int64_t)blockIdx.x * kWlThreads + threadIdx.x;
   if (p >= n_pairs) return;
@@ -188,7 +189,7 @@ wedit_long_kernel(const uint8_t* __restrict__ packed, int stride, int64_t n,
 template <int STRIDE>
 int launch_short(sq_ctx* c, const uint32_t* pairs, int64_t n_pairs, const uint8_t* sub, int indel,
                  int max_d, uint16_t* dist_out) {
-  const bool big = (size_t)c->n * (size_t)c->stride > ((size_t)96 << 20);
+  const bool big = (size_t)c->n * (size_t)c->stride > (size_t)c->sched_min_bytes;
   if (big && c->sched && c->sched_pairs == pairs && c->sched_npairs == n_pairs && c->sched_chunks > 0) {
     const int64_t blocks = (c->sched_chunks + kWeWarps - 1) / kWeWarps;
     SQ_TIMED(c, SQ_K_EDIT, wedit_short_kernel<STRIDE, true><<<(unsigned)blocks, kWeWarps * 32, 0, c->stream>>>(

@@ -108,6 +108,78 @@ def test_config4_full_size_sampled():
                    rng=np.random.default_rng(4))
 
 
+def _digest128(pairs_u32):
+    """order-independent 128-bit digest of a pair set (two 64-bit sums of mixed keys, mod 2^64)"""
+    k = (pairs_u32[:, 0].astype(np.uint64) << np.uint64(32)) | pairs_u32[:, 1].astype(np.uint64)
+    with np.errstate(over="ignore"):
+        a = k * np.uint64(0x9E3779B97F4A7C15)
+        a ^= a >> np.uint64(29)
+        b = (k ^ np.uint64(0x6A09E667F3BCC908)) * np.uint64(0xD1B54A32D192ED03)
+        b ^= b >> np.uint64(31)
+        return int(a.sum(dtype=np.uint64)), int(b.sum(dtype=np.uint64))
+
+
+def test_config3_whole_candidate_set_and_every_distance_against_the_oracle():
+    """at config 3 the oracle's sort-based tier (validated against the brute force in
+    tests/test_oracle_lsh.py) still fits: count, raw count, a 128-bit order-independent digest of
+    the pair set, the pair list element by element, and ALL distances."""
+    rep, P, sig, pairs, cnt, dist, raw = _run_full("config3")
+    sig_h = _u32(sig)
+    want_p, want_raw, mism = oracle.lsh_sorted(sig_h, P["bands"], P["rows"], P["cap"])
+    assert mism == 0
+    assert cnt == want_p.shape[0] and raw == want_raw
+    got_p = _u32(pairs[:cnt])
+    assert _digest128(got_p) == _digest128(want_p)
+    assert np.array_equal(got_p, want_p)
+    want_d = oracle.edit_distance_pairs(rep.seqs, rep.offsets, want_p, P["max_d"])
+    assert np.array_equal(dist[:cnt].cpu().numpy().view(np.uint16), want_d)
+
+
+def test_config4_one_million_prefix_whole_set_against_the_oracle():
+    """Config 4's generator (power-law families, caps that bind) at the largest n whose raw pair list
+    the oracle sorts in about a minute: count, raw count, digest, pair list and all distances."""
+    rep, P, sig, pairs, cnt, dist, raw = _run_full("config4", n=1_000_000)
+    want_p, want_raw, mism = oracle.lsh_sorted(_u32(sig), P["bands"], P["rows"], P["cap"])
+    assert mism == 0
+    assert cnt == want_p.shape[0] and raw == want_raw
+    got_p = _u32(pairs[:cnt])
+    assert _digest128(got_p) == _digest128(want_p)
+    assert np.array_equal(got_p, want_p)
+    want_d = oracle.edit_distance_pairs(rep.seqs, rep.offsets, want_p, P["max_d"])
+    assert np.array_equal(dist[:cnt].cpu().numpy().view(np.uint16), want_d)
+
+
+def test_config4_full_size_rewritten_pair_buffer():
+    """At full size the packed sequences exceed the L2 and sq_edit_distance follows the schedule
+    left by sq_lsh_candidates (keyed on the buffer's address and count).  The buffer is overwritten
+    in place with random pairs: the distances must be those of the new pairs (sampled oracle)."""
+    from paper_2602_17330_b200 import binding
+    P = dg.PARAMS["config4"]
+    rep = dg.config4(seed=0)
+    sq = binding.SubQuad(0)
+    max_len, total_len = int(rep.lengths.max()), int(rep.offsets[-1])
+    cap = 165 * rep.n
+    sq.set_workspace(sq.workspace_bytes(binding.OP_LSH, rep.n, total_len, max_len, P["H"], P["bands"], P["cap"], cap))
+    sq.pack(torch.from_numpy(rep.seqs).cuda(), torch.from_numpy(rep.offsets).cuda(), 20, max_len)
+    sig = sq.minhash(P["k"], P["H"], SEED)
+    pairs = torch.empty((cap, 2), dtype=torch.int32, device="cuda")
+    cnt = sq.lsh_candidates(sig, P["bands"], P["rows"], P["cap"], pairs)
+    del sig
+    g = torch.Generator(device="cuda"); g.manual_seed(5)
+    pairs[:cnt] = torch.randint(0, rep.n, (cnt, 2), device="cuda", dtype=torch.int32, generator=g)
+    dist = torch.full((cnt,), 0x5A5A, dtype=torch.int16, device="cuda")
+    sq.edit_distance(pairs, cnt, P["max_d"], dist)
+    torch.cuda.synchronize()
+    assert int((dist.to(torch.int32) & 0xFFFF).max()) <= P["max_d"] + 1       # no slot left unwritten
+    rng = np.random.default_rng(6)
+    take = np.sort(rng.choice(cnt, 1_000_000, replace=False))
+    tk = torch.from_numpy(take).cuda()
+    pl = _u32(pairs[tk])
+    assert np.array_equal(dist[tk].cpu().numpy().view(np.uint16),
+                          oracle.edit_distance_pairs(rep.seqs, rep.offsets, pl, P["max_d"]))
+    sq.close()
+
+
 def test_config4_unordered_has_the_same_count_and_set_digest():
     # SQ_LSH_UNORDERED must give the same SET: compare the count and an order-independent digest
     rep, P, sig, pairs, cnt, dist, raw = _run_full("config4", n=2_000_000)

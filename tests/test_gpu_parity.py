@@ -397,6 +397,98 @@ def test_weighted_edit_distance_long_and_tiny_sequences():
     sq.close()
 
 
+def test_weighted_table_diagonal_is_never_used():
+    """PAPER.md L754 Eq. 46: the cost is multiplied by I(a != b) -- a table with a NON-ZERO diagonal
+    gives the distances of the same table with a zero diagonal (reading 22b); short
+    (profile kernel) and long (general kernel) sequences."""
+    binding, sq = _ctx()
+    rng = np.random.default_rng(17)
+    cost = rng.integers(1, 9, (20, 20)).astype(np.uint8)          # diagonal 1..8
+    for rep in (dg.config2(6_007, seed=9), dg.config5(400, seed=4)):
+        _pack(sq, binding, rep, op=binding.OP_EDIT_DISTANCE)
+        ii = np.repeat(rng.integers(0, rep.n, 500), rng.integers(1, 40, 500))
+        pl = np.stack([ii, rng.integers(0, rep.n, ii.size)], 1).astype(np.uint32)
+        pl[::7, 1] = pl[::7, 0]                                   # i == j: all matches, distance 0
+        pt = torch.from_numpy(pl.view(np.int32)).cuda()
+        for indel, md in ((1, -1), (2, 6)):
+            want = oracle.edit_distance_weighted_pairs(rep.seqs, rep.offsets, pl, cost, indel, md)
+            d = sq.edit_distance_weighted(pt, pl.shape[0], torch.from_numpy(cost).cuda(), indel, md)
+            assert np.array_equal(_u16(d)[:pl.shape[0]], want)
+            assert (want[::7] == 0).all()
+    sq.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# the family-ordered schedule of the DP stages, forced on small inputs (SQ_OPT_SCHED_MIN_BYTES = 0)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cfg,n,flags", [("config2", 30_011, 0), ("config2", 30_011, 1), ("config4", 60_013, 0),
+                                         ("config3", 40_009, 0)])
+def test_schedule_forced_edit_weighted_graph(cfg, n, flags):
+    """With the schedule forced, sq_edit_distance / sq_edit_distance_weighted / sq_affinity_graph walk
+    the pairs in the internal family order (chunk schedule, rows of every size, empty rows, chunks that
+    cross rows): every distance and the whole graph still equal the oracle, bit for bit."""
+    binding, sq = _ctx()
+    P = dict(dg.PARAMS[cfg])
+    rep = dg.GENERATORS[cfg](n, seed=31)
+    cap = (160 if cfg == "config4" else 90) * n
+    max_len = int(rep.lengths.max())
+    ws = max(sq.workspace_bytes(binding.OP_LSH, rep.n, int(rep.offsets[-1]), max_len, P["H"], P["bands"], P["cap"], cap),
+             sq.workspace_bytes(binding.OP_GRAPH, rep.n, 0, max_len, 0, 0, 0, cap)) + 4 * cap + 8 * n
+    sq.set_workspace(ws)
+    sq.set_option(binding.OPT_SCHED_MIN_BYTES, 0)
+    sq.pack(torch.from_numpy(rep.seqs).cuda(), torch.from_numpy(rep.offsets).cuda(), 20, max_len)
+    sig = sq.minhash(P["k"], P["H"], SEED)
+    pairs = torch.empty((cap, 2), dtype=torch.int32, device="cuda")
+    cnt = sq.lsh_candidates(sig, P["bands"], P["rows"], P["cap"], pairs, flags=flags)
+    hp = _u32(pairs)[:cnt].copy()
+    dist = torch.full((cnt,), 0x5A5A, dtype=torch.int16, device="cuda")      # an unwritten slot would show
+    sq.edit_distance(pairs, cnt, P["max_d"], dist)
+    want = oracle.edit_distance_pairs(rep.seqs, rep.offsets, hp, P["max_d"])
+    assert np.array_equal(_u16(dist), want)
+    cost = dg.class_substitution_costs()
+    wd = torch.full((cnt,), 0x5A5A, dtype=torch.int16, device="cuda")
+    sq.edit_distance_weighted(pairs, cnt, torch.from_numpy(cost).cuda(), 1, 5, wd)
+    assert np.array_equal(_u16(wd), oracle.edit_distance_weighted_pairs(rep.seqs, rep.offsets, hp, cost, 1, 5))
+    if flags == 0:
+        mm = int(np.ceil(0.7 * P["H"]))
+        row_ptr = torch.empty(rep.n + 1, dtype=torch.int64, device="cuda")
+        col = torch.empty(cnt, dtype=torch.int32, device="cuda")
+        wgt = torch.empty(cnt, dtype=torch.float32, device="cuda")
+        e = sq.affinity_graph(pairs, dist, cnt, P["max_d"], sig, mm, row_ptr, col, wgt)
+        rp, wc, ww = oracle.affinity_graph(hp, want, P["max_d"], _u32(sig), mm, rep.lengths, rep.n)
+        assert e == rp[-1] and np.array_equal(row_ptr.cpu().numpy(), rp)
+        assert np.array_equal(_u32(col)[:e], wc)
+        assert np.allclose(wgt.cpu().numpy()[:e], ww, rtol=0, atol=1.5e-7)
+    sq.close()
+
+
+def test_schedule_hint_survives_an_in_place_rewrite_of_the_pair_buffer():
+    """The schedule hint is keyed on the pair buffer's address and count.  It only permutes the ORDER
+    in which pairs are visited -- every pair is read from the caller's buffer -- so after the caller
+    overwrites that very buffer (same pointer, same count) with arbitrary pairs, the distances are
+    those of the NEW pairs."""
+    binding, sq = _ctx()
+    P = dict(dg.PARAMS["config2"])
+    rep = dg.config2(40_009, seed=33)
+    cap = 60 * rep.n
+    _pack(sq, binding, rep, bands=P["bands"], cap=P["cap"], pair_capacity=cap, H=P["H"])
+    sq.set_option(binding.OPT_SCHED_MIN_BYTES, 0)
+    sig = sq.minhash(P["k"], P["H"], SEED)
+    pairs = torch.empty((cap, 2), dtype=torch.int32, device="cuda")
+    cnt = sq.lsh_candidates(sig, P["bands"], P["rows"], P["cap"], pairs)
+    rng = np.random.default_rng(34)
+    newp = rng.integers(0, rep.n, (cnt, 2)).astype(np.uint32)
+    newp[::11, 0] = rep.n + 5                                      # out-of-range index -> 0xFFFF
+    pairs[:cnt].copy_(torch.from_numpy(newp.view(np.int32)).cuda())
+    dist = torch.full((cnt,), 0x5A5A, dtype=torch.int16, device="cuda")
+    sq.edit_distance(pairs, cnt, P["max_d"], dist)
+    ok = newp[:, 0] < rep.n
+    want = np.full(cnt, 0xFFFF, np.uint16)
+    want[ok] = oracle.edit_distance_pairs(rep.seqs, rep.offsets, newp[ok], P["max_d"])
+    assert np.array_equal(_u16(dist), want)
+    sq.close()
+
+
 # ---------------------------------------------------------------------------------------------
 # next-2: verified candidates -> sparse similarity graph
 # ---------------------------------------------------------------------------------------------

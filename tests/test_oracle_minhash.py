@@ -68,6 +68,48 @@ def test_hash_params_odd_multipliers_and_seed_dependence():
     assert (a64 == a[:64]).all() and (b64 == b[:64]).all()
 
 
+def test_hash_params_hand_worked_values():
+    """a_j = g(lo ^ g(2j+1)) | 1, b_j = g(hi ^ g(2j+2)) with lo / hi the low /
+    high 32 bits of the seed.  Three (seed, j) cases worked step by step from the text of C2 --
+    every intermediate of the mixer is a literal below, so the chain can be checked with a hex
+    calculator; nothing here calls the oracle except the final comparison.  A wrong index
+    (2j for 2j+1), swapped seed halves or a dropped `| 1` changes the literals."""
+    def g_steps(x):                      # C2's mixer, one line per statement
+        s = [x]
+        x ^= x >> 16; s.append(x)
+        x = (x * 0x6A09E667) & M32; s.append(x)
+        x ^= x >> 15; s.append(x)
+        x = (x * 0xBB67AE85) & M32; s.append(x)
+        x ^= x >> 16; s.append(x)
+        return s
+    # g(1) and g(2): the inner values of j = 0
+    assert g_steps(1) == [0x1, 0x1, 0x6A09E667, 0x6A093274, 0x5FBE0E44, 0x5FBE51FA]
+    assert g_steps(2) == [0x2, 0x2, 0xD413CCCE, 0xD41264E9, 0x7AE3CB0D, 0x7AE3B1EE]
+    # seed = 0, j = 0: a_0 = g(0 ^ g(1)) | 1 (the mixer ends on an even value here, so the `| 1`
+    # is visible), b_0 = g(0 ^ g(2))
+    assert g_steps(0x5FBE51FA) == [0x5FBE51FA, 0x5FBE0E44, 0xEEACD55C, 0xEEAD0805, 0x7C5B9099, 0x7C5BECC2]
+    assert g_steps(0x7AE3B1EE) == [0x7AE3B1EE, 0x7AE3CB0D, 0x9F89603B, 0x9F885F29, 0xCF064E4D, 0xCF06814B]
+    a, b = oracle.hash_params(0, 1)
+    assert (int(a[0]), int(b[0])) == (0x7C5BECC3, 0xCF06814B)
+    # the default seed 0x5EED5EED12345678: lo = 0x12345678 feeds a, hi = 0x5EED5EED feeds b
+    assert 0x12345678 ^ 0x5FBE51FA == 0x4D8A0782 and 0x5EED5EED ^ 0x7AE3B1EE == 0x240EEF03
+    assert g_steps(0x4D8A0782) == [0x4D8A0782, 0x4D8A4A08, 0x5B6EF938, 0x5B6E4FE5, 0xE6C027F9, 0xE6C0C139]
+    assert g_steps(0x240EEF03) == [0x240EEF03, 0x240ECB0D, 0x51D6603B, 0x51D6C397, 0x7C453F73, 0x7C454336]
+    a, b = oracle.hash_params(SEED, 8)
+    assert SEED == 0x5EED5EED12345678
+    assert (int(a[0]), int(b[0])) == (0xE6C0C139, 0x7C454336)
+    # j = 5: inner arguments 2j+1 = 11 and 2j+2 = 12
+    assert g_steps(11)[-1] == 0x19F58E71 and g_steps(12)[-1] == 0xFED0F94D
+    assert g_steps(0x12345678 ^ 0x19F58E71)[-1] | 1 == 0x93F264E5
+    assert g_steps(0x5EED5EED ^ 0xFED0F94D)[-1] == 0x55392642
+    assert (int(a[5]), int(b[5])) == (0x93F264E5, 0x55392642)
+    # lo = 0, hi = 1, j = 3: only b sees the seed
+    a, b = oracle.hash_params(1 << 32, 4)
+    assert g_steps(7)[-1] == 0x4E71C736 and g_steps(8)[-1] == 0x797CF042
+    assert (int(a[3]), int(b[3])) == (g_steps(0x4E71C736)[-1] | 1, g_steps(1 ^ 0x797CF042)[-1])
+    assert (int(a[3]), int(b[3])) == (0x6DDCADAF, 0xB0C239BA)
+
+
 def test_closed_form_single_kmer():
     # poly-A: the only k-mer is x = 0 and g(0) = 0, so sig[j] = a_j*0 + b_j = b_j
     _, b = oracle.hash_params(SEED, 64)

@@ -115,3 +115,25 @@ def test_pairs_entry_point_saturates_like_the_unit_cost_one():
         assert np.array_equal(got, np.minimum(exact, md + 1))
     one = oracle.edit_distance_weighted(rep.seq(int(pairs[7, 0])), rep.seq(int(pairs[7, 1])), c, 1)
     assert exact[7] == one
+
+
+def test_equal_residues_cost_nothing_whatever_the_diagonal_says():
+    """PAPER.md L754 Eq. 46 prints  d[x-1][y-1] + I(s_i[x] != s_j[y]) * substitution_cost : the
+    indicator makes a match free, so the table's DIAGONAL is never used (reading 22b)."""
+    rng = np.random.default_rng(7)
+    sigma = 5
+    for _ in range(300):
+        cost = rng.integers(1, 6, (sigma, sigma)).astype(np.uint8)         # non-zero diagonal
+        zero = cost.copy()
+        np.fill_diagonal(zero, 0)
+        a = rng.integers(0, sigma, rng.integers(0, 9))
+        b = rng.integers(0, sigma, rng.integers(0, 9))
+        indel = int(rng.integers(1, 4))
+        assert oracle.edit_distance_weighted(a, b, cost, indel) == oracle.edit_distance_weighted(a, b, zero, indel)
+        assert oracle.edit_distance_weighted(a, a, cost, indel) == 0       # d(s, s) = 0: every step a match
+    # hand-worked: a = [0, 1], b = [0, 2], cost[1][2] = 4, indel = 3, diagonal = 5 everywhere.
+    # Align 0-0 (match: 0, not cost[0][0] = 5) and 1-2 (substitution: 4)  =>  4; the alternative
+    # delete + insert costs 6.
+    cost = np.full((3, 3), 5, np.uint8)
+    cost[1, 2] = 4
+    assert oracle.edit_distance_weighted([0, 1], [0, 2], cost, 3) == 4
