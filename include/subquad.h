@@ -41,7 +41,7 @@ extern "C" {
 #define SQ_ERR_NOT_PACKED    -3   /* an op that needs the packed sequences ran before sq_pack */
 #define SQ_ERR_CAPACITY      -4   /* output did not fit; required count returned             */
 #define SQ_ERR_WORKSPACE     -5   /* workspace missing or too small                          */
-#define SQ_ERR_UNSUPPORTED   -6   /* sequence longer than SQ_MAX_LEN, H > SQ_MAX_H, ...      */
+#define SQ_ERR_UNSUPPORTED   -6   /* sequence longer than max_len / SQ_MAX_LEN, H > SQ_MAX_H, ... */
 #define SQ_ERR_CUDA          -7   /* a CUDA runtime call failed; see sq_last_cuda_error      */
 
 #define SQ_MAX_LEN    240   /* longest sequence the packed layout and the DP kernels accept   */
@@ -95,8 +95,10 @@ int  sq_set_workspace(sq_ctx* ctx, void* dev_ptr, size_t bytes);
 
 /* a1  Pack (App. F.2 "contiguous memory blocks with proper alignment";
  * L157 "trim/pad").  seqs = uint8 residue codes, concatenated; offsets = int64[n+1], sequence
- * i is seqs[offsets[i]..offsets[i+1]).  Validates every code < alphabet (<= 32) and every
- * length <= max_len (<= SQ_MAX_LEN); writes the internal layout into the workspace: one
+ * i is seqs[offsets[i]..offsets[i+1]); offsets[n] is the size of `seqs`.  Validates every code <
+ * alphabet (<= 32, else SQ_ERR_BAD_RESIDUE), every length <= max_len (<= SQ_MAX_LEN, else
+ * SQ_ERR_UNSUPPORTED) and the offsets themselves (offsets[0] >= 0, non-decreasing, none beyond
+ * offsets[n]; else SQ_ERR_INVALID_ARG -- nothing outside [0, offsets[n]) is ever read); writes the internal layout into the workspace: one
  * fixed-stride slot per sequence, stride = round_up(max_len + 1, 16) bytes, residues at
  * [0, len), 0xFF padding, the length in the slot's last byte -- so a slot is read with
  * aligned 16-byte vector loads and a CDR3 (len <= 31) is exactly one 32-byte sector.

@@ -196,6 +196,7 @@ size_t sq_allpairs_scratch_bytes(int64_t n, int64_t pair_capacity) {
 extern "C" int sq_all_pairs(sq_ctx* c, int max_d, uint32_t* pairs_out, uint16_t* dist_out,
                             int64_t capacity, int64_t* n_out) {
   if (!c || !n_out) return SQ_ERR_INVALID_ARG;
+  SqDeviceGuard guard(c);
   *n_out = 0;
   if (c->n < 0) return SQ_ERR_NOT_PACKED;
   const int64_t n = c->n;

@@ -21,12 +21,19 @@ int sq_create(sq_ctx** out, int device, void* cuda_stream) {
     delete c;
     return SQ_ERR_CUDA;
   }
+  // second stream of the *_host entry points (device->host copies beside the compute stream)
+  if (cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) != cudaSuccess) {
+    cudaFreeHost(c->pinned);
+    delete c;
+    return SQ_ERR_CUDA;
+  }
   *out = c;
   return SQ_OK;
 }
 
 void sq_destroy(sq_ctx* c) {
   if (!c) return;
+  SqDeviceGuard guard(c);
   if (c->prof_ev) {
     for (int i = 0; i < 2 * kSqProfSlots; ++i) cudaEventDestroy(c->prof_ev[i]);
     delete[] c->prof_ev;
@@ -53,6 +60,7 @@ int sq_set_workspace(sq_ctx* c, void* dev_ptr, size_t bytes) {
 
 int sq_profile_enable(sq_ctx* c, int on) {
   if (!c) return SQ_ERR_INVALID_ARG;
+  SqDeviceGuard guard(c);
   if (on && !c->prof_ev) {
     c->prof_ev = new (std::nothrow) cudaEvent_t[2 * kSqProfSlots];
     if (!c->prof_ev) return SQ_ERR_INVALID_ARG;
@@ -65,6 +73,7 @@ int sq_profile_enable(sq_ctx* c, int on) {
 
 int sq_profile_reset(sq_ctx* c) {
   if (!c) return SQ_ERR_INVALID_ARG;
+  SqDeviceGuard guard(c);
   sq_prof_drain(c);
   for (int k = 0; k < SQ_K_COUNT; ++k) { c->prof_ms[k] = 0.0; c->prof_launches[k] = 0; }
   return SQ_OK;
@@ -72,6 +81,7 @@ int sq_profile_reset(sq_ctx* c) {
 
 int sq_profile_read(sq_ctx* c, int cls, double* ms, int64_t* launches) {
   if (!c || cls < 0 || cls >= SQ_K_COUNT || !ms || !launches) return SQ_ERR_INVALID_ARG;
+  SqDeviceGuard guard(c);
   sq_prof_drain(c);
   *ms = c->prof_ms[cls];
   *launches = c->prof_launches[cls];
@@ -97,11 +107,11 @@ const char* sq_strerror(int code) {
   switch (code) {
     case SQ_OK: return "ok";
     case SQ_ERR_INVALID_ARG: return "invalid argument";
-    case SQ_ERR_BAD_RESIDUE: return "residue code >= alphabet, or sequence longer than max_len";
+    case SQ_ERR_BAD_RESIDUE: return "residue code >= alphabet";
     case SQ_ERR_NOT_PACKED: return "sq_pack has not been called on this workspace";
     case SQ_ERR_CAPACITY: return "output capacity too small (required count returned)";
     case SQ_ERR_WORKSPACE: return "workspace missing or too small";
-    case SQ_ERR_UNSUPPORTED: return "unsupported size (sequence length, H or bands over the compiled maximum)";
+    case SQ_ERR_UNSUPPORTED: return "unsupported size (sequence longer than max_len, or length, H or bands over the compiled maximum)";
     case SQ_ERR_CUDA: return "CUDA runtime error";
     default: return "unknown error";
   }
@@ -147,12 +157,14 @@ int sq_set_option(sq_ctx* c, int option, int64_t value) {
 
 int sq_minhash(sq_ctx* c, int k, int H, uint64_t seed, uint32_t* sig_out) {
   if (!c) return SQ_ERR_INVALID_ARG;
+  SqDeviceGuard guard(c);
   return sq_minhash_impl(c, k, H, seed, sig_out);
 }
 
 int sq_edit_distance(sq_ctx* c, const uint32_t* pairs, int64_t n_pairs, int max_d,
                      uint16_t* dist_out) {
   if (!c) return SQ_ERR_INVALID_ARG;
+  SqDeviceGuard guard(c);
   return sq_edit_distance_impl(c, pairs, n_pairs, max_d, dist_out);
 }
 
@@ -164,11 +176,18 @@ static int pipeline_host_impl(sq_ctx* c, const uint8_t* seqs_host, const int64_t
                               int64_t capacity, int64_t* n_pairs) {
   const bool csr = row_ptr_host != nullptr;
   if (!c || !offsets_host || !n_pairs || n < 0 || capacity < 0) return SQ_ERR_INVALID_ARG;
+  SqDeviceGuard guard(c);
+  *n_pairs = 0;
+  // everything the carving of the I/O region depends on is checked before it is used
+  if (H < 1 || k < 1 || bands < 1 || rows < 1 || bucket_cap < 1 || alphabet < 1 || alphabet > 32)
+    return SQ_ERR_INVALID_ARG;
+  if (H > SQ_MAX_H || bands > SQ_MAX_BANDS) return SQ_ERR_UNSUPPORTED;
   if (!c->ws) return SQ_ERR_WORKSPACE;
   if (max_len < 0 || max_len > SQ_MAX_LEN) return SQ_ERR_UNSUPPORTED;
   if (csr && (max_d < 0 || max_d > 254)) return SQ_ERR_UNSUPPORTED;      // min(d, max_d+1) in a byte
-  *n_pairs = 0;
-  int64_t total = offsets_host[n];
+  const int64_t total = offsets_host[n];
+  if (total < 0 || offsets_host[0] != 0 || (total > 0 && !seqs_host)) return SQ_ERR_INVALID_ARG;
+  if (capacity > 0 && !csr && (!pairs_out_host || !dist_out_host)) return SQ_ERR_INVALID_ARG;
   // Device I/O buffers sit at the END of the workspace so that sq_pack's persistent region
   // and the per-op scratch (both allocated from the front) cannot overlap them.
   size_t io = sq_align_up((size_t)total + 16) + sq_align_up((size_t)(n + 1) * 8 + 16) +
@@ -204,11 +223,7 @@ static int pipeline_host_impl(sq_ctx* c, const uint8_t* seqs_host, const int64_t
     if ((rc = sq_lsh_candidates(c, d_sig, H, bands, rows, bucket_cap, SQ_LSH_SORTED, d_pairs,
                                 capacity, n_pairs)) != SQ_OK) break;
     // sq_lsh_candidates has synchronised: the pairs are final.  Their copy to the host (the bulk
-    // of the output) runs on a second stream while the DP kernel works on the first.
-    if (!c->copy_stream &&
-        cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) != cudaSuccess) {
-      rc = SQ_ERR_CUDA; break;
-    }
+    // of the output) runs on the context's second stream while the DP kernel works on the first.
     const int64_t np = *n_pairs;
     if (!csr) {
       if (np > 0 &&
@@ -255,6 +270,11 @@ static int pipeline_host_impl(sq_ctx* c, const uint8_t* seqs_host, const int64_t
     if (cudaStreamSynchronize(c->stream) != cudaSuccess) { rc = SQ_ERR_CUDA; break; }
   } while (0);
   if (rc == SQ_ERR_CUDA) c->last_err = cudaGetLastError();
+  if (rc != SQ_OK) {
+    // nothing may still be writing the caller's host buffers once an error is returned
+    cudaStreamSynchronize(c->copy_stream);
+    cudaStreamSynchronize(c->stream);
+  }
   c->ws_bytes = saved;
   return rc;
 }

@@ -64,6 +64,18 @@ struct sq_ctx {
 
 void sq_prof_drain(sq_ctx* c);           // synchronises the pending events into prof_ms
 
+// RAII: every extern "C" entry point runs with the context's device current and puts the caller's
+// device back on return, so contexts of several devices can live in one process
+struct SqDeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  explicit SqDeviceGuard(const sq_ctx* c) {
+    if (!c) return;
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != c->device) switched = cudaSetDevice(c->device) == cudaSuccess;
+  }
+  ~SqDeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
+
 // RAII: times everything enqueued on the context's stream during its lifetime as one launch
 struct SqProfScope {
   sq_ctx* c; int slot;

@@ -115,6 +115,7 @@ extern "C" int sq_affinity_graph(sq_ctx* c, const uint32_t* pairs, const uint16_
                                  int64_t* row_ptr, uint32_t* col, float* weight, int64_t capacity,
                                  int64_t* n_edges) {
   if (!c || !n_edges || !row_ptr) return SQ_ERR_INVALID_ARG;
+  SqDeviceGuard guard(c);
   *n_edges = 0;
   if (c->n < 0) return SQ_ERR_NOT_PACKED;
   if (n_pairs < 0 || capacity < 0 || max_d < 0 || min_matches < 0) return SQ_ERR_INVALID_ARG;

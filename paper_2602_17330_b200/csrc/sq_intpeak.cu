@@ -42,11 +42,16 @@ int_peak_kernel(int iters, uint32_t seed, uint32_t* __restrict__ sink) {
 extern "C" int sq_int_peak(sq_ctx* c, int kind, int iters, double* ops_per_s) {
   if (!c || !ops_per_s || iters < 1 || kind < 0 || kind > 6) return SQ_ERR_INVALID_ARG;
   if (!c->ws) return SQ_ERR_WORKSPACE;
-  uint32_t* sink = reinterpret_cast<uint32_t*>(c->ws + 128);
+  SqDeviceGuard guard(c);
+  // 256 words of the free scratch (handed back at once: the kernels practically never write them)
+  const size_t top = c->scratch_top;
+  uint32_t* sink = sq_scratch<uint32_t>(c, 256);
+  c->scratch_top = top;
+  if (!sink) return SQ_ERR_WORKSPACE;
   const int blocks = c->sm_count * 8;
   cudaEvent_t e0, e1;
   SQ_CUDA(c, cudaEventCreate(&e0));
-  SQ_CUDA(c, cudaEventCreate(&e1));
+  if (cudaEventCreate(&e1) != cudaSuccess) { c->last_err = cudaGetLastError(); cudaEventDestroy(e0); return SQ_ERR_CUDA; }
   float best = 1e30f;
   for (int rep = 0; rep < 4; ++rep) {
     cudaEventRecord(e0, c->stream);
@@ -61,7 +66,11 @@ extern "C" int sq_int_peak(sq_ctx* c, int kind, int iters, double* ops_per_s) {
     }
     c->launches++;
     cudaEventRecord(e1, c->stream);
-    if (cudaEventSynchronize(e1) != cudaSuccess) { c->last_err = cudaGetLastError(); return SQ_ERR_CUDA; }
+    if (cudaEventSynchronize(e1) != cudaSuccess) {
+      c->last_err = cudaGetLastError();
+      cudaEventDestroy(e0); cudaEventDestroy(e1);
+      return SQ_ERR_CUDA;
+    }
     float ms = 0.f;
     cudaEventElapsedTime(&ms, e0, e1);
     if (rep > 0 && ms < best) best = ms;

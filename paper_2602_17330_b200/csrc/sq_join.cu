@@ -402,6 +402,7 @@ extern "C" int sq_join(sq_ctx* a, const sq_ctx* b, int64_t a_begin, int64_t a_en
   *n_out = 0;
   int rc = join_check(a, b, max_d);
   if (rc != SQ_OK) return rc;
+  SqDeviceGuard guard(a);
   if (a_begin < 0 || a_end < a_begin || a_end > a->n || capacity < 0) return SQ_ERR_INVALID_ARG;
   if (capacity > 0 && (!pairs_out || !dist_out)) return SQ_ERR_INVALID_ARG;
   if (max_d > 65534) max_d = 65534;
@@ -416,6 +417,7 @@ extern "C" int sq_join_host(sq_ctx* a, const sq_ctx* b, int max_d, int flags, in
   *n_out = 0;
   int rc = join_check(a, b, max_d);
   if (rc != SQ_OK) return rc;
+  SqDeviceGuard guard(a);
   if (capacity < 0 || block_capacity < 1) return SQ_ERR_INVALID_ARG;
   if (capacity > 0 && (!pairs_host || !dist_host)) return SQ_ERR_INVALID_ARG;
   if (max_d > 65534) max_d = 65534;

@@ -1008,6 +1008,7 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
                                  int bucket_cap, int flags, uint32_t* pairs_out, int64_t capacity,
                                  int64_t* n_pairs) {
   if (!c || !n_pairs) return SQ_ERR_INVALID_ARG;
+  SqDeviceGuard guard(c);
   *n_pairs = 0;
   if (c->n < 0) return SQ_ERR_NOT_PACKED;
   if (H < 1 || bands < 1 || rows < 1 || bucket_cap < 1 || capacity < 0 ||

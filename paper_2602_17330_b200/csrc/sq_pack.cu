@@ -37,7 +37,10 @@ pack_kernel(const uint8_t* __restrict__ seqs, const int64_t* __restrict__ off, i
     const int c = (int)(t - i * chunks);
     const int64_t beg = off[i];
     int64_t len64 = off[i + 1] - beg;
-    if (len64 < 0 || len64 > max_len) { bad |= 2u; len64 = 0; }
+    // offsets must start at >= 0, never decrease and stay inside [0, offsets[n]] (the caller's
+    // statement of the size of `seqs`): anything else would read outside the buffer
+    if (beg < 0 || len64 < 0 || off[i + 1] > off[n]) { bad |= 4u; len64 = 0; }
+    else if (len64 > max_len) { bad |= 2u; len64 = 0; }
     const int len = (int)len64;
     uint32_t w[4];
 #pragma unroll
@@ -73,6 +76,7 @@ extern "C" int sq_pack(sq_ctx* c, const uint8_t* seqs, const int64_t* offsets, i
   if (n >= (1ll << 31)) return SQ_ERR_UNSUPPORTED;
   if (max_len > SQ_MAX_LEN) return SQ_ERR_UNSUPPORTED;
   if (!c->ws) return SQ_ERR_WORKSPACE;
+  SqDeviceGuard guard(c);
   c->n = -1;
   c->sched = nullptr;
   const int stride = sq_stride_for(max_len);
@@ -109,7 +113,9 @@ extern "C" int sq_pack(sq_ctx* c, const uint8_t* seqs, const int64_t* offsets, i
   }
   SQ_CUDA(c, cudaMemcpyAsync(c->pinned, c->dflags, 8, cudaMemcpyDeviceToHost, c->stream));
   SQ_CUDA(c, cudaStreamSynchronize(c->stream));
-  if (c->pinned[0] & 3ull) return SQ_ERR_BAD_RESIDUE;
+  if (c->pinned[0] & 4ull) return SQ_ERR_INVALID_ARG;       // malformed offsets
+  if (c->pinned[0] & 2ull) return SQ_ERR_UNSUPPORTED;       // a sequence longer than max_len
+  if (c->pinned[0] & 1ull) return SQ_ERR_BAD_RESIDUE;
   c->n = n;
   c->stride = stride;
   c->max_len = max_len;

@@ -458,12 +458,9 @@ int sq_onesweep_sort(sq_ctx* c, uint64_t* keys_in, uint64_t* keys_alt, uint32_t*
     SQ_TIMED(c, SQ_K_SORT_HIST, os_hist_scan_kernel<<<(unsigned)(nbatch * 8), 32, 0, st>>>(hist));
     SQ_LAUNCH_CHECK(c);
   }
-  static bool attr_set = false;
-  if (!attr_set) {
-    SQ_CUDA(c, cudaFuncSetAttribute(os_pass_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kOsSmem));
-    SQ_CUDA(c, cudaFuncSetAttribute(os_pass_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kOsSmem));
-    attr_set = true;
-  }
+  // (per device and cheap: set on every call, not once per process)
+  SQ_CUDA(c, cudaFuncSetAttribute(os_pass_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kOsSmem));
+  SQ_CUDA(c, cudaFuncSetAttribute(os_pass_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kOsSmem));
   uint64_t* kin = keys_in; uint64_t* kout = keys_alt;
   uint32_t* vin = vals_in; uint32_t* vout = vals_alt;
   dim3 grid((unsigned)ntiles, (unsigned)nbatch);

@@ -212,6 +212,7 @@ extern "C" int sq_edit_distance_weighted(sq_ctx* c, const uint32_t* pairs, int64
                                          const uint8_t* sub_cost, int indel, int max_d,
                                          uint16_t* dist_out) {
   if (!c) return SQ_ERR_INVALID_ARG;
+  SqDeviceGuard guard(c);
   if (c->n < 0) return SQ_ERR_NOT_PACKED;
   if (n_pairs < 0 || indel < 1 || indel > 255) return SQ_ERR_INVALID_ARG;
   if (n_pairs == 0) return SQ_OK;

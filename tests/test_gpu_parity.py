@@ -290,7 +290,11 @@ def test_error_codes():
     with pytest.raises(binding.SubQuadError) as ei:              # longer than the declared bound
         sq.pack(torch.zeros(40, dtype=torch.uint8, device="cuda"),
                 torch.tensor([0, 40], dtype=torch.int64, device="cuda"), alphabet=20, max_len=8)
-    assert ei.value.code == binding.SQ_ERR_BAD_RESIDUE
+    assert ei.value.code == binding.SQ_ERR_UNSUPPORTED
+    for bad_offs in ([0, 3, 2], [-1, 2, 4], [0, 9, 4]):          # decreasing, negative, beyond offsets[n]
+        with pytest.raises(binding.SubQuadError) as ei:
+            sq.pack(seqs, torch.tensor(bad_offs, dtype=torch.int64, device="cuda"), alphabet=20, max_len=8)
+        assert ei.value.code == binding.SQ_ERR_INVALID_ARG
     with pytest.raises(binding.SubQuadError) as ei:
         sq.pack(seqs, offs, alphabet=20, max_len=1000)
     assert ei.value.code == binding.SQ_ERR_UNSUPPORTED
