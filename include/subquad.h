@@ -132,6 +132,42 @@ int  sq_lsh_candidates(sq_ctx* ctx, const uint32_t* sig, int H, int bands, int r
                        int bucket_cap, int flags, uint32_t* pairs_out, int64_t capacity,
                        int64_t* n_pairs);
 
+/* a3-a5 in two steps, for callers that emit the candidate list piecewise (the streamed entry point
+ * below; one rank of a multi-GPU run).  sq_lsh_prepare runs band keys, bucket sort and bucket scan
+ * once and keeps the sorted records, the bucket-id table and the work lists in the workspace scratch
+ * (valid until the next call that resets the scratch: sq_pack, sq_lsh_prepare / sq_lsh_candidates,
+ * sq_all_pairs, sq_join*, sq_affinity_graph without the schedule).  *n_raw (host, may be NULL) = pairs
+ * before cross-band dedupe, over ALL rows.  sq_lsh_emit_range then writes the candidates (i, j) of
+ * the rows row_lo <= i < row_hi -- the same pairs sq_lsh_candidates would list for those i, in the
+ * same order -- into pairs_out; any number of calls, any ranges.  sq_lsh_candidates is
+ * prepare + emit_range(0, n).  SQ_ERR_NOT_PACKED if the prepared state is gone; both synchronise;
+ * SQ_ERR_CAPACITY as for sq_lsh_candidates (per call: fewer than 2^32 - 1 pairs per range). */
+int  sq_lsh_prepare(sq_ctx* ctx, const uint32_t* sig, int H, int bands, int rows, int bucket_cap,
+                    int64_t* n_raw);
+int  sq_lsh_emit_range(sq_ctx* ctx, int64_t row_lo, int64_t row_hi, int flags, uint32_t* pairs_out,
+                       int64_t capacity, int64_t* n_pairs);
+
+/* next-3  Out-of-core and sharded candidates + distances (PAPER.md L139-143
+ * Eq. 12 batch sizing, L334: 10^7 sequences at 186 GB).  The rows 0..n-1 are cut into batches of
+ * `batch_rows` consecutive ids; batch b is handled by this call iff b % n_parts == part (one GPU:
+ * part = 0, n_parts = 1; rank g of G: part = g, n_parts = G -- block-cyclic, because row i pairs only
+ * with j > i and low ids carry more pairs).  Per batch: sq_lsh_emit_range into a device block of
+ * `block_capacity` pairs, sq_edit_distance on it, both copied to the host buffers on the context's
+ * second stream while the next batch is emitted.  A batch that overflows the block is halved and
+ * redone, so only ONE block (twice, double-buffered) lives on the device: the list may exceed HBM and
+ * 2^32 pairs (64-bit totals; each block < 2^32 - 1).  batch_rows <= 0: B of Eq. 12 with M_avail = 10 *
+ * block_capacity bytes, c = 10 (bytes per candidate), l_max = 1.
+ * pairs_host uint32[capacity][2], dist_host uint16[capacity] (pinned for full speed): the batches of
+ * this part in ascending order, each ascending in (i, j) -- with n_parts = 1 exactly the output of
+ * sq_lsh_candidates + sq_edit_distance.  *n_pairs (host) = pairs of this part; *n_raw (may be NULL) as
+ * sq_lsh_prepare.  Workspace: SQ_OP_LSH with pair_capacity = block_capacity, plus 20 *
+ * block_capacity + 1024 bytes.  SQ_ERR_CAPACITY (required count returned) if the part exceeds
+ * `capacity`, or if one single row exceeds block_capacity.  Synchronises. */
+int  sq_candidates_stream_host(sq_ctx* ctx, const uint32_t* sig, int H, int bands, int rows,
+                               int bucket_cap, int max_d, int64_t batch_rows, int64_t block_capacity,
+                               int part, int n_parts, uint32_t* pairs_host, uint16_t* dist_host,
+                               int64_t capacity, int64_t* n_pairs, int64_t* n_raw);
+
 /* a6  Batched exact Levenshtein distance (Eq. 46, unit costs, boundary
  * D[x][0]=x, D[0][y]=y; spec C1) by Myers/Hyyro bit-parallel DP.
  * pairs: uint32[n_pairs][2], any order, any i,j < n (i == j allowed, gives 0).

@@ -25,7 +25,7 @@ JOIN_UPPER = 1
 OPT_SORT_KEY_BYTES, OPT_SCHED_MIN_BYTES = 1, 2
 
 EXPORTS = ["sq_create", "sq_destroy", "sq_workspace_bytes", "sq_set_workspace", "sq_pack",
-           "sq_minhash", "sq_lsh_candidates", "sq_edit_distance", "sq_edit_distance_weighted", "sq_affinity_graph", "sq_all_pairs",
+           "sq_minhash", "sq_lsh_candidates", "sq_lsh_prepare", "sq_lsh_emit_range", "sq_candidates_stream_host", "sq_edit_distance", "sq_edit_distance_weighted", "sq_affinity_graph", "sq_all_pairs",
            "sq_join", "sq_join_host", "sq_batch_size", "sq_set_option", "sq_pipeline_host", "sq_pipeline_host_csr", "sq_packed_n", "sq_packed_stride", "sq_last_raw_pairs",
            "sq_kernel_launches", "sq_last_cuda_error", "sq_strerror", "sq_int_peak",
            "sq_profile_enable", "sq_profile_reset", "sq_profile_read", "sq_profile_name"]
@@ -72,6 +72,13 @@ def load_library():
     L.sq_minhash.argtypes = [vp, i32, i32, C.c_uint64, vp]
     L.sq_lsh_candidates.restype = i32
     L.sq_lsh_candidates.argtypes = [vp, vp, i32, i32, i32, i32, i32, vp, i64, C.POINTER(i64)]
+    L.sq_lsh_prepare.restype = i32
+    L.sq_lsh_prepare.argtypes = [vp, vp, i32, i32, i32, i32, C.POINTER(i64)]
+    L.sq_lsh_emit_range.restype = i32
+    L.sq_lsh_emit_range.argtypes = [vp, i64, i64, i32, vp, i64, C.POINTER(i64)]
+    L.sq_candidates_stream_host.restype = i32
+    L.sq_candidates_stream_host.argtypes = [vp, vp, i32, i32, i32, i32, i32, i64, i64, i32, i32, vp, vp, i64,
+                                            C.POINTER(i64), C.POINTER(i64)]
     L.sq_edit_distance.restype = i32
     L.sq_edit_distance.argtypes = [vp, vp, i64, i32, vp]
     L.sq_edit_distance_weighted.restype = i32
@@ -220,6 +227,39 @@ class SubQuad:
                                         pairs_out.shape[0], C.byref(cnt))
         self._check(rc, required=cnt.value)
         return cnt.value
+
+    def lsh_prepare(self, sig, bands, rows, bucket_cap) -> int:
+        """Band keys, bucket sort and bucket scan, kept in the workspace; returns the raw pair count."""
+        H = sig.shape[1] if sig.dim() == 2 else 0
+        raw = C.c_int64(0)
+        self._check(self.lib.sq_lsh_prepare(self.h, _dev_ptr(sig, torch.int32, "sig"), H, bands, rows,
+                                            bucket_cap, C.byref(raw)))
+        return raw.value
+
+    def lsh_emit_range(self, row_lo, row_hi, pairs_out, flags=LSH_SORTED) -> int:
+        """Candidates of the rows [row_lo, row_hi) after lsh_prepare; returns their number."""
+        cnt = C.c_int64(0)
+        rc = self.lib.sq_lsh_emit_range(self.h, row_lo, row_hi, flags,
+                                        _dev_ptr(pairs_out, torch.int32, "pairs_out"), pairs_out.shape[0],
+                                        C.byref(cnt))
+        self._check(rc, required=cnt.value)
+        return cnt.value
+
+    def candidates_stream_host(self, sig, bands, rows, bucket_cap, max_d, pairs_out_host, dist_out_host,
+                               block_capacity, batch_rows=0, part=0, n_parts=1):
+        """Out-of-core / sharded candidates + distances into (pinned) HOST tensors.  Returns
+        (pairs of this part, raw pairs over all rows)."""
+        for t in (pairs_out_host, dist_out_host):
+            if t.is_cuda or not t.is_contiguous():
+                raise TypeError("candidates_stream_host takes contiguous host tensors")
+        H = sig.shape[1] if sig.dim() == 2 else 0
+        cnt, raw = C.c_int64(0), C.c_int64(0)
+        rc = self.lib.sq_candidates_stream_host(
+            self.h, _dev_ptr(sig, torch.int32, "sig"), H, bands, rows, bucket_cap, max_d, batch_rows,
+            block_capacity, part, n_parts, C.c_void_p(pairs_out_host.data_ptr()),
+            C.c_void_p(dist_out_host.data_ptr()), dist_out_host.shape[0], C.byref(cnt), C.byref(raw))
+        self._check(rc, required=cnt.value)
+        return cnt.value, raw.value
 
     def edit_distance(self, pairs, n_pairs, max_d, dist_out=None):
         if dist_out is None:

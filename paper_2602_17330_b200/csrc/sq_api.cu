@@ -298,6 +298,104 @@ int sq_pipeline_host_csr(sq_ctx* c, const uint8_t* seqs_host, const int64_t* off
                             capacity, n_pairs);
 }
 
+// Out-of-core / sharded form of a3-a6: the candidate list is produced and verified batch by batch of
+// rows (external ids), every batch copied to the host on the copy stream while the next one is
+// emitted.  See subquad.h.
+int sq_candidates_stream_host(sq_ctx* c, const uint32_t* sig, int H, int bands, int rows, int bucket_cap,
+                              int max_d, int64_t batch_rows, int64_t block_capacity, int part, int n_parts,
+                              uint32_t* pairs_host, uint16_t* dist_host, int64_t capacity, int64_t* n_pairs,
+                              int64_t* n_raw) {
+  if (!c || !n_pairs) return SQ_ERR_INVALID_ARG;
+  SqDeviceGuard guard(c);
+  *n_pairs = 0;
+  if (n_raw) *n_raw = 0;
+  if (c->n < 0) return SQ_ERR_NOT_PACKED;
+  if (capacity < 0 || block_capacity < 1 || n_parts < 1 || part < 0 || part >= n_parts) return SQ_ERR_INVALID_ARG;
+  if (capacity > 0 && (!pairs_host || !dist_host)) return SQ_ERR_INVALID_ARG;
+  if (block_capacity >= (1ll << 32) - 1) return SQ_ERR_UNSUPPORTED;
+  if (!c->ws) return SQ_ERR_WORKSPACE;
+  const int64_t n = c->n;
+  // two device blocks (pairs + distances) at the END of the workspace, out of the scratch's way
+  const size_t blk = sq_align_up((size_t)block_capacity * 8 + 16) + sq_align_up((size_t)block_capacity * 2 + 16);
+  if (2 * blk + c->persist + 4096 > c->ws_bytes) return SQ_ERR_WORKSPACE;
+  const size_t saved = c->ws_bytes;
+  uint8_t* io = c->ws + (saved - 2 * blk) / 256 * 256;
+  c->ws_bytes = (size_t)(io - c->ws);
+  uint32_t* dp[2]; uint16_t* dd[2];
+  for (int s = 0; s < 2; ++s) {
+    dp[s] = reinterpret_cast<uint32_t*>(io + s * blk);
+    dd[s] = reinterpret_cast<uint16_t*>(io + s * blk + sq_align_up((size_t)block_capacity * 8 + 16));
+  }
+  cudaEvent_t done[2] = {nullptr, nullptr}, ready = nullptr;
+  int rc = SQ_OK;
+  int64_t total = 0;
+  do {
+    if ((rc = sq_lsh_prepare(c, sig, H, bands, rows, bucket_cap, n_raw)) != SQ_OK) break;
+    if (cudaEventCreateWithFlags(&done[0], cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&done[1], cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&ready, cudaEventDisableTiming) != cudaSuccess) { rc = SQ_ERR_CUDA; break; }
+    if (batch_rows <= 0) {
+      // PAPER.md Eq. 12 with M_avail = the bytes of one device block, c = 10 bytes per candidate
+      // (pair + distance) and l_max = 1: B rows whose B x B tile of cells would fill the block
+      batch_rows = sq_batch_size(n, (uint64_t)block_capacity * 10ull, 10u, 1u);
+    }
+    if (batch_rows < 1) batch_rows = 1;
+    bool used[2] = {false, false};
+    int slot = 0;
+    const int64_t nbatch = n > 0 ? (n + batch_rows - 1) / batch_rows : 0;
+    for (int64_t b = part; b < nbatch && rc == SQ_OK; b += n_parts) {
+      // a batch that does not fit one block is halved (a small stack of row ranges, in order)
+      int64_t stack_lo[64], stack_hi[64];
+      int sp = 0;
+      stack_lo[0] = b * batch_rows;
+      stack_hi[0] = stack_lo[0] + batch_rows < n ? stack_lo[0] + batch_rows : n;
+      sp = 1;
+      while (sp > 0 && rc == SQ_OK) {
+        const int64_t lo = stack_lo[sp - 1], hi = stack_hi[sp - 1];
+        --sp;
+        if (used[slot]) {
+          if (cudaEventSynchronize(done[slot]) != cudaSuccess) { rc = SQ_ERR_CUDA; break; }   // its last copy has left
+          used[slot] = false;
+        }
+        int64_t cnt = 0;
+        int r2 = sq_lsh_emit_range(c, lo, hi, SQ_LSH_SORTED, dp[slot], block_capacity, &cnt);
+        if (r2 == SQ_ERR_CAPACITY || r2 == SQ_ERR_WORKSPACE || r2 == SQ_ERR_UNSUPPORTED) {
+          if (hi - lo <= 1 || sp + 2 > 64) { rc = r2; if (r2 == SQ_ERR_CAPACITY) total += cnt; break; }
+          const int64_t mid = lo + (hi - lo) / 2;
+          stack_lo[sp] = mid; stack_hi[sp] = hi; ++sp;          // second half is done after the first
+          stack_lo[sp] = lo; stack_hi[sp] = mid; ++sp;
+          continue;
+        }
+        if (r2 != SQ_OK) { rc = r2; break; }
+        if (cnt == 0) continue;
+        if (total + cnt <= capacity) {
+          if ((rc = sq_edit_distance_impl(c, dp[slot], cnt, max_d, dd[slot])) != SQ_OK) break;
+          if (cudaEventRecord(ready, c->stream) != cudaSuccess ||
+              cudaStreamWaitEvent(c->copy_stream, ready, 0) != cudaSuccess ||
+              cudaMemcpyAsync(pairs_host + 2 * total, dp[slot], (size_t)cnt * 8, cudaMemcpyDeviceToHost,
+                              c->copy_stream) != cudaSuccess ||
+              cudaMemcpyAsync(dist_host + total, dd[slot], (size_t)cnt * 2, cudaMemcpyDeviceToHost,
+                              c->copy_stream) != cudaSuccess ||
+              cudaEventRecord(done[slot], c->copy_stream) != cudaSuccess) { rc = SQ_ERR_CUDA; break; }
+          used[slot] = true;
+          slot ^= 1;
+        }
+        total += cnt;                                            // keeps counting past `capacity`
+      }
+    }
+  } while (0);
+  cudaStreamSynchronize(c->copy_stream);
+  cudaStreamSynchronize(c->stream);
+  if (rc == SQ_ERR_CUDA) c->last_err = cudaGetLastError();
+  for (int s = 0; s < 2; ++s) if (done[s]) cudaEventDestroy(done[s]);
+  if (ready) cudaEventDestroy(ready);
+  c->ws_bytes = saved;
+  sq_scratch_reset(c);
+  if (rc != SQ_OK) return rc;
+  *n_pairs = total;
+  return total > capacity ? SQ_ERR_CAPACITY : SQ_OK;
+}
+
 }  // extern "C"
 
 void sq_prof_drain(sq_ctx* c) {

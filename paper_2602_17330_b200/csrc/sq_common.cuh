@@ -44,6 +44,21 @@ struct sq_ctx {
   int64_t sched_chunks = 0;
   const void* sched_pairs = nullptr;          // the pair buffer it describes
   int64_t sched_npairs = 0;
+  // State left by sq_lsh_prepare for sq_lsh_emit_range: the sorted records, the bucket-id table and
+  // the unit lists live in the scratch below `mark`; every emit call allocates above it.  Dies with
+  // the next scratch reset.
+  struct LshState {
+    bool valid = false;
+    int64_t n = 0, n2 = 0, raw = 0;
+    int bands = 0, bw = 0;
+    uint32_t *vin = nullptr, *vint = nullptr, *S = nullptr, *cnt = nullptr, *ubase = nullptr;
+    uint32_t *rowidx = nullptr, *ext_off = nullptr, *rowstart = nullptr, *active = nullptr;
+    uint2 *loc = nullptr, *units = nullptr, *units0 = nullptr;
+    uint8_t* tmp = nullptr;
+    uint32_t nunits = 0, nunits0 = 0;
+    unsigned long long ntiles = 0;
+    size_t mark = 0;
+  } lsh;
   // tuning (sq_set_option)
   int sort_key_bytes = 4;       // top bytes of the band key the bucket sort orders by (1..8)
   int64_t sched_min_bytes = (int64_t)96 << 20;   // packed bytes above which the DP follows the schedule
@@ -100,7 +115,7 @@ static inline T* sq_scratch(sq_ctx* c, size_t count) {
   c->scratch_top += bytes;
   return p;
 }
-static inline void sq_scratch_reset(sq_ctx* c) { c->scratch_top = c->persist; c->sched = nullptr; }
+static inline void sq_scratch_reset(sq_ctx* c) { c->scratch_top = c->persist; c->sched = nullptr; c->lsh.valid = false; }
 
 #define SQ_CUDA(ctx, call)                                   \
   do {                                                       \

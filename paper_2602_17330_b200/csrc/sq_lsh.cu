@@ -442,18 +442,23 @@ template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
 
 // Band 0: every pair of kept members is new.  One warp per unit.
+// `active` (may be nullptr = all): the units that hold a row of the id range [row_lo, row_hi) the
+// call emits (sq_lsh_emit_range); rows outside the range emit nothing.
 template <int MODE>
 __global__ void __launch_bounds__(kEmWarps * 32)
-emit_band0_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint32_t* __restrict__ ids,
-                  int bands, uint32_t* __restrict__ cnt_off, uint32_t* __restrict__ outJ) {
+emit_band0_kernel(const uint2* __restrict__ units, const uint32_t* __restrict__ active, uint32_t nunits,
+                  const uint32_t* __restrict__ ids, int bands, uint32_t* __restrict__ cnt_off,
+                  uint32_t* __restrict__ outJ, uint32_t row_lo, uint32_t row_hi) {
   const int lane = threadIdx.x & 31;
-  const uint32_t u = blockIdx.x * kEmWarps + (threadIdx.x >> 5);
-  if (u >= nunits) return;
-  const uint2 unit = units[u];
+  const uint32_t ua = blockIdx.x * kEmWarps + (threadIdx.x >> 5);
+  if (ua >= nunits) return;
+  const uint2 unit = units[active ? active[ua] : ua];
   const uint32_t mrem = unit.y;
   const uint32_t* __restrict__ idp = ids + unit.x;
   const uint32_t nrows = min(32u, mrem - 1u);
-  const bool rowok = (uint32_t)lane < nrows;
+  bool rowok = (uint32_t)lane < nrows;
+  if (rowok) { const uint32_t me = idp[lane]; rowok = me >= row_lo && me < row_hi; }
+  const uint32_t okm = __ballot_sync(kFull, rowok);
   // internal row of a band-0 record = its sorted position: the rows of a unit are consecutive
   const int64_t myrow = (int64_t)unit.x + lane;
   if (MODE == EM_COUNT) {
@@ -462,6 +467,7 @@ emit_band0_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint32
   }
   const uint32_t off = rowok ? cnt_off[myrow] : 0u;
   for (uint32_t l = 0; l < nrows; ++l) {     // coalesced: the warp writes row l's partners
+    if (!((okm >> l) & 1u)) continue;
     const uint32_t o = __shfl_sync(kFull, off, l);
     for (uint32_t cc = l + 1 + lane; cc < mrem; cc += 32) outJ[o + cc - l - 1] = idp[cc];
   }
@@ -495,7 +501,7 @@ __device__ __forceinline__ void sweep_tile(const uint32_t* __restrict__ sm,
   }
 }
 
-struct EmDesc { uint32_t u, g0, mrem, c0; int b; bool ok; };
+struct EmDesc { uint32_t u, uid, g0, mrem, c0; int b; bool ok; };   // u = place in the (active) list, uid = unit
 
 // Bands >= 1.  Persistent warps stride over the unit list; the stream of (unit, column tile)
 // items is software-pipelined: ids two tiles ahead (registers), S rows one tile ahead
@@ -511,11 +517,11 @@ struct EmDesc { uint32_t u, g0, mrem, c0; int b; bool ok; };
 // MODE EM_FILL_J: outJ[off[g] + t] = external id of its t-th new partner.
 template <int BW, int MODE>
 __global__ void __launch_bounds__(kEmWarps * 32)
-emit_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint32_t* __restrict__ ids,
-            const uint32_t* __restrict__ ids_int, uint32_t n2, int bands,
+emit_kernel(const uint2* __restrict__ units, const uint32_t* __restrict__ active, uint32_t nunits,
+            const uint32_t* __restrict__ ids, const uint32_t* __restrict__ ids_int, uint32_t n2, int bands,
             const uint32_t* __restrict__ S, uint32_t* __restrict__ cnt_off,
             uint32_t* __restrict__ outJ, const uint32_t* __restrict__ ubase,
-            uint32_t* __restrict__ masks, uint2* __restrict__ loc) {
+            uint32_t* __restrict__ masks, uint2* __restrict__ loc, uint32_t row_lo, uint32_t row_hi) {
   constexpr int SW = 4 * BW;
   constexpr int RS = SW + 4;                 // shared row stride in words (16-byte aligned)
   constexpr int RPR = 32 / BW;               // S rows fetched per load round
@@ -525,16 +531,18 @@ emit_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint32_t* __
   const uint32_t nw = gridDim.x * kEmWarps;
   const uint32_t wg = blockIdx.x * kEmWarps + w;
   if (wg >= nunits) return;
-  uint2 unit_pref = units[wg];               // always the next unit this warp will open
+  auto uidx = [&](uint32_t k) -> uint32_t { return active ? active[k] : k; };
+  uint32_t uid_pref = uidx(wg);              // always the next unit this warp will open
+  uint2 unit_pref = units[uid_pref];
 
   auto next_desc = [&](EmDesc d) -> EmDesc {
     if (d.ok && d.c0 + 32 < d.mrem) { d.c0 += 32; return d; }
     EmDesc r;
     r.u = d.u + nw;
     r.ok = d.ok && r.u < nunits;
-    r.g0 = unit_pref.x; r.mrem = unit_pref.y; r.c0 = 0;
+    r.g0 = unit_pref.x; r.mrem = unit_pref.y; r.c0 = 0; r.uid = uid_pref;
     r.b = (int)(r.g0 / n2);
-    if (r.ok && r.u + nw < nunits) unit_pref = units[r.u + nw];
+    if (r.ok && r.u + nw < nunits) { uid_pref = uidx(r.u + nw); unit_pref = units[uid_pref]; }
     return r;
   };
   auto load_ids = [&](const EmDesc& d) -> uint32_t {          // internal rows of a column tile
@@ -556,7 +564,7 @@ emit_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint32_t* __
   };
 
   EmDesc dc;                                  // current tile
-  dc.u = wg - nw; dc.ok = true; dc.mrem = 0; dc.c0 = 0; dc.g0 = 0; dc.b = 0;
+  dc.u = wg - nw; dc.uid = 0; dc.ok = true; dc.mrem = 0; dc.c0 = 0; dc.g0 = 0; dc.b = 0;
   dc = next_desc(dc);
   uint32_t idc_c = load_ids(dc), idx_c = load_ext(dc);
   EmDesc dn = next_desc(dc);                  // next tile
@@ -580,13 +588,14 @@ emit_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint32_t* __
     if (dc.c0 == 0) {                         // a unit starts: its rows are the first 32 columns
       myid = idc_c;
       rowok = lane < min(32u, dc.mrem - 1u);
+      if (rowok) { const uint32_t me = ids[(int64_t)dc.g0 + lane]; rowok = me >= row_lo && me < row_hi; }
       acc = 0;
       if (MODE != EM_COUNT && rowok) {
         acc = cnt_off[(int64_t)dc.g0 + lane];
         const uint32_t nxt = cnt_off[(int64_t)dc.g0 + lane + 1];
         if (nxt > acc) loc[(int64_t)b * n2 + myid] = make_uint2(acc, nxt - acc);
       }
-      if (MODE == EM_COUNT && masks) ub = ubase[dc.u];
+      if (MODE == EM_COUNT && masks) ub = ubase[dc.uid];
 #pragma unroll
       for (int ch = 0; ch < BW; ++ch) {
         if (4 * ch < b) {
@@ -633,7 +642,7 @@ emit_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint32_t* __
 constexpr int kFillDepth = 5;
 
 __global__ void __launch_bounds__(kEmWarps * 32)
-emit_fill_masks_kernel(const uint2* __restrict__ units, uint32_t nunits,
+emit_fill_masks_kernel(const uint2* __restrict__ units, const uint32_t* __restrict__ active, uint32_t nunits,
                        const uint32_t* __restrict__ ubase, const uint32_t* __restrict__ masks,
                        const uint32_t* __restrict__ ids, const uint32_t* __restrict__ ids_int,
                        uint32_t n2, int bands, const uint32_t* __restrict__ cnt_off,
@@ -646,7 +655,7 @@ emit_fill_masks_kernel(const uint2* __restrict__ units, uint32_t nunits,
   struct L2 { uint32_t idx, idi, msk, acc, nxt; };
   auto load1 = [&](uint32_t uu) -> L1 {              // needs only the unit index
     L1 r; r.un = make_uint2(0u, 0u); r.tb = 0u;
-    if (uu < nunits) { r.un = units[uu]; r.tb = ubase[uu]; }
+    if (uu < nunits) { const uint32_t uid = active ? active[uu] : uu; r.un = units[uid]; r.tb = ubase[uid]; }
     return r;
   };
   auto load2 = [&](const L1& a) -> L2 {              // needs the descriptor
@@ -863,7 +872,7 @@ row_sort_kernel(const uint32_t* __restrict__ off, const uint2* __restrict__ loc,
                 const uint32_t* __restrict__ ids0, const uint32_t* __restrict__ ext_off,
                 bool do_sort, const uint32_t* __restrict__ inJ, uint2* out,
                 unsigned long long* __restrict__ next_row, const uint32_t* __restrict__ rowstart,
-                uint32_t* __restrict__ delta, uint4* __restrict__ sched) {
+                uint32_t* __restrict__ delta, uint4* __restrict__ sched, uint32_t row_lo, uint32_t row_hi) {
   __shared__ __align__(16) uint32_t bins_sh[kRsWarps][kRsBins + kRsBins / 32];
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   // Rows differ by four orders of magnitude in size: persistent warps fetch rows kRsChunk at a
@@ -905,16 +914,17 @@ row_sort_kernel(const uint32_t* __restrict__ off, const uint2* __restrict__ loc,
         for (uint32_t k = (b + 31) / 32 + lane; (uint64_t)k * 32 < e; k += 32)
           sched[k] = make_uint4((uint32_t)r, d, e, b);
       }
-      sort_one_row(inJ, out, g.x, g.y, i, eo, do_sort, bins_sh[w], lane);
+      if (i >= row_lo && i < row_hi) sort_one_row(inJ, out, g.x, g.y, i, eo, do_sort, bins_sh[w], lane);
       __syncwarp();
     }
   }
 }
 
 template <int BW>
-int launch_emit(sq_ctx* c, int mode, const uint2* units, uint32_t nunits, const uint32_t* ids,
+int launch_emit(sq_ctx* c, int mode, const uint2* units, const uint32_t* active, uint32_t nunits, const uint32_t* ids,
                 const uint32_t* ids_int, uint32_t n2, int bands, const uint32_t* S,
-                uint32_t* cnt_off, uint32_t* outJ, const uint32_t* ubase, uint32_t* masks, uint2* loc) {
+                uint32_t* cnt_off, uint32_t* outJ, const uint32_t* ubase, uint32_t* masks, uint2* loc,
+                uint32_t row_lo, uint32_t row_hi) {
   // persistent warps: exactly the resident blocks of every SM, never more warps than units
   int per_sm = 0;
   cudaError_t e;
@@ -928,56 +938,81 @@ int launch_emit(sq_ctx* c, int mode, const uint2* units, uint32_t nunits, const 
   if (g > need) g = need;
   if (mode == EM_COUNT)
     SQ_TIMED(c, SQ_K_EMIT, emit_kernel<BW, EM_COUNT><<<g, kEmWarps * 32, 0, c->stream>>>(
-        units, nunits, ids, ids_int, n2, bands, S, cnt_off, outJ, ubase, masks, loc));
+        units, active, nunits, ids, ids_int, n2, bands, S, cnt_off, outJ, ubase, masks, loc, row_lo, row_hi));
   else
     SQ_TIMED(c, SQ_K_EMIT, emit_kernel<BW, EM_FILL_J><<<g, kEmWarps * 32, 0, c->stream>>>(
-        units, nunits, ids, ids_int, n2, bands, S, cnt_off, outJ, ubase, masks, loc));
+        units, active, nunits, ids, ids_int, n2, bands, S, cnt_off, outJ, ubase, masks, loc, row_lo, row_hi));
   SQ_LAUNCH_CHECK(c);
   return SQ_OK;
 }
 
-int launch_emit_band0(sq_ctx* c, int mode, const uint2* units0, uint32_t nunits0,
-                      const uint32_t* ids, int bands, uint32_t* cnt_off, uint32_t* outJ) {
+int launch_emit_band0(sq_ctx* c, int mode, const uint2* units0, const uint32_t* active0, uint32_t nunits0,
+                      const uint32_t* ids, int bands, uint32_t* cnt_off, uint32_t* outJ,
+                      uint32_t row_lo, uint32_t row_hi) {
   const unsigned g = (nunits0 + kEmWarps - 1) / kEmWarps;
   if (mode == EM_COUNT)
     SQ_TIMED(c, SQ_K_EMIT, emit_band0_kernel<EM_COUNT><<<g, kEmWarps * 32, 0, c->stream>>>(
-        units0, nunits0, ids, bands, cnt_off, outJ));
+        units0, active0, nunits0, ids, bands, cnt_off, outJ, row_lo, row_hi));
   else
     SQ_TIMED(c, SQ_K_EMIT, emit_band0_kernel<EM_FILL_J><<<g, kEmWarps * 32, 0, c->stream>>>(
-        units0, nunits0, ids, bands, cnt_off, outJ));
+        units0, active0, nunits0, ids, bands, cnt_off, outJ, row_lo, row_hi));
   SQ_LAUNCH_CHECK(c);
   return SQ_OK;
 }
 
-int launch_fill_masks(sq_ctx* c, const uint2* units, uint32_t nunits, const uint32_t* ubase,
+int launch_fill_masks(sq_ctx* c, const uint2* units, const uint32_t* active, uint32_t nunits, const uint32_t* ubase,
                       const uint32_t* masks, const uint32_t* ids, const uint32_t* ids_int,
                       uint32_t n2, int bands, const uint32_t* cnt_off, uint32_t* outJ, uint2* loc) {
   unsigned g = (unsigned)c->sm_count * 16u;          // 64 warps per SM, persistent
   const unsigned need = (nunits + kEmWarps - 1) / kEmWarps;
   if (g > need) g = need;
   SQ_TIMED(c, SQ_K_EMIT, emit_fill_masks_kernel<<<g, kEmWarps * 32, 0, c->stream>>>(
-      units, nunits, ubase, masks, ids, ids_int, n2, bands, cnt_off, outJ, loc));
+      units, active, nunits, ubase, masks, ids, ids_int, n2, bands, cnt_off, outJ, loc));
   SQ_LAUNCH_CHECK(c);
   return SQ_OK;
 }
 
 // both unit lists, one mode.  `masks` (may be nullptr): the per-tile masks of new pairs, written
 // by the count pass and, when present, read by the fill pass instead of repeating the compares.
-int dispatch_emit(sq_ctx* c, int bw, int mode, const uint2* units, uint32_t nunits,
-                  const uint2* units0, uint32_t nunits0, const uint32_t* ids,
+// (active / active0 = the units of this call's row range, nullptr = all; nunits / nunits0 = their number)
+int dispatch_emit(sq_ctx* c, int bw, int mode, const uint2* units, const uint32_t* active, uint32_t nunits,
+                  const uint2* units0, const uint32_t* active0, uint32_t nunits0, const uint32_t* ids,
                   const uint32_t* ids_int, uint32_t n2, int bands, const uint32_t* S,
-                  uint32_t* cnt_off, uint32_t* outJ, const uint32_t* ubase, uint32_t* masks, uint2* loc) {
+                  uint32_t* cnt_off, uint32_t* outJ, const uint32_t* ubase, uint32_t* masks, uint2* loc,
+                  uint32_t row_lo, uint32_t row_hi) {
   int rc = SQ_OK;
-  if (nunits0) rc = launch_emit_band0(c, mode, units0, nunits0, ids, bands, cnt_off, outJ);
+  if (nunits0) rc = launch_emit_band0(c, mode, units0, active0, nunits0, ids, bands, cnt_off, outJ, row_lo, row_hi);
   if (rc != SQ_OK || nunits == 0) return rc;
   if (mode != EM_COUNT && masks)
-    return launch_fill_masks(c, units, nunits, ubase, masks, ids, ids_int, n2, bands, cnt_off, outJ, loc);
+    return launch_fill_masks(c, units, active, nunits, ubase, masks, ids, ids_int, n2, bands, cnt_off, outJ, loc);
   switch (bw) {
-    case 1: return launch_emit<1>(c, mode, units, nunits, ids, ids_int, n2, bands, S, cnt_off, outJ, ubase, masks, loc);
-    case 2: return launch_emit<2>(c, mode, units, nunits, ids, ids_int, n2, bands, S, cnt_off, outJ, ubase, masks, loc);
-    case 4: return launch_emit<4>(c, mode, units, nunits, ids, ids_int, n2, bands, S, cnt_off, outJ, ubase, masks, loc);
-    default: return launch_emit<8>(c, mode, units, nunits, ids, ids_int, n2, bands, S, cnt_off, outJ, ubase, masks, loc);
+    case 1: return launch_emit<1>(c, mode, units, active, nunits, ids, ids_int, n2, bands, S, cnt_off, outJ, ubase, masks, loc, row_lo, row_hi);
+    case 2: return launch_emit<2>(c, mode, units, active, nunits, ids, ids_int, n2, bands, S, cnt_off, outJ, ubase, masks, loc, row_lo, row_hi);
+    case 4: return launch_emit<4>(c, mode, units, active, nunits, ids, ids_int, n2, bands, S, cnt_off, outJ, ubase, masks, loc, row_lo, row_hi);
+    default: return launch_emit<8>(c, mode, units, active, nunits, ids, ids_int, n2, bands, S, cnt_off, outJ, ubase, masks, loc, row_lo, row_hi);
   }
+}
+
+// the units with at least one row of the id range [row_lo, row_hi): the ids of a bucket ascend, so a
+// unit's rows lie between the ids of its first and its last row (order of the list is irrelevant)
+__global__ void __launch_bounds__(256)
+active_units_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint32_t* __restrict__ ids,
+                    uint32_t row_lo, uint32_t row_hi, uint32_t* __restrict__ active,
+                    unsigned long long* __restrict__ nactive) {
+  const uint32_t u = blockIdx.x * blockDim.x + threadIdx.x;
+  bool on = false;
+  if (u < nunits) {
+    const uint2 un = units[u];
+    const uint32_t nrows = min(32u, un.y - 1u);
+    on = ids[un.x] < row_hi && ids[un.x + nrows - 1u] >= row_lo;
+  }
+  const uint32_t m = __ballot_sync(kFull, on);
+  if (!m) return;
+  const int lane = threadIdx.x & 31;
+  unsigned long long base = 0;
+  if (lane == 0) base = atomicAdd(nactive, (unsigned long long)__popc(m));
+  base = __shfl_sync(kFull, base, 0);
+  if (on) active[base + __popc(m & ((1u << lane) - 1u))] = u;
 }
 
 inline int chunks_for(int bands) { return bands <= 4 ? 1 : bands <= 8 ? 2 : bands <= 16 ? 4 : 8; }
@@ -1004,26 +1039,28 @@ size_t sq_lsh_scratch_bytes(int64_t n, int bands, int64_t pair_capacity) {
   return s + 4096;
 }
 
-extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int bands, int rows,
-                                 int bucket_cap, int flags, uint32_t* pairs_out, int64_t capacity,
-                                 int64_t* n_pairs) {
-  if (!c || !n_pairs) return SQ_ERR_INVALID_ARG;
+// a3, a4, a5.1: band keys -> bucket sort -> bucket scan.  Leaves the sorted records, the bucket-id
+// table S and the unit lists in the scratch (c->lsh) for any number of sq_lsh_emit_range calls.
+extern "C" int sq_lsh_prepare(sq_ctx* c, const uint32_t* sig, int H, int bands, int rows, int bucket_cap,
+                              int64_t* n_raw) {
+  if (!c) return SQ_ERR_INVALID_ARG;
   SqDeviceGuard guard(c);
-  *n_pairs = 0;
+  if (n_raw) *n_raw = 0;
   if (c->n < 0) return SQ_ERR_NOT_PACKED;
-  if (H < 1 || bands < 1 || rows < 1 || bucket_cap < 1 || capacity < 0 ||
-      (int64_t)bands * rows > H || (flags != SQ_LSH_SORTED && flags != SQ_LSH_UNORDERED))
-    return SQ_ERR_INVALID_ARG;
+  if (H < 1 || bands < 1 || rows < 1 || bucket_cap < 1 || (int64_t)bands * rows > H) return SQ_ERR_INVALID_ARG;
   if (bands > SQ_MAX_BANDS || H > SQ_MAX_H) return SQ_ERR_UNSUPPORTED;
   const int64_t n = c->n;
   c->last_raw_pairs = 0;
-  if (n == 0) return SQ_OK;
-  if (!sig || (capacity > 0 && !pairs_out)) return SQ_ERR_INVALID_ARG;
+  sq_scratch_reset(c);
+  sq_ctx::LshState& L = c->lsh;
+  L = sq_ctx::LshState();
+  L.n = n; L.bands = bands; L.bw = chunks_for(bands);
+  if (n == 0) { L.valid = true; L.mark = c->scratch_top; return SQ_OK; }
+  if (!sig) return SQ_ERR_INVALID_ARG;
   if (n * bands >= (1ll << 31)) return SQ_ERR_UNSUPPORTED;
 
-  sq_scratch_reset(c);
   const size_t rec = (size_t)n * bands;
-  const int bw = chunks_for(bands), sw = 4 * bw;
+  const int sw = 4 * L.bw;
   uint64_t* k0 = sq_scratch<uint64_t>(c, rec);
   uint64_t* k1 = sq_scratch<uint64_t>(c, rec);
   uint32_t* v0 = sq_scratch<uint32_t>(c, rec);
@@ -1056,7 +1093,8 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
   SQ_CUDA(c, cudaMemcpyAsync(c->pinned, counters + 2, 8, cudaMemcpyDeviceToHost, st));
   SQ_CUDA(c, cudaStreamSynchronize(st));
   const int64_t n2 = (int64_t)c->pinned[0];
-  if (n2 < 2) return SQ_OK;                       // fewer than two usable signatures: no pairs
+  L.n2 = n2;
+  if (n2 < 2) { L.valid = true; L.mark = c->scratch_top; return SQ_OK; }   // no pairs
   uint64_t* kin = k0; uint64_t* kalt = k1; uint32_t* vin = v0; uint32_t* valt = v1;
   if (n2 != n) {
     SQ_TIMED(c, SQ_K_BANDKEY, compact_kernel<<<gb, 256, 0, st>>>(k0, nonempty, n, n2, bands, k1, v1));
@@ -1100,7 +1138,6 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
   // a5.1: buckets -> S table + unit lists (the unit lists live in the dead key buffer)
   uint2* units = reinterpret_cast<uint2*>(kalt);
   uint2* units0 = units + rec / 2 + 1;           // <= n2/2 units of band 0, <= rec/2 in all
-  SQ_CUDA(c, cudaMemsetAsync(cnt, 0, (rec + 2) * 4, st));
   SQ_TIMED(c, SQ_K_SEGMENT, s_prefill_kernel<<<(unsigned)((n2 * (sw / 4) + 255) / 256), 256, 0, st>>>(S, n2, sw));
   SQ_LAUNCH_CHECK(c);
   {
@@ -1112,40 +1149,103 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
   SQ_CUDA(c, cudaMemcpyAsync(c->pinned, counters, 64, cudaMemcpyDeviceToHost, st));
   SQ_CUDA(c, cudaStreamSynchronize(st));
   c->last_raw_pairs = (int64_t)c->pinned[1];
-  const uint32_t nunits = (uint32_t)c->pinned[4], nunits0 = (uint32_t)c->pinned[5];
-  if (nunits + nunits0 == 0) return SQ_OK;
+  if (n_raw) *n_raw = c->last_raw_pairs;
+  L.raw = c->last_raw_pairs;
+  L.nunits = (uint32_t)c->pinned[4]; L.nunits0 = (uint32_t)c->pinned[5]; L.ntiles = c->pinned[7];
+  L.vin = vin; L.vint = vint; L.S = S; L.cnt = cnt; L.ubase = ubase; L.loc = loc; L.rowidx = rowidx;
+  L.ext_off = ext_off; L.rowstart = rowstart; L.tmp = tmp; L.units = units; L.units0 = units0;
+  // the sorted keys are dead from here on: the lists of a call's active units take their place
+  L.active = reinterpret_cast<uint32_t*>(kin);
+  L.mark = c->scratch_top;
+  L.valid = true;
+  return SQ_OK;
+}
+
+// a5.2, a5.3 for the rows (external ids) [row_lo, row_hi): count -> offsets -> fill -> every row of the
+// range into its slice of pairs_out, ascending (i, j) (or grouped, SQ_LSH_UNORDERED).
+extern "C" int sq_lsh_emit_range(sq_ctx* c, int64_t row_lo, int64_t row_hi, int flags, uint32_t* pairs_out,
+                                 int64_t capacity, int64_t* n_pairs) {
+  if (!c || !n_pairs) return SQ_ERR_INVALID_ARG;
+  SqDeviceGuard guard(c);
+  *n_pairs = 0;
+  if (c->n < 0) return SQ_ERR_NOT_PACKED;
+  sq_ctx::LshState& L = c->lsh;
+  if (!L.valid || L.n != c->n) return SQ_ERR_NOT_PACKED;          // sq_lsh_prepare has not run (or its scratch is gone)
+  if (capacity < 0 || (flags != SQ_LSH_SORTED && flags != SQ_LSH_UNORDERED) || row_lo < 0 || row_hi < row_lo ||
+      row_hi > L.n)
+    return SQ_ERR_INVALID_ARG;
+  if (capacity > 0 && !pairs_out) return SQ_ERR_INVALID_ARG;
+  c->scratch_top = L.mark;
+  c->sched = nullptr;
+  if (L.n2 < 2 || L.nunits + L.nunits0 == 0 || row_lo == row_hi) return SQ_OK;
+  const int64_t n = L.n, n2 = L.n2;
+  const int bands = L.bands, bw = L.bw;
+  const size_t rec = (size_t)n * bands;
+  const int64_t total = n2 * bands;
+  const uint32_t lo = (uint32_t)row_lo, hi = (uint32_t)(row_hi > 0xFFFFFFFFll ? 0xFFFFFFFFll : row_hi);
+  cudaStream_t st = c->stream;
+  unsigned long long* counters = c->dflags;
+  uint32_t* cnt = L.cnt; uint2* loc = L.loc;
+  uint32_t* tmp32 = reinterpret_cast<uint32_t*>(L.tmp);
+  const unsigned gb = (unsigned)((n + 255) / 256);
+  int rc;
+  // the units that hold a row of the range (all of them for the whole repertoire)
+  const bool whole = row_lo == 0 && row_hi == n;
+  const uint32_t* active = nullptr; const uint32_t* active0 = nullptr;
+  uint32_t nunits = L.nunits, nunits0 = L.nunits0;
+  if (!whole) {
+    uint32_t* act = L.active;                    // <= rec / 2 units in all; the key buffer holds 2 * rec words
+    uint32_t* act0 = act + rec / 2 + 1;
+    SQ_CUDA(c, cudaMemsetAsync(counters + 4, 0, 16, st));
+    if (nunits) {
+      SQ_TIMED(c, SQ_K_SEGMENT, active_units_kernel<<<(nunits + 255) / 256, 256, 0, st>>>(
+          L.units, nunits, L.vin, lo, hi, act, counters + 4));
+      SQ_LAUNCH_CHECK(c);
+    }
+    if (nunits0) {
+      SQ_TIMED(c, SQ_K_SEGMENT, active_units_kernel<<<(nunits0 + 255) / 256, 256, 0, st>>>(
+          L.units0, nunits0, L.vin, lo, hi, act0, counters + 5));
+      SQ_LAUNCH_CHECK(c);
+    }
+    SQ_CUDA(c, cudaMemcpyAsync(c->pinned, counters, 64, cudaMemcpyDeviceToHost, st));
+    SQ_CUDA(c, cudaStreamSynchronize(st));
+    nunits = (uint32_t)c->pinned[4]; nunits0 = (uint32_t)c->pinned[5];
+    active = act; active0 = act0;
+    if (nunits + nunits0 == 0) return SQ_OK;
+  }
   // mask cache: 32 words per (unit, column tile); optional -- without it pass 2 repeats the compares
-  const unsigned long long ntiles = c->pinned[7];
-  uint32_t* masks = (nunits && ntiles) ? sq_scratch<uint32_t>(c, (size_t)ntiles * 32) : nullptr;
-  // a5.2 pass 1: counts per (internal row, band) -> offsets
-  rc = dispatch_emit(c, bw, EM_COUNT, units, nunits, units0, nunits0, vin, vint, (uint32_t)n2, bands, S,
-                     cnt, nullptr, ubase, masks, loc);
+  uint32_t* masks = (nunits && L.ntiles) ? sq_scratch<uint32_t>(c, (size_t)L.ntiles * 32) : nullptr;
+  // a5.2 pass 1: counts per sorted record -> offsets
+  SQ_CUDA(c, cudaMemsetAsync(cnt, 0, (rec + 2) * 4, st));
+  rc = dispatch_emit(c, bw, EM_COUNT, L.units, active, nunits, L.units0, active0, nunits0, L.vin, L.vint, (uint32_t)n2,
+                     bands, L.S, cnt, nullptr, L.ubase, masks, loc, lo, hi);
   if (rc != SQ_OK) return rc;
-  rc = sq_exclusive_scan_u32(c, cnt, cnt, total + 1, reinterpret_cast<uint32_t*>(tmp), counters);
+  rc = sq_exclusive_scan_u32(c, cnt, cnt, total + 1, tmp32, counters);
   if (rc != SQ_OK) return rc;
   SQ_CUDA(c, cudaMemcpyAsync(c->pinned, counters, 8, cudaMemcpyDeviceToHost, st));
   SQ_CUDA(c, cudaStreamSynchronize(st));
   const int64_t uniq = (int64_t)c->pinned[0];
   *n_pairs = uniq;
   if (uniq > capacity) return SQ_ERR_CAPACITY;
-  if (uniq >= (1ll << 32) - 1) return SQ_ERR_UNSUPPORTED;   // 32-bit output offsets
+  if (uniq >= (1ll << 32) - 1) return SQ_ERR_UNSUPPORTED;   // 32-bit output offsets (per call)
   if (uniq == 0) return SQ_OK;
   // a5.2 pass 2: the new partners of every sorted record into the partner scratch (unit by unit,
   // contiguous); it also leaves loc[band][row] = (start, length) of every non-empty group
   uint32_t* tmpJ = sq_scratch<uint32_t>(c, (size_t)uniq);
   if (!tmpJ) return SQ_ERR_WORKSPACE;
   SQ_CUDA(c, cudaMemsetAsync(loc, 0, (rec + 2) * 8, st));
-  rc = dispatch_emit(c, bw, EM_FILL_J, units, nunits, units0, nunits0, vin, vint, (uint32_t)n2, bands, S,
-                     cnt, tmpJ, ubase, masks, loc);
+  rc = dispatch_emit(c, bw, EM_FILL_J, L.units, active, nunits, L.units0, active0, nunits0, L.vin, L.vint, (uint32_t)n2,
+                     bands, L.S, cnt, tmpJ, L.ubase, masks, loc, lo, hi);
   if (rc != SQ_OK) return rc;
   // where every EXTERNAL row starts in the output
+  uint32_t* rowstart = L.rowstart; uint32_t* ext_off = L.ext_off;
   SQ_TIMED(c, SQ_K_SEGMENT, row_total_kernel<<<(unsigned)((n2 + 256) / 256), 256, 0, st>>>(cnt, loc, n2, bands, rowstart));
   SQ_LAUNCH_CHECK(c);
-  SQ_TIMED(c, SQ_K_SEGMENT, ext_count_kernel<<<gb, 256, 0, st>>>(rowidx, rowstart, n, ext_off));
+  SQ_TIMED(c, SQ_K_SEGMENT, ext_count_kernel<<<gb, 256, 0, st>>>(L.rowidx, rowstart, n, ext_off));
   SQ_LAUNCH_CHECK(c);
-  rc = sq_exclusive_scan_u32(c, ext_off, ext_off, n, reinterpret_cast<uint32_t*>(tmp), nullptr);
+  rc = sq_exclusive_scan_u32(c, ext_off, ext_off, n, tmp32, nullptr);
   if (rc != SQ_OK) return rc;
-  rc = sq_exclusive_scan_u32(c, rowstart, rowstart, n2 + 1, reinterpret_cast<uint32_t*>(tmp), nullptr);
+  rc = sq_exclusive_scan_u32(c, rowstart, rowstart, n2 + 1, tmp32, nullptr);
   if (rc != SQ_OK) return rc;                     // rowstart[r] = first internal position of row r
   // a5.3: every row (sorted if asked) into its slice of the output
   {
@@ -1164,8 +1264,8 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
     uint32_t* delta = sq_scratch<uint32_t>(c, (size_t)n2 + 1);
     if (!sched || !delta) { sched = nullptr; delta = nullptr; }
     SQ_TIMED(c, SQ_K_ROWSORT, row_sort_kernel<<<g, kRsWarps * 32, 0, st>>>(
-        cnt, loc, n2, bands, vin, ext_off, flags == SQ_LSH_SORTED, tmpJ, reinterpret_cast<uint2*>(pairs_out),
-        counters + 6, rowstart, delta, sched));
+        cnt, loc, n2, bands, L.vin, ext_off, flags == SQ_LSH_SORTED, tmpJ, reinterpret_cast<uint2*>(pairs_out),
+        counters + 6, rowstart, delta, sched, lo, hi));
     SQ_LAUNCH_CHECK(c);
     if (sched) {
       c->sched = sched;
@@ -1178,4 +1278,17 @@ extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int band
   }
   SQ_CUDA(c, cudaStreamSynchronize(st));
   return SQ_OK;
+}
+
+extern "C" int sq_lsh_candidates(sq_ctx* c, const uint32_t* sig, int H, int bands, int rows,
+                                 int bucket_cap, int flags, uint32_t* pairs_out, int64_t capacity,
+                                 int64_t* n_pairs) {
+  if (!c || !n_pairs) return SQ_ERR_INVALID_ARG;
+  *n_pairs = 0;
+  if (c->n < 0) return SQ_ERR_NOT_PACKED;
+  if (capacity < 0 || (flags != SQ_LSH_SORTED && flags != SQ_LSH_UNORDERED)) return SQ_ERR_INVALID_ARG;
+  if (c->n > 0 && capacity > 0 && !pairs_out) return SQ_ERR_INVALID_ARG;
+  int rc = sq_lsh_prepare(c, sig, H, bands, rows, bucket_cap, nullptr);
+  if (rc != SQ_OK) return rc;
+  return sq_lsh_emit_range(c, 0, c->n, flags, pairs_out, capacity, n_pairs);
 }
