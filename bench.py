@@ -11,6 +11,7 @@ Multi-GPU: the path partitions into independent repertoires (donors), one per ra
 data-path collective ("scaling": "weak").  `--impl reference` times the CPU oracle.
 """
 import argparse
+import hashlib
 import json
 import os
 import statistics
@@ -22,6 +23,7 @@ import numpy as np
 
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
+TRAFFIC_JSON = os.path.join(ROOT, "profiles", "traffic.json")
 
 from paper_2602_17330_b200 import datagen as dg  # noqa: E402
 from paper_2602_17330_b200 import shard  # noqa: E402
@@ -29,11 +31,13 @@ from paper_2602_17330_b200 import shard  # noqa: E402
 METRIC = "candidate_pairs_verified_per_s"
 UNIT = "pairs/s"
 ALU_OPS_PER_COLUMN_WORD = 7         # ALU-pipe logic ops of one Myers/Hyyro column step
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
-# committed `ncu --set full` capture of this very command line (profiles/r1_v42_top_config4.md)
-NCU_TRAFFIC_BYTES = {("config4", 10_000_000, "edit_distance"): 54.67e9 + 3.49e9}
-# bounded oracle samples (first n_s sequences of the same workload)
-ORACLE_SAMPLE = {"config1": 2000, "config2": 100_000, "config3": 300_000, "config4": 300_000}
+SAD_OPS_PER_FILTER_CELL = 5         # byte-wise SAD instructions per cell of the bag filter (20 residues)
+# dram bytes per launch of the dominant kernel come from the committed `ncu --set full` summary
+# profiles/traffic.json, which names the sha256 of the kernel sources it was captured on: a build
+# from other sources reports "traffic": null instead of a stale number
+# bounded oracle samples: whole clonal families (so that candidates per sequence stay those of the full
+# workload), about this many sequences
+ORACLE_SAMPLE = {"config1": 2000, "config2": 100_000, "config3": 150_000, "config4": 60_000, "config5": 2000}
 CAP_PER_SEQ = {"config2": 40, "config3": 60, "config4": 200}
 
 
@@ -49,6 +53,54 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
+
+
+def kernel_source_sha():
+    """sha256 over the CUDA sources of libsubquad.so (what an ncu capture is valid for)"""
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2602_17330_b200", "csrc")
+    for name in sorted(os.listdir(d)):
+        if name.endswith((".cu", ".cuh")):
+            with open(os.path.join(d, name), "rb") as f:
+                h.update(name.encode() + b"\0" + f.read())
+    return h.hexdigest()
+
+
+def captured_traffic(workload, n, kernel_class):
+    """(bytes per launch, source) from profiles/traffic.json if it was captured on these very
+    kernel sources for this workload and kernel class, else (None, why)."""
+    try:
+        with open(TRAFFIC_JSON) as f:
+            t = json.load(f)
+    except Exception:
+        return None, "no profiles/traffic.json"
+    if t.get("kernel_source_sha256") != kernel_source_sha():
+        return None, "profiles/traffic.json was captured on other kernel sources"
+    for e in t.get("entries", []):
+        if e.get("workload") == workload and e.get("n") == n and e.get("kernel_class") == kernel_class:
+            return float(e["dram_bytes_per_launch"]), e.get("capture", "profiles/traffic.json")
+    return None, "no entry for this workload / kernel in profiles/traffic.json"
+
+
+def cpu_model():
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    return "unknown"
+
+
+def spawn_ranks(args):
+    """`python bench.py --gpus N` without a launcher: start the N ranks ourselves (one process per
+    GPU, torch.distributed.run on this node) and hand their output through."""
+    import socket
+    s = socket.socket(); s.bind(("127.0.0.1", 0)); port = s.getsockname()[1]; s.close()
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
 
 
 def measured_peaks():
@@ -131,8 +183,11 @@ def make_repertoire(workload, n, rank):
 # ---------------------------------------------------------------------------------------------
 # reference arm / cpu_baseline: the oracle as it stands, on a bounded sample
 # ---------------------------------------------------------------------------------------------
-def oracle_step(rep_sample, P):
+def oracle_step(rep_sample, P, threads=None):
+    """one pass of the oracle over a repertoire: (pairs, seconds per stage, cells)"""
     import oracle
+    if threads is not None:
+        oracle.set_num_threads(threads)
     t0 = time.perf_counter()
     sig = oracle.minhash(rep_sample.seqs, rep_sample.offsets, P["k"], P["H"], dg.DEFAULT_SEED64)
     t1 = time.perf_counter()
@@ -142,62 +197,141 @@ def oracle_step(rep_sample, P):
     t3 = time.perf_counter()
     L = rep_sample.lengths
     cells = float((L[pairs[:, 0]].astype(np.float64) * L[pairs[:, 1]]).sum()) if pairs.size else 0.0
-    return {"pairs": int(pairs.shape[0]), "t": t3 - t0, "t_minhash": t1 - t0, "t_lsh": t2 - t1,
-            "t_edit": t3 - t2, "cells": cells, "hits": int((dist <= P["max_d"]).sum())}
+    return {"pairs": int(pairs.shape[0]), "raw": int(raw), "t": t3 - t0, "t_minhash": t1 - t0, "t_lsh": t2 - t1,
+            "t_edit": t3 - t2, "cells": cells, "hits": int((dist <= P["max_d"]).sum()), "pair_list": pairs}
+
+
+def subset(rep, idx):
+    """the sequences `idx` (ascending) of a repertoire, as a repertoire of their own"""
+    lens = rep.lengths[idx]
+    offs = np.zeros(idx.size + 1, np.int64)
+    np.cumsum(lens, out=offs[1:])
+    src = np.repeat(rep.offsets[idx] - offs[:-1], lens) + np.arange(int(offs[-1]), dtype=np.int64)
+    return dg.Repertoire(rep.seqs[src], offs, rep.family[idx], rep.n_edits[idx], rep.name)
 
 
 def sample_of(rep, n_s):
+    """About n_s sequences: WHOLE clonal families (family ids 0, 1, ... in the generator's order, every
+    member wherever the final permutation put it), so that the sample has the candidate density of
+    the full workload; a plain prefix when the repertoire has no families."""
     n_s = min(n_s, rep.n)
-    end = int(rep.offsets[n_s])
-    return dg.Repertoire(rep.seqs[:end], rep.offsets[:n_s + 1].copy(), rep.family[:n_s],
-                         rep.n_edits[:n_s], rep.name)
+    if rep.n == n_s or rep.family.size == 0 or int(rep.family.min()) < 0:
+        return subset(rep, np.arange(n_s)), f"first {n_s} sequences"
+    sizes = np.bincount(rep.family)
+    nf = int(np.searchsorted(np.cumsum(sizes), n_s)) + 1
+    idx = np.nonzero(rep.family < nf)[0]
+    return subset(rep, idx), f"all {idx.size} members of the first {nf} clonal families"
 
 
 def cpu_baseline(rep, workload, P):
+    """The oracle as it stands on this box's host cores, on a bounded sample of the same workload:
+    all cores (OpenMP over independent items; the sort of the LSH stage is single-threaded) and one
+    core.  A reported baseline, not a target."""
     import oracle
-    n_s = ORACLE_SAMPLE[workload]
-    s = sample_of(rep, n_s)
+    cores = oracle.num_threads()
+    s, what = sample_of(rep, ORACLE_SAMPLE[workload])
     r = oracle_step(s, P)
-    return {"value": r["pairs"] / r["t"], "unit": UNIT, "cores": oracle.num_threads(),
-            "kind": "oracle",
-            "sample": f"first {s.n} sequences of {workload} (of {rep.n}); {r['pairs']} candidate "
-                      f"pairs in {r['t']:.2f} s (minhash {r['t_minhash']:.2f} s, lsh "
-                      f"{r['t_lsh']:.2f} s single-thread qsort, edit {r['t_edit']:.2f} s)",
+    pl = r.pop("pair_list")
+    # one thread: the two parallel stages again (the LSH stage is single-threaded anyway)
+    oracle.set_num_threads(1)
+    t0 = time.perf_counter()
+    oracle.minhash(s.seqs, s.offsets, P["k"], P["H"], dg.DEFAULT_SEED64)
+    t1 = time.perf_counter()
+    oracle.edit_distance_pairs(s.seqs, s.offsets, pl, P["max_d"])
+    t2 = time.perf_counter()
+    oracle.set_num_threads(cores)
+    t_single = (t1 - t0) + r["t_lsh"] + (t2 - t1)
+    return {"value": r["pairs"] / r["t"], "unit": UNIT, "cores": cores, "kind": "oracle",
+            "cpu_model": cpu_model(),
+            "sample": f"{what} of {workload} (of {rep.n}); {r['pairs']} candidate pairs "
+                      f"({r['pairs'] / max(s.n, 1):.1f} per sequence, {r['raw']} before dedupe) in {r['t']:.2f} s "
+                      f"(minhash {r['t_minhash']:.2f} s, lsh {r['t_lsh']:.2f} s single-thread qsort, "
+                      f"edit {r['t_edit']:.2f} s)",
             "minhash_seqs_per_s": s.n / max(r["t_minhash"], 1e-9),
-            "edit_gcups": r["cells"] / max(r["t_edit"], 1e-9) / 1e9}
+            "lsh_candidate_pairs_per_s": r["pairs"] / max(r["t_lsh"], 1e-9),
+            "edit_gcups": r["cells"] / max(r["t_edit"], 1e-9) / 1e9,
+            "single_thread": {"value": r["pairs"] / t_single, "unit": UNIT,
+                              "minhash_seqs_per_s": s.n / max(t1 - t0, 1e-9),
+                              "edit_gcups": r["cells"] / max(t2 - t1, 1e-9) / 1e9}}
+
+
+def all_pairs_oracle(rep, P):
+    """oracle on the all-pairs block of the first 2,000 sequences: seconds, pairs, cells"""
+    import oracle
+    s, what = sample_of(rep, ORACLE_SAMPLE["config1"])
+    L = s.lengths.astype(np.float64)
+    cells = (L.sum() ** 2 - (L ** 2).sum()) / 2
+    npairs = s.n * (s.n - 1) // 2
+    t0 = time.perf_counter()
+    if P["max_d"] < 0:
+        oracle.all_pairs_full(s.seqs, s.offsets)
+    else:
+        oracle.all_pairs_threshold(s.seqs, s.offsets, P["max_d"], use_cutoff=False)
+    return time.perf_counter() - t0, npairs, cells, s, what
+
+
+def cpu_baseline_all_pairs(rep, workload, P):
+    import oracle
+    cores = oracle.num_threads()
+    t, npairs, cells, s, what = all_pairs_oracle(rep, P)
+    oracle.set_num_threads(1)
+    sub1 = subset(s, np.arange(min(s.n, 500)))
+    t1, np1, cells1, _, _ = all_pairs_oracle(sub1, P)
+    oracle.set_num_threads(cores)
+    return {"value": npairs / t, "unit": UNIT, "cores": cores, "kind": "oracle", "cpu_model": cpu_model(),
+            "sample": f"all-pairs block of the {what} of {workload} (of {rep.n}): {npairs} pairs, plain "
+                      f"Wagner-Fischer, in {t:.2f} s",
+            "gcups": cells / t / 1e9,
+            "single_thread": {"value": np1 / t1, "unit": UNIT, "gcups": cells1 / t1 / 1e9,
+                              "sample": f"first {sub1.n} sequences"}}
 
 
 def run_reference(args):
+    """--impl reference: there is no reference implementation (PAPER.md only); the base contract's
+    reference arm is the oracle, as it stands, on the host cores, on a bounded sample per step."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     import oracle
+    world = int(os.environ.get("WORLD_SIZE", "1"))
     workload = args.workload
-    if workload in ("config1", "config5"):
-        print(json.dumps({"impl": "reference", "unavailable": "the reference arm times the LSH path "
-                          "(configs 2-4); the all-pairs oracle is exercised by tests/ only"}))
-        return
     P = dg.PARAMS[workload]
-    n_s = min(ORACLE_SAMPLE[workload], 100_000)
-    rep = dg.GENERATORS[workload](n_s, seed=0)
-    for _ in range(args.warmup):
-        oracle_step(rep, P)
-    ts, pairs = [], 0
-    for _ in range(args.steps):
-        r = oracle_step(rep, P)
-        ts.append(r["t"]); pairs = r["pairs"]
-    t = sum(ts)
-    value = pairs * args.steps / t
+    cores = oracle.num_threads()
+    if workload in ("config1", "config5"):
+        rep = dg.GENERATORS[workload](ORACLE_SAMPLE[workload], seed=0)
+        for _ in range(min(args.warmup, 1)):
+            all_pairs_oracle(rep, P)
+        ts = []
+        for _ in range(args.steps):
+            t, npairs, cells, s, what = all_pairs_oracle(rep, P)
+            ts.append(t)
+        t = sum(ts)
+        value = npairs * args.steps / t
+        metric = "all_pairs_evaluated_per_s"
+        sample = f"{workload} generator at n={rep.n}: {npairs} pairs per step, plain Wagner-Fischer"
+        cfg = {"workload": f"{workload} generator at n={rep.n} (bounded oracle sample)", "max_d": P["max_d"]}
+    else:
+        n_s = min(ORACLE_SAMPLE[workload], 60_000)
+        rep = dg.GENERATORS[workload](n_s, seed=0)
+        for _ in range(min(args.warmup, 1)):
+            oracle_step(rep, P)
+        ts, pairs = [], 0
+        for _ in range(args.steps):
+            r = oracle_step(rep, P)
+            ts.append(r["t"]); pairs = r["pairs"]
+        t = sum(ts)
+        value = pairs * args.steps / t
+        metric = METRIC
+        sample = f"{workload} generator at n={n_s}, {pairs} pairs per step"
+        cfg = {"workload": f"{workload} generator at n={n_s} (bounded oracle sample)",
+               **{k: P[k] for k in ("k", "H", "bands", "rows", "cap", "max_d")}}
     line = {
-        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps,
+        "impl": "reference", "metric": metric, "value": value, "unit": UNIT, "n_gpus": world,
+        "ranks_that_computed": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u32/u64 integer",
-        "data": "synthetic", "gpu_launches": 0,
-        "config": {"workload": f"{workload} generator at n={n_s} (bounded oracle sample)",
-                   **{k: P[k] for k in ("k", "H", "bands", "rows", "cap", "max_d")}},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(),
-                         "kind": "oracle",
-                         "sample": f"{workload} generator at n={n_s}, {pairs} pairs per step"},
+        "data": "synthetic", "gpu_launches": 0, "config": cfg,
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "cpu_model": cpu_model(),
+                         "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }
     print(json.dumps(line))
@@ -524,9 +658,7 @@ def run_ours(args):
         roof = {"kernel": dom, "bound": "hbm", "achieved": kd.get("achieved_GBs"), "peak": hbm_peak,
                 "unit": "GB/s", "frac": kd.get("frac"), "traffic": None, "peak_source": peak_src}
     roof["avg_launch_ms"] = kd["ms_per_step"] / max(kd["launches_per_step"], 1)
-    roof["traffic"] = NCU_TRAFFIC_BYTES.get((workload, n, dom))
-    if roof["traffic"] is not None:
-        roof["traffic_source"] = "profiles/r1_v42_top_config4.md (ncu --set full, bytes per launch)"
+    roof["traffic"], roof["traffic_source"] = captured_traffic(workload, n, dom)
 
     cpu = None if args.no_cpu_baseline else cpu_baseline(rep, workload, P)
     line = {
@@ -615,12 +747,85 @@ def run_all_pairs(args):
     L = rep.lengths.astype(np.float64)
     cells = (L.sum() ** 2 - (L ** 2).sum()) / 2
     step_ms_all, tot = shard.aggregate(step_ms, {"pairs": npairs, "cells": cells}, dev)
+    survivors = sq.last_raw_pairs() if P["max_d"] >= 0 else npairs
+
+    # ---- e2e: the same through HOST buffers (pinned): H2D of sequences + offsets, pack, all pairs,
+    # D2H of the results, all inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        seqs_h = torch.from_numpy(rep.seqs).pin_memory()
+        offs_h = torch.from_numpy(rep.offsets).pin_memory()
+        n_out = int(cnt)
+        dist_h = torch.empty(max(n_out, 1), dtype=torch.int16).pin_memory()
+        pairs_h = torch.empty((max(n_out, 1), 2), dtype=torch.int32).pin_memory() if pairs is not None else None
+
+        def host_step():
+            sd = seqs_h.to(dev, non_blocking=True)
+            od = offs_h.to(dev, non_blocking=True)
+            sq.pack(sd, od, 20, max_len)
+            c = sq.all_pairs(P["max_d"], pairs, dist_out)
+            dist_h[:c].copy_(dist_out[:c], non_blocking=True)
+            if pairs_h is not None:
+                pairs_h[:c].copy_(pairs[:c], non_blocking=True)
+            torch.cuda.synchronize()
+            return c
+        host_step()
+        e2e_steps = max(1, min(args.steps, 5))
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            c3 = host_step()
+        te = (time.perf_counter() - t0) / e2e_steps
+        assert c3 == cnt
+        te_ms, _ = shard.aggregate(1e3 * te, {}, dev)
+        e2e = {"value": tot["pairs"] / (te_ms * 1e-3), "unit": UNIT,
+               "h2d_bytes_per_step": total_len + 8 * (n + 1),
+               "d2h_bytes_per_step": n_out * (2 if pairs_h is None else 10), "ms_per_step": te_ms,
+               "steps": e2e_steps,
+               "api": "pinned host tensors -> sq_pack -> sq_all_pairs -> pinned host tensors (copies timed)"}
     if rank != 0:
         return
     K = args.steps
-    kernels = {k: {"ms_per_step": ms / K, "launches_per_step": ln / K} for k, (ms, ln) in prof.items() if ln}
-    dom = max(kernels, key=lambda q: kernels[q]["ms_per_step"])
+    words = (max_len + 31) // 32
     lop3 = sq.int_peak(0, 2048)
+    sad = sq.int_peak(7, 2048)
+    kernels = {k: {"ms_per_step": ms / K, "launches_per_step": ln / K} for k, (ms, ln) in prof.items() if ln}
+    Ls = rep.lengths.astype(np.float64)
+    if P["max_d"] < 0:
+        # fused tile kernel: every pair i < j runs every column of its text j (the row i is the pattern)
+        text_cols = float((Ls * np.arange(n)).sum())            # sequence j is the text of j pairs
+        k = kernels["all_pairs"]
+        ops = ALU_OPS_PER_COLUMN_WORD * text_cols * words
+        k.update(bound="alu", achieved_Gops=ops / (k["ms_per_step"] * 1e-3) / 1e9)
+        k["frac"] = k["achieved_Gops"] * 1e9 / lop3
+        roof = {"kernel": "all_pairs", "bound": "alu", "achieved": k["achieved_Gops"], "peak": lop3 / 1e9,
+                "unit": "Gop/s", "frac": k["frac"], "peak_source": "sq_int_peak LOP3 stream measured in this run",
+                "ops": f"{ALU_OPS_PER_COLUMN_WORD} logic ops x text columns x {words} word(s) per pair (DESIGN.md 5)"}
+        cells_computed = cells
+    else:
+        # two kernels: the bag-distance filter over all cells (SAD instructions) and the banded DP on
+        # its survivors (window of NWIN words per column)
+        nwin = 2 if P["max_d"] <= 16 else 3
+        kf = kernels["all_pairs"]
+        f_ops = SAD_OPS_PER_FILTER_CELL * float(npairs)
+        kf.update(bound="alu", achieved_Gops=f_ops / (kf["ms_per_step"] * 1e-3) / 1e9)
+        kf["frac"] = kf["achieved_Gops"] * 1e9 / sad
+        kf["peak"] = "sq_int_peak vabsdiff4 stream (%.0f Gop/s)" % (sad / 1e9)
+        mean_len = float(Ls.mean())
+        cells_computed = survivors * mean_len * 32.0 * nwin        # band cells of the survivors' DP
+        if "edit_distance" in kernels:
+            kd = kernels["edit_distance"]
+            d_ops = ALU_OPS_PER_COLUMN_WORD * survivors * mean_len * nwin
+            kd.update(bound="alu", achieved_Gops=d_ops / (kd["ms_per_step"] * 1e-3) / 1e9,
+                      columns="survivors x mean text length (the survivor list is not returned)")
+            kd["frac"] = kd["achieved_Gops"] * 1e9 / lop3
+        roof = {"kernel": "all_pairs (bag-distance filter)", "bound": "alu", "achieved": kf["achieved_Gops"],
+                "peak": sad / 1e9, "unit": "Gop/s", "frac": kf["frac"],
+                "peak_source": "sq_int_peak vabsdiff4 stream measured in this run",
+                "ops": f"{SAD_OPS_PER_FILTER_CELL} byte-wise SAD instructions per cell i<j (DESIGN.md 5)"}
+    dom = max(kernels, key=lambda q: kernels[q]["ms_per_step"])
+    roof["avg_launch_ms"] = kernels["all_pairs"]["ms_per_step"] / max(kernels["all_pairs"]["launches_per_step"], 1)
+    roof["traffic"], roof["traffic_source"] = captured_traffic(workload, n, "all_pairs")
+    cpu = None if args.no_cpu_baseline else cpu_baseline_all_pairs(rep, workload, P)
     line = {
         "metric": "all_pairs_evaluated_per_s", "value": tot["pairs"] / (step_ms_all * 1e-3), "unit": UNIT,
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": step_ms_all,
@@ -629,19 +834,22 @@ def run_all_pairs(args):
         "config": {"workload": f"{workload}: exhaustive tile path over N={n} sequences "
                                f"(BASELINE.json configs[{int(workload[-1]) - 1}])",
                    "max_d": P["max_d"], "max_len": max_len, "outputs": int(cnt),
+                   "filter_survivors": int(survivors),
                    "timing": "CUDA events per step; 256 MB L2 flush between timed steps"},
-        "stages": {"gcups_full_matrix_equivalent": tot["cells"] / (step_ms_all * 1e-3) / 1e9},
-        "roofline": {"kernel": dom, "bound": "alu", "achieved": None, "peak": lop3 / 1e9, "unit": "Gop/s",
-                     "frac": None, "traffic": None,
-                     "note": "thresholded: most pairs end in the bag-distance filter (8 SAD ops), "
-                             "so ops per pair are data dependent; see DESIGN.md 5"},
-        "kernels": kernels, "cpu_baseline": None, "e2e": None, "gpu_launches": launches, "clocks": clocks,
+        "stages": {"gcups_full_matrix_equivalent": tot["cells"] / (step_ms_all * 1e-3) / 1e9,
+                   "gcups_cells_actually_computed": cells_computed / (step_ms * 1e-3) / 1e9,
+                   "cells_full_matrix": cells, "cells_actually_computed": cells_computed},
+        "roofline": roof, "dominant_class": dom, "kernels": kernels,
+        "int_peak_ops_per_s": {"lop3": lop3, "vabsdiff4": sad},
+        "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
     }
     print(json.dumps(line))
 
 
 def main():
     args = parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl != "reference":
+        sys.exit(spawn_ranks(args))          # no launcher: start one rank per GPU ourselves
     if args.impl == "reference":
         run_reference(args)
     elif args.workload in ("config1", "config5"):

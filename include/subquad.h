@@ -285,7 +285,8 @@ int  sq_set_option(sq_ctx* ctx, int option, int64_t value);
 /* Introspection (host values, valid after the call they describe). */
 int64_t sq_packed_n(const sq_ctx* ctx);          /* n of the current pack, -1 if none        */
 int     sq_packed_stride(const sq_ctx* ctx);     /* slot stride in bytes                     */
-int64_t sq_last_raw_pairs(const sq_ctx* ctx);    /* pairs before cross-band dedupe (last LSH) */
+int64_t sq_last_raw_pairs(const sq_ctx* ctx);    /* pairs before cross-band dedupe (last LSH); after a
+                                                    thresholded sq_all_pairs: survivors of its bag filter */
 int64_t sq_kernel_launches(const sq_ctx* ctx);   /* kernels launched by this context so far  */
 const char* sq_last_cuda_error(const sq_ctx* ctx);
 const char* sq_strerror(int code);
@@ -303,7 +304,8 @@ const char* sq_profile_name(int kernel_class);   /* NULL past the last class */
 /* Integer-pipe micro-benchmark (roofline denominator for the DP stage):
  * runs `iters` dependent-free instructions of `kind` per thread on a full grid and returns
  * achieved lane-operations per second in *ops_per_s (host).
- * kind: 0 LOP3, 1 IADD3, 2 SHF, 3 IMAD, 4 min.u32, 5 LOP3+IMAD mix, 6 POPC. */
+ * kind: 0 LOP3, 1 IADD3, 2 SHF, 3 IMAD, 4 min.u32, 5 LOP3+IMAD mix, 6 POPC, 7 byte-wise sum of
+ * absolute differences (vabsdiff4 ... add; the instruction of the bag-distance filter). */
 int  sq_int_peak(sq_ctx* ctx, int kind, int iters, double* ops_per_s);
 
 #ifdef __cplusplus

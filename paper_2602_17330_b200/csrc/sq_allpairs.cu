@@ -249,6 +249,7 @@ extern "C" int sq_all_pairs(sq_ctx* c, int max_d, uint32_t* pairs_out, uint16_t*
       SQ_CUDA(c, cudaMemcpyAsync(c->pinned, c->dflags + 1, 8, cudaMemcpyDeviceToHost, st));
       SQ_CUDA(c, cudaStreamSynchronize(st));
       const int64_t ns = (int64_t)c->pinned[0];
+      c->last_raw_pairs = ns;                    // survivors of the filter (sq_last_raw_pairs)
       if ((size_t)ns <= scap) {
         filtered = true;
         if (ns > 0) {

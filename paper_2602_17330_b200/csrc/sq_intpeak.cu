@@ -28,6 +28,7 @@ int_peak_kernel(int iters, uint32_t seed, uint32_t* __restrict__ sink) {
           else asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(r[q]) : "r"(k1), "r"(k2));
         }
         if (KIND == 6) asm volatile("popc.b32 %0, %0;" : "+r"(r[q]));
+        if (KIND == 7) asm volatile("vabsdiff4.u32.u32.u32.add %0, %0, %1, %2;" : "+r"(r[q]) : "r"(k1), "r"(k2));
       }
     }
   }
@@ -40,7 +41,7 @@ int_peak_kernel(int iters, uint32_t seed, uint32_t* __restrict__ sink) {
 }  // namespace
 
 extern "C" int sq_int_peak(sq_ctx* c, int kind, int iters, double* ops_per_s) {
-  if (!c || !ops_per_s || iters < 1 || kind < 0 || kind > 6) return SQ_ERR_INVALID_ARG;
+  if (!c || !ops_per_s || iters < 1 || kind < 0 || kind > 7) return SQ_ERR_INVALID_ARG;
   if (!c->ws) return SQ_ERR_WORKSPACE;
   SqDeviceGuard guard(c);
   // 256 words of the free scratch (handed back at once: the kernels practically never write them)
@@ -62,7 +63,8 @@ extern "C" int sq_int_peak(sq_ctx* c, int kind, int iters, double* ops_per_s) {
       case 3: int_peak_kernel<3><<<blocks, 256, 0, c->stream>>>(iters, 12345u + rep, sink); break;
       case 4: int_peak_kernel<4><<<blocks, 256, 0, c->stream>>>(iters, 12345u + rep, sink); break;
       case 5: int_peak_kernel<5><<<blocks, 256, 0, c->stream>>>(iters, 12345u + rep, sink); break;
-      default: int_peak_kernel<6><<<blocks, 256, 0, c->stream>>>(iters, 12345u + rep, sink); break;
+      case 6: int_peak_kernel<6><<<blocks, 256, 0, c->stream>>>(iters, 12345u + rep, sink); break;
+      default: int_peak_kernel<7><<<blocks, 256, 0, c->stream>>>(iters, 12345u + rep, sink); break;
     }
     c->launches++;
     cudaEventRecord(e1, c->stream);
