@@ -647,10 +647,12 @@ emit_fill_masks_kernel(const uint2* __restrict__ units, const uint32_t* __restri
                        const uint32_t* __restrict__ ids, const uint32_t* __restrict__ ids_int,
                        uint32_t n2, int bands, const uint32_t* __restrict__ cnt_off,
                        uint32_t* __restrict__ outJ, uint2* __restrict__ loc) {
+  __shared__ uint32_t idt_sm[kEmWarps][32];
   const uint32_t lane = threadIdx.x & 31;
   const uint32_t nw = gridDim.x * kEmWarps;
   uint32_t u = blockIdx.x * kEmWarps + (threadIdx.x >> 5);
   if (u >= nunits) return;
+  uint32_t* idt = idt_sm[threadIdx.x >> 5];
   struct L1 { uint2 un; uint32_t tb; };
   struct L2 { uint32_t idx, idi, msk, acc, nxt; };
   auto load1 = [&](uint32_t uu) -> L1 {              // needs only the unit index
@@ -697,14 +699,15 @@ emit_fill_masks_kernel(const uint2* __restrict__ units, const uint32_t* __restri
         mask_n = mp[(size_t)(c0 + 32)];              // (c0+32)/32 tiles further = (c0+32) words
         if (c0 + 32 + lane < mrem) idc_n = idp[c0 + 32 + lane];
       }
-      while (__any_sync(kFull, mask != 0u)) {
-        const int c = mask ? __ffs(mask) - 1 : 0;
-        const uint32_t j = __shfl_sync(kFull, idc, c);
-        if (mask) {
-          outJ[acc] = j;
-          ++acc;
-          mask &= mask - 1;
-        }
+      // the tile's 32 column ids go through shared memory; every lane then walks its own bits (no
+      // vote, no shuffle per partner: the loop is divergent, but it is half the instructions)
+      __syncwarp();
+      idt[lane] = idc;
+      __syncwarp();
+      while (mask) {
+        const int c = __ffs(mask) - 1;
+        mask &= mask - 1;
+        outJ[acc++] = idt[c];
       }
       mask = mask_n; idc = idc_n;
     }
