@@ -16,7 +16,7 @@ int sq_create(sq_ctx** out, int device, void* cuda_stream) {
   c->device = device;
   c->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
   cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
-  if (cudaHostAlloc(reinterpret_cast<void**>(&c->pinned), 8 * sizeof(unsigned long long),
+  if (cudaHostAlloc(reinterpret_cast<void**>(&c->pinned), 16 * sizeof(unsigned long long),
                     cudaHostAllocDefault) != cudaSuccess) {
     delete c;
     return SQ_ERR_CUDA;

@@ -53,9 +53,9 @@ struct sq_ctx {
     int bands = 0, bw = 0;
     uint32_t *vin = nullptr, *vint = nullptr, *S = nullptr, *cnt = nullptr, *ubase = nullptr;
     uint32_t *rowidx = nullptr, *ext_off = nullptr, *rowstart = nullptr, *active = nullptr;
-    uint2 *loc = nullptr, *units = nullptr, *units0 = nullptr;
+    uint2 *loc = nullptr, *units = nullptr, *units0 = nullptr, *units_s = nullptr;
     uint8_t* tmp = nullptr;
-    uint32_t nunits = 0, nunits0 = 0;
+    uint32_t nunits = 0, nunits0 = 0, nsmall = 0;
     unsigned long long ntiles = 0;
     size_t mark = 0;
   } lsh;
@@ -66,8 +66,8 @@ struct sq_ctx {
   int64_t launches = 0;
   int64_t last_raw_pairs = 0;
   cudaError_t last_err = cudaSuccess;
-  unsigned long long* pinned = nullptr;   // 8 pinned host words for count / flag read-back
-  unsigned long long* dflags = nullptr;   // 8 device words (lives at the start of the workspace)
+  unsigned long long* pinned = nullptr;   // 16 pinned host words for count / flag read-back
+  unsigned long long* dflags = nullptr;   // 16 device words (lives at the start of the workspace)
   // per-kernel-class CUDA-event timer (off by default)
   bool prof_on = false;
   cudaEvent_t* prof_ev = nullptr;         // 2 * kSqProfSlots events, created on first enable

@@ -285,16 +285,21 @@ s_prefill_kernel(uint32_t* __restrict__ S, int64_t n2, int SW) {
 // units: (global sorted position of the unit's first row, kept members from there to the end
 // of the bucket); band 0's units go to their own list units0 (they need no compares).
 // ubase[u] = index of unit u's first 32-word tile in the mask cache (bands >= 1).
-// counters: [1] raw pairs, [4] units of bands >= 1, [5] units of band 0, [7] mask tiles.
+// counters: [1] raw pairs, [4] units of bands >= 1, [5] units of band 0, [7] mask tiles, [8] small units.
+// A bucket of bands >= 1 with at most kSmallMax kept members is ONE small unit (list units_s): it is
+// handled by a single thread (small_units_kernel), not by a warp, and has no mask tiles -- three
+// quarters of all units are of this kind and hold under 1 % of the pairs.
+constexpr int kSmallMax = 8;
+
 __global__ void __launch_bounds__(kBsThreads)
 bucket_scan_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict__ ids, int64_t n2,
                    int cap, int SW, uint32_t* __restrict__ S, uint2* __restrict__ units,
-                   uint2* __restrict__ units0, uint32_t* __restrict__ ubase,
+                   uint2* __restrict__ units0, uint2* __restrict__ units_s, uint32_t* __restrict__ ubase,
                    unsigned long long* __restrict__ counters) {
   __shared__ int sh_w[kBsThreads / 32];
   __shared__ int sh_carry_head, sh_carry_end;
   __shared__ unsigned long long sh_raw;
-  __shared__ uint32_t sh_unit_base, sh_unit_cnt, sh_tile_cnt;
+  __shared__ uint32_t sh_unit_base, sh_unit_cnt, sh_tile_cnt, sh_small_base, sh_small_cnt;
   __shared__ unsigned long long sh_tile_base;
   const int band = blockIdx.y;
   const uint64_t* __restrict__ k = keys + (int64_t)band * n2;
@@ -303,7 +308,7 @@ bucket_scan_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict
   const int64_t tile_end = min(n2, tile0 + kBsTile);             // exclusive
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int64_t p0 = tile0 + (int64_t)threadIdx.x * kBsItems;
-  if (threadIdx.x == 0) { sh_raw = 0ull; sh_unit_cnt = 0u; sh_tile_cnt = 0u; }
+  if (threadIdx.x == 0) { sh_raw = 0ull; sh_unit_cnt = 0u; sh_tile_cnt = 0u; sh_small_cnt = 0u; }
 
   uint64_t kk[kBsItems];
   bool valid[kBsItems], head[kBsItems], tail[kBsItems];
@@ -377,10 +382,11 @@ bucket_scan_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict
   unsigned long long raw = 0;
   uint32_t nunit = 0;
   uint2 unit[kBsItems];
-  bool has_unit[kBsItems];
+  bool has_unit[kBsItems], is_small[kBsItems];
+  uint32_t nsmall = 0;
 #pragma unroll
   for (int t = 0; t < kBsItems; ++t) {
-    has_unit[t] = false;
+    has_unit[t] = false; is_small[t] = false;
     if (!valid[t]) continue;
     const uint32_t id = idb[p0 + t];
     const int r = (int)(p0 + t) - hpos[t];
@@ -393,9 +399,9 @@ bucket_scan_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict
     if (kept) {
       raw += (unsigned long long)(m - 1 - r);
       if ((r & 31) == 0 && r + 1 < m) {
-        has_unit[t] = true;
-        ++nunit;
         unit[t] = make_uint2((uint32_t)((int64_t)band * n2 + p0 + t), (uint32_t)(m - r));
+        if (band != 0 && m <= kSmallMax) { is_small[t] = true; ++nsmall; }      // (then r == 0)
+        else { has_unit[t] = true; ++nunit; }
       }
     }
   }
@@ -404,6 +410,8 @@ bucket_scan_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict
 #pragma unroll
   for (int t = 0; t < kBsItems; ++t) if (has_unit[t]) ntiles += (unit[t].y + 31u) >> 5;
   if (nunit) { my = atomicAdd(&sh_unit_cnt, nunit); my_tiles = atomicAdd(&sh_tile_cnt, ntiles); }
+  uint32_t my_small = 0;
+  if (nsmall) my_small = atomicAdd(&sh_small_cnt, nsmall);
 #pragma unroll
   for (int d = 16; d > 0; d >>= 1) raw += __shfl_xor_sync(kFull, raw, d);
   if (lane == 0 && raw) atomicAdd(&sh_raw, raw);
@@ -413,6 +421,7 @@ bucket_scan_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict
       sh_unit_base = (uint32_t)atomicAdd(counters + (band == 0 ? 5 : 4), (unsigned long long)sh_unit_cnt);
     if (sh_raw) atomicAdd(counters + 1, sh_raw);
     if (band != 0 && sh_tile_cnt) sh_tile_base = atomicAdd(counters + 7, (unsigned long long)sh_tile_cnt);
+    if (sh_small_cnt) sh_small_base = (uint32_t)atomicAdd(counters + 8, (unsigned long long)sh_small_cnt);
   }
   __syncthreads();
   uint2* __restrict__ ulist = band == 0 ? units0 : units;
@@ -425,6 +434,10 @@ bucket_scan_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict
       ulist[q++] = unit[t];
     }
   }
+  uint32_t qs = sh_small_base + my_small;
+#pragma unroll
+  for (int t = 0; t < kBsItems; ++t)
+    if (is_small[t]) units_s[qs++] = unit[t];
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -481,7 +494,37 @@ __device__ __forceinline__ void sweep_tile(const uint32_t* __restrict__ sm,
                                            bool rowok, uint32_t myid, uint32_t& acc,
                                            uint32_t& tmask, uint32_t* __restrict__ outJ) {
   constexpr int RS = 4 * BW + 4;
-  if constexpr (NCH <= BW) {
+  if constexpr (NCH <= BW && MODE == EM_COUNT) {
+    // Count pass.  Per column and chunk of four earlier bands: one broadcast LDS.128, four chained
+    // ISETP.NE.AND and one SEL that keeps the column's bit while every band differs -- written as PTX
+    // so that the predicate chain survives the compiler.  The row's validity and the triangle of the
+    // unit's first tile (row l pairs with columns > l only) are applied ONCE per tile.
+    auto keep = [&](uint32_t c, uint32_t bit) -> uint32_t {       // bit if (row, column c) is new, else 0
+#pragma unroll
+      for (int ch = 0; ch < NCH; ++ch) {
+        const uint4 v = *reinterpret_cast<const uint4*>(sm + c * RS + 4 * ch);   // broadcast
+        asm("{\n\t.reg .pred p;\n\t"
+            "setp.ne.u32 p, %1, %5;\n\t"
+            "setp.ne.and.u32 p, %2, %6, p;\n\t"
+            "setp.ne.and.u32 p, %3, %7, p;\n\t"
+            "setp.ne.and.u32 p, %4, %8, p;\n\t"
+            "selp.u32 %0, %0, 0, p;\n\t}"
+            : "+r"(bit)
+            : "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w), "r"(R[ch].x), "r"(R[ch].y), "r"(R[ch].z), "r"(R[ch].w));
+      }
+      return bit;
+    };
+    uint32_t tm = 0u, c = 0u;
+#pragma unroll 1
+    for (; c + 4 <= ncol; c += 4) {
+      const uint32_t m4 = keep(c, 1u) | keep(c + 1, 2u) | keep(c + 2, 4u) | keep(c + 3, 8u);
+      tm |= m4 << c;
+    }
+    for (; c < ncol; ++c) tm |= keep(c, 1u) << c;
+    if (c0 == 0) tm &= lane < 31u ? (0xFFFFFFFEu << lane) : 0u;      // columns c > lane
+    tmask = rowok ? tm : 0u;
+    (void)cbeg;
+  } else if constexpr (NCH <= BW) {
 #pragma unroll 4
     for (uint32_t c = cbeg; c < ncol; ++c) {
       bool dup = false;
@@ -639,7 +682,7 @@ emit_kernel(const uint2* __restrict__ units, const uint32_t* __restrict__ active
 // column's id from the owning lane (SHFL) and appends it to its row's group.  A unit is a chain
 // of three dependent loads (descriptor -> ids + first mask -> output offset); the warp keeps the
 // chains of its next kFillDepth units in flight while it works on the current one.
-constexpr int kFillDepth = 5;
+constexpr int kFillDepth = 12;
 
 __global__ void __launch_bounds__(kEmWarps * 32)
 emit_fill_masks_kernel(const uint2* __restrict__ units, const uint32_t* __restrict__ active, uint32_t nunits,
@@ -717,6 +760,63 @@ emit_fill_masks_kernel(const uint2* __restrict__ units, const uint32_t* __restri
 #pragma unroll
     for (int q = 0; q + 2 < kFillDepth; ++q) b[q] = b[q + 1];
     b[kFillDepth - 2] = bn;
+  }
+}
+
+// Small units: ONE THREAD per bucket of at most kSmallMax kept members (bands >= 1).  The thread
+// walks the bucket's pairs (row r, column c > r) itself: the row's S values of the earlier bands in
+// registers, the column's read chunk by chunk; the same first-band rule as the warp kernels.  No
+// mask cache: the fill pass repeats the few compares.  MODE EM_COUNT writes cnt[g] per row record,
+// EM_FILL_J appends the partners at the scanned offsets and leaves loc[band][row].
+template <int BW, int MODE>
+__global__ void __launch_bounds__(128)
+small_units_kernel(const uint2* __restrict__ units_s, uint32_t nsmall, const uint32_t* __restrict__ ids,
+                   const uint32_t* __restrict__ ids_int, uint32_t n2, const uint32_t* __restrict__ S,
+                   uint32_t* __restrict__ cnt_off, uint32_t* __restrict__ outJ, uint2* __restrict__ loc,
+                   uint32_t row_lo, uint32_t row_hi) {
+  constexpr int SW = 4 * BW;
+  const uint32_t u = blockIdx.x * blockDim.x + threadIdx.x;
+  if (u >= nsmall) return;
+  const uint2 unit = units_s[u];
+  const uint32_t g0 = unit.x, m = unit.y;                 // m kept members, 2 <= m <= kSmallMax
+  const int b = (int)(g0 / n2);
+  const int nch = (b + 3) >> 2;
+  // the bucket's members lie in [first id, last id]: nothing to do outside the range of this call
+  if (ids[g0] >= row_hi || ids[g0 + m - 2] < row_lo) return;
+  for (uint32_t r = 0; r + 1 < m; ++r) {
+    const uint32_t ext = ids[g0 + r];
+    if (ext < row_lo || ext >= row_hi) continue;
+    const uint32_t row = ids_int[g0 + r];
+    uint4 R[BW];
+#pragma unroll
+    for (int ch = 0; ch < BW; ++ch) {
+      if (ch < nch) {
+        uint4 v = *reinterpret_cast<const uint4*>(S + (int64_t)row * SW + 4 * ch);
+        if (4 * ch + 1 >= b) v.y = kFull;                 // bands >= b never match (no S value is 0xFFFFFFFF)
+        if (4 * ch + 2 >= b) v.z = kFull;
+        if (4 * ch + 3 >= b) v.w = kFull;
+        R[ch] = v;
+      }
+    }
+    uint32_t acc = 0, first = 0;
+    if (MODE != EM_COUNT) { acc = cnt_off[g0 + r]; first = acc; }
+    for (uint32_t c = r + 1; c < m; ++c) {
+      const uint32_t col = ids_int[g0 + c];
+      bool dup = false;
+#pragma unroll
+      for (int ch = 0; ch < BW; ++ch) {
+        if (ch < nch) {
+          const uint4 v = *reinterpret_cast<const uint4*>(S + (int64_t)col * SW + 4 * ch);
+          dup |= (v.x == R[ch].x) | (v.y == R[ch].y) | (v.z == R[ch].z) | (v.w == R[ch].w);
+        }
+      }
+      if (!dup) {
+        if (MODE != EM_COUNT) outJ[acc] = ids[g0 + c];
+        ++acc;
+      }
+    }
+    if (MODE == EM_COUNT) cnt_off[g0 + r] = acc;
+    else if (acc > first) loc[(size_t)b * n2 + row] = make_uint2(first, acc - first);
   }
 }
 
@@ -978,12 +1078,37 @@ int launch_fill_masks(sq_ctx* c, const uint2* units, const uint32_t* active, uin
 // both unit lists, one mode.  `masks` (may be nullptr): the per-tile masks of new pairs, written
 // by the count pass and, when present, read by the fill pass instead of repeating the compares.
 // (active / active0 = the units of this call's row range, nullptr = all; nunits / nunits0 = their number)
+template <int BW>
+int launch_small(sq_ctx* c, int mode, const uint2* units_s, uint32_t nsmall, const uint32_t* ids,
+                 const uint32_t* ids_int, uint32_t n2, const uint32_t* S, uint32_t* cnt_off, uint32_t* outJ,
+                 uint2* loc, uint32_t row_lo, uint32_t row_hi) {
+  const unsigned g = (nsmall + 127) / 128;
+  if (mode == EM_COUNT)
+    SQ_TIMED(c, SQ_K_EMIT, small_units_kernel<BW, EM_COUNT><<<g, 128, 0, c->stream>>>(
+        units_s, nsmall, ids, ids_int, n2, S, cnt_off, outJ, loc, row_lo, row_hi));
+  else
+    SQ_TIMED(c, SQ_K_EMIT, small_units_kernel<BW, EM_FILL_J><<<g, 128, 0, c->stream>>>(
+        units_s, nsmall, ids, ids_int, n2, S, cnt_off, outJ, loc, row_lo, row_hi));
+  SQ_LAUNCH_CHECK(c);
+  return SQ_OK;
+}
+
 int dispatch_emit(sq_ctx* c, int bw, int mode, const uint2* units, const uint32_t* active, uint32_t nunits,
-                  const uint2* units0, const uint32_t* active0, uint32_t nunits0, const uint32_t* ids,
+                  const uint2* units0, const uint32_t* active0, uint32_t nunits0, const uint2* units_s,
+                  uint32_t nsmall, const uint32_t* ids,
                   const uint32_t* ids_int, uint32_t n2, int bands, const uint32_t* S,
                   uint32_t* cnt_off, uint32_t* outJ, const uint32_t* ubase, uint32_t* masks, uint2* loc,
                   uint32_t row_lo, uint32_t row_hi) {
   int rc = SQ_OK;
+  if (nsmall) {
+    switch (bw) {
+      case 1: rc = launch_small<1>(c, mode, units_s, nsmall, ids, ids_int, n2, S, cnt_off, outJ, loc, row_lo, row_hi); break;
+      case 2: rc = launch_small<2>(c, mode, units_s, nsmall, ids, ids_int, n2, S, cnt_off, outJ, loc, row_lo, row_hi); break;
+      case 4: rc = launch_small<4>(c, mode, units_s, nsmall, ids, ids_int, n2, S, cnt_off, outJ, loc, row_lo, row_hi); break;
+      default: rc = launch_small<8>(c, mode, units_s, nsmall, ids, ids_int, n2, S, cnt_off, outJ, loc, row_lo, row_hi); break;
+    }
+    if (rc != SQ_OK) return rc;
+  }
   if (nunits0) rc = launch_emit_band0(c, mode, units0, active0, nunits0, ids, bands, cnt_off, outJ, row_lo, row_hi);
   if (rc != SQ_OK || nunits == 0) return rc;
   if (mode != EM_COUNT && masks)
@@ -1027,7 +1152,7 @@ size_t sq_lsh_scratch_bytes(int64_t n, int bands, int64_t pair_capacity) {
   const size_t rec = nn * B;
   const size_t sw = 4 * (size_t)chunks_for((int)B);
   size_t s = 0;
-  s += 2 * sq_align_up(rec * 8 + 16);          // keys ping-pong (the unit lists reuse one)
+  s += 2 * sq_align_up((rec + 4) * 8 + 16);    // keys ping-pong (the unit lists reuse one)
   s += 2 * sq_align_up(rec * 4 + 16);          // ids ping-pong (the internal rows reuse one)
   s += sq_align_up(nn * sw * 4 + 16);          // bucket-id table S
   s += sq_align_up((rec + 2) * 4 + 16);        // per record counts -> offsets
@@ -1064,8 +1189,8 @@ extern "C" int sq_lsh_prepare(sq_ctx* c, const uint32_t* sig, int H, int bands, 
 
   const size_t rec = (size_t)n * bands;
   const int sw = 4 * L.bw;
-  uint64_t* k0 = sq_scratch<uint64_t>(c, rec);
-  uint64_t* k1 = sq_scratch<uint64_t>(c, rec);
+  uint64_t* k0 = sq_scratch<uint64_t>(c, rec + 4);     // (+4: the three unit lists end 2 entries past rec)
+  uint64_t* k1 = sq_scratch<uint64_t>(c, rec + 4);
   uint32_t* v0 = sq_scratch<uint32_t>(c, rec);
   uint32_t* v1 = sq_scratch<uint32_t>(c, rec);
   uint32_t* S = sq_scratch<uint32_t>(c, (size_t)n * sw);
@@ -1081,7 +1206,7 @@ extern "C" int sq_lsh_prepare(sq_ctx* c, const uint32_t* sig, int H, int bands, 
     return SQ_ERR_WORKSPACE;
   cudaStream_t st = c->stream;
   unsigned long long* counters = c->dflags;      // [0] unique, [1] raw, [2] n2, [4] units
-  SQ_CUDA(c, cudaMemsetAsync(counters, 0, 64, st));
+  SQ_CUDA(c, cudaMemsetAsync(counters, 0, 128, st));
 
   // a3: band keys + non-empty flags
   const unsigned gb = (unsigned)((n + 255) / 256);
@@ -1141,20 +1266,22 @@ extern "C" int sq_lsh_prepare(sq_ctx* c, const uint32_t* sig, int H, int bands, 
   // a5.1: buckets -> S table + unit lists (the unit lists live in the dead key buffer)
   uint2* units = reinterpret_cast<uint2*>(kalt);
   uint2* units0 = units + rec / 2 + 1;           // <= n2/2 units of band 0, <= rec/2 in all
+  uint2* units_s = units0 + (size_t)n2 / 2 + 1;  // <= (rec - n2)/2 small units of bands >= 1
   SQ_TIMED(c, SQ_K_SEGMENT, s_prefill_kernel<<<(unsigned)((n2 * (sw / 4) + 255) / 256), 256, 0, st>>>(S, n2, sw));
   SQ_LAUNCH_CHECK(c);
   {
     dim3 grid((unsigned)((n2 + kBsTile - 1) / kBsTile), (unsigned)bands);
     SQ_TIMED(c, SQ_K_SEGMENT, bucket_scan_kernel<<<grid, kBsThreads, 0, st>>>(
-        kin, vint, n2, bucket_cap, sw, S, units, units0, ubase, counters));
+        kin, vint, n2, bucket_cap, sw, S, units, units0, units_s, ubase, counters));
     SQ_LAUNCH_CHECK(c);
   }
-  SQ_CUDA(c, cudaMemcpyAsync(c->pinned, counters, 64, cudaMemcpyDeviceToHost, st));
+  SQ_CUDA(c, cudaMemcpyAsync(c->pinned, counters, 128, cudaMemcpyDeviceToHost, st));
   SQ_CUDA(c, cudaStreamSynchronize(st));
   c->last_raw_pairs = (int64_t)c->pinned[1];
   if (n_raw) *n_raw = c->last_raw_pairs;
   L.raw = c->last_raw_pairs;
   L.nunits = (uint32_t)c->pinned[4]; L.nunits0 = (uint32_t)c->pinned[5]; L.ntiles = c->pinned[7];
+  L.nsmall = (uint32_t)c->pinned[8]; L.units_s = units_s;
   L.vin = vin; L.vint = vint; L.S = S; L.cnt = cnt; L.ubase = ubase; L.loc = loc; L.rowidx = rowidx;
   L.ext_off = ext_off; L.rowstart = rowstart; L.tmp = tmp; L.units = units; L.units0 = units0;
   // the sorted keys are dead from here on: the lists of a call's active units take their place
@@ -1180,7 +1307,7 @@ extern "C" int sq_lsh_emit_range(sq_ctx* c, int64_t row_lo, int64_t row_hi, int 
   if (capacity > 0 && !pairs_out) return SQ_ERR_INVALID_ARG;
   c->scratch_top = L.mark;
   c->sched = nullptr;
-  if (L.n2 < 2 || L.nunits + L.nunits0 == 0 || row_lo == row_hi) return SQ_OK;
+  if (L.n2 < 2 || L.nunits + L.nunits0 + L.nsmall == 0 || row_lo == row_hi) return SQ_OK;
   const int64_t n = L.n, n2 = L.n2;
   const int bands = L.bands, bw = L.bw;
   const size_t rec = (size_t)n * bands;
@@ -1214,13 +1341,13 @@ extern "C" int sq_lsh_emit_range(sq_ctx* c, int64_t row_lo, int64_t row_hi, int 
     SQ_CUDA(c, cudaStreamSynchronize(st));
     nunits = (uint32_t)c->pinned[4]; nunits0 = (uint32_t)c->pinned[5];
     active = act; active0 = act0;
-    if (nunits + nunits0 == 0) return SQ_OK;
+    if (nunits + nunits0 + L.nsmall == 0) return SQ_OK;
   }
   // mask cache: 32 words per (unit, column tile); optional -- without it pass 2 repeats the compares
   uint32_t* masks = (nunits && L.ntiles) ? sq_scratch<uint32_t>(c, (size_t)L.ntiles * 32) : nullptr;
   // a5.2 pass 1: counts per sorted record -> offsets
   SQ_CUDA(c, cudaMemsetAsync(cnt, 0, (rec + 2) * 4, st));
-  rc = dispatch_emit(c, bw, EM_COUNT, L.units, active, nunits, L.units0, active0, nunits0, L.vin, L.vint, (uint32_t)n2,
+  rc = dispatch_emit(c, bw, EM_COUNT, L.units, active, nunits, L.units0, active0, nunits0, L.units_s, L.nsmall, L.vin, L.vint, (uint32_t)n2,
                      bands, L.S, cnt, nullptr, L.ubase, masks, loc, lo, hi);
   if (rc != SQ_OK) return rc;
   rc = sq_exclusive_scan_u32(c, cnt, cnt, total + 1, tmp32, counters);
@@ -1237,7 +1364,7 @@ extern "C" int sq_lsh_emit_range(sq_ctx* c, int64_t row_lo, int64_t row_hi, int 
   uint32_t* tmpJ = sq_scratch<uint32_t>(c, (size_t)uniq);
   if (!tmpJ) return SQ_ERR_WORKSPACE;
   SQ_CUDA(c, cudaMemsetAsync(loc, 0, (rec + 2) * 8, st));
-  rc = dispatch_emit(c, bw, EM_FILL_J, L.units, active, nunits, L.units0, active0, nunits0, L.vin, L.vint, (uint32_t)n2,
+  rc = dispatch_emit(c, bw, EM_FILL_J, L.units, active, nunits, L.units0, active0, nunits0, L.units_s, L.nsmall, L.vin, L.vint, (uint32_t)n2,
                      bands, L.S, cnt, tmpJ, L.ubase, masks, loc, lo, hi);
   if (rc != SQ_OK) return rc;
   // where every EXTERNAL row starts in the output
