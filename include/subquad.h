@@ -176,6 +176,30 @@ int  sq_candidates_stream_host(sq_ctx* ctx, const uint32_t* sig, int H, int band
 int  sq_edit_distance(sq_ctx* ctx, const uint32_t* pairs, int64_t n_pairs, int max_d,
                       uint16_t* dist_out);
 
+/* a6 with compacted hits (north_star (d) "warp-ballot compaction of hits"; PAPER.md
+ * L750-762 App. F.3): sq_edit_distance, then the pairs with d <= max_d (0 <= max_d <= 65534) are
+ * compacted IN INPUT ORDER: hit_pairs_out uint32[capacity][2], hit_dist_out uint16[capacity] (hit k is
+ * the k-th pair of `pairs` whose distance is within the threshold); dist_out uint16[n_pairs] as for
+ * sq_edit_distance; *n_hits (host).  n_pairs < 2^32 - 1.  Scratch: one word per 2,048 pairs from the
+ * free workspace (the schedule of sq_lsh_candidates survives).  Synchronises.  SQ_ERR_CAPACITY (with
+ * the required *n_hits; the first `capacity` hits are written) if the hits do not fit. */
+int  sq_edit_distance_hits(sq_ctx* ctx, const uint32_t* pairs, int64_t n_pairs, int max_d,
+                           uint16_t* dist_out, uint32_t* hit_pairs_out, uint16_t* hit_dist_out,
+                           int64_t capacity, int64_t* n_hits);
+
+/* The same, for callers that cannot allocate (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): this entry point allocates NOTHING and takes no scratch from the
+ * workspace -- its scratch is a file-scope __device__ array of 256 KB inside the library (every GPU
+ * that loads libsubquad.so holds it until the process exits), which bounds the call to
+ * n_pairs <= SQ_HITS_STATIC_MAX_PAIRS (SQ_ERR_UNSUPPORTED beyond).  Same outputs, same order, same
+ * error codes as sq_edit_distance_hits.  All calls (all contexts of a device) share the array, and it
+ * keeps the last call's contents: a call overwrites every word before it reads it, so consecutive
+ * calls are independent, but two calls that OVERLAP on the GPU (different streams) race on it. */
+#define SQ_HITS_STATIC_MAX_PAIRS (1ll << 27)
+int  sq_edit_distance_hits_static(sq_ctx* ctx, const uint32_t* pairs, int64_t n_pairs, int max_d,
+                                  uint16_t* dist_out, uint32_t* hit_pairs_out, uint16_t* hit_dist_out,
+                                  int64_t capacity, int64_t* n_hits);
+
 /* next-1  Weighted edit distance: Eq. 46 as printed, with
  * substitution_cost(a, b) from a table ("typically based on biochemical similarity", L760) and
  * one insertion/deletion cost; boundary D[x][0] = x*indel, D[0][y] = y*indel.

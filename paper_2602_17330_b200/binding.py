@@ -19,13 +19,14 @@ SQ_OK = 0
 SQ_ERR_INVALID_ARG, SQ_ERR_BAD_RESIDUE, SQ_ERR_NOT_PACKED, SQ_ERR_CAPACITY = -1, -2, -3, -4
 SQ_ERR_WORKSPACE, SQ_ERR_UNSUPPORTED, SQ_ERR_CUDA = -5, -6, -7
 SQ_MAX_LEN, SQ_MAX_H, SQ_MAX_BANDS = 240, 256, 32
+SQ_HITS_STATIC_MAX_PAIRS = 1 << 27
 OP_PACK, OP_MINHASH, OP_LSH, OP_EDIT_DISTANCE, OP_ALL_PAIRS, OP_PIPELINE_HOST, OP_GRAPH, OP_JOIN = range(8)
 LSH_SORTED, LSH_UNORDERED = 0, 1
 JOIN_UPPER = 1
 OPT_SORT_KEY_BYTES, OPT_SCHED_MIN_BYTES = 1, 2
 
 EXPORTS = ["sq_create", "sq_destroy", "sq_workspace_bytes", "sq_set_workspace", "sq_pack",
-           "sq_minhash", "sq_lsh_candidates", "sq_lsh_prepare", "sq_lsh_emit_range", "sq_candidates_stream_host", "sq_edit_distance", "sq_edit_distance_weighted", "sq_affinity_graph", "sq_all_pairs",
+           "sq_minhash", "sq_lsh_candidates", "sq_lsh_prepare", "sq_lsh_emit_range", "sq_candidates_stream_host", "sq_edit_distance", "sq_edit_distance_hits", "sq_edit_distance_hits_static", "sq_edit_distance_weighted", "sq_affinity_graph", "sq_all_pairs",
            "sq_join", "sq_join_host", "sq_batch_size", "sq_set_option", "sq_pipeline_host", "sq_pipeline_host_csr", "sq_packed_n", "sq_packed_stride", "sq_last_raw_pairs",
            "sq_kernel_launches", "sq_last_cuda_error", "sq_strerror", "sq_int_peak",
            "sq_profile_enable", "sq_profile_reset", "sq_profile_read", "sq_profile_name"]
@@ -81,6 +82,9 @@ def load_library():
                                             C.POINTER(i64), C.POINTER(i64)]
     L.sq_edit_distance.restype = i32
     L.sq_edit_distance.argtypes = [vp, vp, i64, i32, vp]
+    for fn in (L.sq_edit_distance_hits, L.sq_edit_distance_hits_static):
+        fn.restype = i32
+        fn.argtypes = [vp, vp, i64, i32, vp, vp, vp, i64, C.POINTER(i64)]
     L.sq_edit_distance_weighted.restype = i32
     L.sq_edit_distance_weighted.argtypes = [vp, vp, i64, vp, i32, i32, vp]
     L.sq_affinity_graph.restype = i32
@@ -268,6 +272,17 @@ class SubQuad:
                                               n_pairs, max_d,
                                               _dev_ptr(dist_out, torch.int16, "dist_out")))
         return dist_out
+
+    def edit_distance_hits(self, pairs, n_pairs, max_d, dist_out, hit_pairs_out, hit_dist_out, static=False):
+        """Distances + the pairs with d <= max_d compacted in input order; returns the hit count.
+        static=True: the entry point whose scratch is a static device array (allocates nothing)."""
+        fn = self.lib.sq_edit_distance_hits_static if static else self.lib.sq_edit_distance_hits
+        cnt = C.c_int64(0)
+        rc = fn(self.h, _dev_ptr(pairs, torch.int32, "pairs"), n_pairs, max_d,
+                _dev_ptr(dist_out, torch.int16, "dist_out"), _dev_ptr(hit_pairs_out, torch.int32, "hit_pairs_out"),
+                _dev_ptr(hit_dist_out, torch.int16, "hit_dist_out"), hit_dist_out.shape[0], C.byref(cnt))
+        self._check(rc, required=cnt.value)
+        return cnt.value
 
     def edit_distance_weighted(self, pairs, n_pairs, sub_cost, indel, max_d, dist_out=None):
         """sub_cost: uint8 CUDA tensor [alphabet, alphabet]."""
