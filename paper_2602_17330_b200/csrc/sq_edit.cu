@@ -143,30 +143,27 @@ edit_pairs_w1_kernel(const uint8_t* __restrict__ packed, int64_t n,
       const uint32_t two = blockDim.x / (kEdWarps * 16), one = blockDim.x / (kEdWarps * 32);
       const uint32_t four = blockDim.x / (kEdWarps * 8);
       uint32_t Pv = 0xFFFFFFFFu, Mv = 0u;
+      // one exit per column and ONE reconvergence point behind the loop: a lane whose text has ended
+      // leaves the chain and never rejoins it, so the columns need no reconvergence of their own
+      // (15 instead of 17 instructions per column: 29.5 -> 28.7 ms)
 #pragma unroll
-      for (int wi = 0; wi < WORDS; ++wi) {
-        if (4 * wi < nlen) {
-#pragma unroll
-          for (int q = 0; q < 4; ++q) {
-            if (4 * wi + q < nlen) {
-              uint32_t res, ad, Eq;
-              // (not volatile, so the loads of a word can be issued ahead of the DP chain; the
-              // dummy input m -- read from shared memory after the warp barrier -- keeps them
-              // behind the barrier that publishes the table and the texts)
-              asm("ld.shared.u8 %0, [%1];" : "=r"(res) : "r"(tb + (uint32_t)(wi * 128 + q)), "r"(m));
-              asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(ad) : "r"(res), "r"(four), "r"(pq));
-              asm("ld.shared.u32 %0, [%1];" : "=r"(Eq) : "r"(ad), "r"(m));
-              const uint32_t Xv = Eq | Mv;
-              const uint32_t Xh = (((Eq & Pv) + Pv) ^ Pv) | Eq;
-              uint32_t Ph = Mv | ~(Xh | Pv);
-              uint32_t Mh = Pv & Xh;
-              asm("mad.lo.u32 %0, %0, %1, %2;" : "+r"(Ph) : "r"(two), "r"(one));
-              Mh <<= 1;
-              Pv = Mh | ~(Xv | Ph);
-              Mv = Ph & Xv;
-            }
-          }
-        }
+      for (int y = 0; y < STRIDE - 1; ++y) {
+        if (y >= nlen) break;
+        uint32_t res, ad, Eq;
+        // (not volatile, so the loads can be issued ahead of the DP chain; the dummy input m -- read
+        // from shared memory after the warp barrier -- keeps them behind the barrier that publishes
+        // the table and the texts)
+        asm("ld.shared.u8 %0, [%1];" : "=r"(res) : "r"(tb + (uint32_t)((y >> 2) * 128 + (y & 3))), "r"(m));
+        asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(ad) : "r"(res), "r"(four), "r"(pq));
+        asm("ld.shared.u32 %0, [%1];" : "=r"(Eq) : "r"(ad), "r"(m));
+        const uint32_t Xv = Eq | Mv;
+        const uint32_t Xh = (((Eq & Pv) + Pv) ^ Pv) | Eq;
+        uint32_t Ph = Mv | ~(Xh | Pv);
+        uint32_t Mh = Pv & Xh;
+        asm("mad.lo.u32 %0, %0, %1, %2;" : "+r"(Ph) : "r"(two), "r"(one));
+        Mh <<= 1;
+        Pv = Mh | ~(Xv | Ph);
+        Mv = Ph & Xv;
       }
       const uint32_t mask = (1u << m) - 1u;                        // m <= 31
       d = nlen + __popc(Pv & mask) - __popc(Mv & mask);
