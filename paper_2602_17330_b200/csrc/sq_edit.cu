@@ -44,6 +44,32 @@ constexpr int kEdRuns = 8;      // Peq tables resident per warp
 // sq_lsh_candidates (sq_common.cuh) instead of pairs [32k, 32k+32): consecutive warps then work
 // on rows of the same family, whose partners are the same few sequences -- the text gathers hit
 // L2.  The schedule only permutes the pair indices; every pair is still read from `pairs`.
+// One column of the single-word chain on the fast path (below).  Every column is entered by the
+// warp-uniform indexed jump, i.e. it is a basic block of its own and the assembler moves no load
+// across its border -- so the loads are pipelined by hand: column U computes on the table word
+// fetched by column U - 1, fetches the word of column U + 1 (address = one multiply-add on the
+// FMA pipe) and the residue of column U + 2 (LDS.U8 at a compile-time offset).  13 instructions:
+// 2 shared loads, 7 logic ops (ALU pipe), the address, the add and the two shifts as multiply-adds
+// (FMA pipe); no branch, no predicate.  Even columns compute on EqA and fetch into EqB, odd ones the
+// other way round (no register move).
+#define SQ_W1_COL(U, Eq, EqN)                                                                            \
+  {                                                                                               \
+    if ((U) + 1 < NCOL) {                                                                         \
+      uint32_t ad;                                                                                \
+      asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(ad) : "r"(resN), "r"(four), "r"(pq));              \
+      asm("ld.shared.u32 %0, [%1];" : "=r"(EqN) : "r"(ad), "r"(ones));                           \
+    }                                                                                             \
+    if ((U) + 2 < NCOL) asm("ld.shared.u8 %0, [%1+" #U "+2];" : "=r"(resN) : "r"(tbase), "r"(ones)); \
+    const uint32_t Xv = Eq | Mv;                                                                  \
+    const uint32_t Xh = (((Eq & Pv) + Pv) ^ Pv) | Eq;                                             \
+    uint32_t Ph = Mv | ~(Xh | Pv);                                                                \
+    uint32_t Mh = Pv & Xh;                                                                        \
+    asm("mad.lo.u32 %0, %0, %1, %2;" : "+r"(Ph) : "r"(two), "r"(one));                           \
+    Mh <<= 1;                                                                                     \
+    Pv = Mh | ~(Xv | Ph);                                                                         \
+    Mv = Ph & Xv;                                                                                 \
+  }
+
 template <int STRIDE, bool SCHED>
 __global__ void __launch_bounds__(kEdWarps * 32, 64 / kEdWarps)
 edit_pairs_w1_kernel(const uint8_t* __restrict__ packed, int64_t n,
@@ -52,10 +78,15 @@ edit_pairs_w1_kernel(const uint8_t* __restrict__ packed, int64_t n,
                      const uint4* __restrict__ sched, const uint32_t* __restrict__ rowstart,
                      const uint32_t* __restrict__ delta) {
   constexpr int WORDS = STRIDE / 4;
+  constexpr int NCOL = STRIDE - 1;                 // longest text of a slot
+  constexpr int LSTR = STRIDE + 4;                 // byte stride of a lane's text on the fast path (odd word count)
   __shared__ uint32_t peq_sm[kEdWarps][kEdRuns * 33];
   __shared__ uint32_t mlen_sm[kEdWarps][kEdRuns];
-  __shared__ uint32_t text_sm[kEdWarps][STRIDE / 4][32];      // the lanes' texts, [word][lane]
+  // the lanes' texts: [word][lane] on the general path, byte-linear [lane][LSTR] on the fast path
+  __shared__ __align__(16) uint32_t text_raw[kEdWarps][32 * LSTR / 4];
+  static_assert(sizeof(uint32_t) * (STRIDE / 4) * 32 <= sizeof(text_raw[0]), "text area");
   const uint32_t lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  uint32_t (*text_sm)[32] = reinterpret_cast<uint32_t (*)[32]>(&text_raw[w][0]);
   const int64_t wk = (int64_t)blockIdx.x * kEdWarps + w;
   int64_t p = wk * 32 + lane;
   bool valid = p < n_pairs;
@@ -94,6 +125,126 @@ edit_pairs_w1_kernel(const uint8_t* __restrict__ packed, int64_t n,
       }
     }
   }
+  const int nlen = (int)(tw[WORDS - 1] >> 24);
+  // ---- fast path: the 32 pairs share ONE pattern (the common case: a row has 161 partners on
+  // average at config 4, and the pairs arrive grouped by i).  One table, no run loop; and NO
+  // per-column exit: a column whose table word is all ones (every position "matches") moves the whole
+  // state up by one bit -- Pv' = Pv << 1, Mv' = Mv << 1 | 1 -- so a lane whose text has ended keeps
+  // feeding its slot's pad bytes (0xFF -> table word 255 = ~0) until the warp's longest text is done,
+  // and reads D[m][n] from bits [q, q + m) of the final deltas, q = the number of pad columns it ran.
+  // That needs m + q <= 32 for every lane that passes the length filter (checked, else the general
+  // path below).  The texts are stored byte-linear per lane, so that the warp can ENTER the unrolled
+  // chain at column NCOL - Lmax (one warp-uniform indexed jump) and all lanes read "their residue
+  // U - (NCOL - Lmax)" at a compile-time offset U of a per-lane base.
+  {
+    int same;
+    __match_all_sync(0xFFFFFFFFu, i, &same);
+    if (same && i != 0xFFFFFFFFu) {                   // (i == 0xFFFFFFFF: some lane invalid or out of range)
+      uint32_t* peq = peq_sm[w];
+      uint32_t chb = 0xFFu;
+      if (lane < (uint32_t)STRIDE) chb = packed[(int64_t)i * STRIDE + lane];
+      peq[lane] = 0u;
+      if (lane == 0) peq[255] = 0xFFFFFFFFu;          // inside the warp's own kEdRuns * 33 words
+      const int m = (int)__shfl_sync(0xFFFFFFFFu, chb, STRIDE - 1);
+      const uint32_t maskm = (1u << m) - 1u;          // m <= 31
+      __syncwarp();
+      const uint32_t mm = __match_any_sync(0xFFFFFFFFu, chb);
+      if ((int)lane < m) peq[chb] = mm & maskm;
+      uint8_t* trow = reinterpret_cast<uint8_t*>(&text_raw[w][0]) + lane * LSTR;
+#pragma unroll
+      for (int q = 0; q < WORDS; ++q) reinterpret_cast<uint32_t*>(trow)[q] = tw[q];
+      const int diff = m > nlen ? m - nlen : nlen - m;
+      const bool pass = max_d < 0 || diff <= max_d;
+      const int Lmax = __reduce_max_sync(0xFFFFFFFFu, pass ? nlen : 0);
+      const int Lmin = __reduce_min_sync(0xFFFFFFFFu, pass ? nlen : NCOL);
+      if (m + Lmax - Lmin <= 32) {
+        __syncwarp();
+        const uint32_t pq = (uint32_t)__cvta_generic_to_shared(peq);
+        const uint32_t tbase = (uint32_t)__cvta_generic_to_shared(trow) - (uint32_t)(NCOL - Lmax);
+        const uint32_t two = blockDim.x / (kEdWarps * 16), one = blockDim.x / (kEdWarps * 32);
+        const uint32_t four = blockDim.x / (kEdWarps * 8);
+        // (the chain's loads are not volatile, so that they can be issued ahead of the dependent logic
+        // chain; their dummy input `ones` -- read from shared memory behind the warp barrier that
+        // publishes table and texts -- keeps them behind that barrier)
+        uint32_t ones;
+        asm volatile("ld.shared.u32 %0, [%1+1020];" : "=r"(ones) : "r"(pq) : "memory");
+        uint32_t Pv = ones, Mv = 0u;
+        // residue 0 -> its table word, residue 1: what the first column of the chain expects
+        uint32_t resN, EqA, EqB;
+        {
+          const uint32_t t0 = (uint32_t)__cvta_generic_to_shared(trow);
+          uint32_t r0, ad;
+          asm("ld.shared.u8 %0, [%1];" : "=r"(r0) : "r"(t0), "r"(ones));
+          asm("ld.shared.u8 %0, [%1+1];" : "=r"(resN) : "r"(t0), "r"(ones));
+          asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(ad) : "r"(r0), "r"(four), "r"(pq));
+          // (the entry column may be an even or an odd one: the word is fetched into both registers)
+          asm volatile("ld.shared.u32 %0, [%1];" : "=r"(EqA) : "r"(ad), "r"(ones));
+          asm volatile("ld.shared.u32 %0, [%1];" : "=r"(EqB) : "r"(ad), "r"(ones));
+        }
+        if (STRIDE == 32) {
+          switch (Lmax) {
+            case 31: SQ_W1_COL(0, EqA, EqB)
+            case 30: SQ_W1_COL(1, EqB, EqA)
+            case 29: SQ_W1_COL(2, EqA, EqB)
+            case 28: SQ_W1_COL(3, EqB, EqA)
+            case 27: SQ_W1_COL(4, EqA, EqB)
+            case 26: SQ_W1_COL(5, EqB, EqA)
+            case 25: SQ_W1_COL(6, EqA, EqB)
+            case 24: SQ_W1_COL(7, EqB, EqA)
+            case 23: SQ_W1_COL(8, EqA, EqB)
+            case 22: SQ_W1_COL(9, EqB, EqA)
+            case 21: SQ_W1_COL(10, EqA, EqB)
+            case 20: SQ_W1_COL(11, EqB, EqA)
+            case 19: SQ_W1_COL(12, EqA, EqB)
+            case 18: SQ_W1_COL(13, EqB, EqA)
+            case 17: SQ_W1_COL(14, EqA, EqB)
+            case 16: SQ_W1_COL(15, EqB, EqA)
+            case 15: SQ_W1_COL(16, EqA, EqB)
+            case 14: SQ_W1_COL(17, EqB, EqA)
+            case 13: SQ_W1_COL(18, EqA, EqB)
+            case 12: SQ_W1_COL(19, EqB, EqA)
+            case 11: SQ_W1_COL(20, EqA, EqB)
+            case 10: SQ_W1_COL(21, EqB, EqA)
+            case 9: SQ_W1_COL(22, EqA, EqB)
+            case 8: SQ_W1_COL(23, EqB, EqA)
+            case 7: SQ_W1_COL(24, EqA, EqB)
+            case 6: SQ_W1_COL(25, EqB, EqA)
+            case 5: SQ_W1_COL(26, EqA, EqB)
+            case 4: SQ_W1_COL(27, EqB, EqA)
+            case 3: SQ_W1_COL(28, EqA, EqB)
+            case 2: SQ_W1_COL(29, EqB, EqA)
+            case 1: SQ_W1_COL(30, EqA, EqB)
+            default: break;
+          }
+        } else {
+          switch (Lmax) {
+            case 15: SQ_W1_COL(0, EqA, EqB)
+            case 14: SQ_W1_COL(1, EqB, EqA)
+            case 13: SQ_W1_COL(2, EqA, EqB)
+            case 12: SQ_W1_COL(3, EqB, EqA)
+            case 11: SQ_W1_COL(4, EqA, EqB)
+            case 10: SQ_W1_COL(5, EqB, EqA)
+            case 9: SQ_W1_COL(6, EqA, EqB)
+            case 8: SQ_W1_COL(7, EqB, EqA)
+            case 7: SQ_W1_COL(8, EqA, EqB)
+            case 6: SQ_W1_COL(9, EqB, EqA)
+            case 5: SQ_W1_COL(10, EqA, EqB)
+            case 4: SQ_W1_COL(11, EqB, EqA)
+            case 3: SQ_W1_COL(12, EqA, EqB)
+            case 2: SQ_W1_COL(13, EqB, EqA)
+            case 1: SQ_W1_COL(14, EqA, EqB)
+            default: break;
+          }
+        }
+        const uint32_t mask = maskm << ((Lmax - nlen) & 31);       // (a lane that failed the filter: unused)
+        int d = nlen + __popc(Pv & mask) - __popc(Mv & mask);
+        if (!pass || (max_d >= 0 && d > max_d)) d = max_d + 1;
+        dist[p] = (uint16_t)d;
+        return;
+      }
+      __syncwarp();                                    // the general path reuses the shared arrays
+    }
+  }
   // runs of equal i
   const uint32_t prev = __shfl_up_sync(0xFFFFFFFFu, i, 1);
   const bool head = lane == 0 || i != prev;
@@ -102,11 +253,10 @@ edit_pairs_w1_kernel(const uint8_t* __restrict__ packed, int64_t n,
   const int nruns = __popc(hm);
   uint32_t* peq = peq_sm[w];
   uint32_t rem = hm;
-  const int nlen = (int)(tw[WORDS - 1] >> 24);
 #pragma unroll
-  for (int q = 0; q < WORDS; ++q) text_sm[w][q][lane] = tw[q];
+  for (int q = 0; q < WORDS; ++q) text_sm[q][lane] = tw[q];
   // byte y of this lane's text is at tb + (y / 4) * 128 + y % 4 (a compile-time offset per column)
-  const uint32_t tb = (uint32_t)__cvta_generic_to_shared(&text_sm[w][0][lane]);
+  const uint32_t tb = (uint32_t)__cvta_generic_to_shared(&text_sm[0][lane]);
   int d = 0;
   // kEdRuns Peq tables fit at a time; a warp with more runs (many tiny rows) takes several rounds
 #pragma unroll 1

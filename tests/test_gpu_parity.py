@@ -230,6 +230,57 @@ def test_edit_distance_textbook_and_edge_cases():
     sq.close()
 
 
+# ---------------------------------------------------------------------------------------------
+# single-word DP, one-pattern chunks: 32 consecutive pairs that share i take the branch-free chain
+# in which a lane whose text has ended keeps shifting its state through all-ones table words
+# (sq_edit.cu).  Rows of >= 32 partners with every mix of text lengths: equal lengths, spreads that
+# still fit m + Lmax - Lmin <= 32, spreads that do not (general path), empty patterns and texts,
+# thresholds from "everything filtered" to none, both slot strides.
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("max_len,alphabet", [(31, 20), (15, 20), (25, 4), (31, 2)])
+def test_edit_distance_one_pattern_chunks(max_len, alphabet):
+    binding, sq = _ctx()
+    rng = np.random.default_rng(1234 + max_len + alphabet)
+    seqs = []
+    # group g: sequences whose lengths are drawn from a narrow or a wide window
+    windows = [(0, 0), (0, 3), (1, 1), (max_len, max_len), (max_len - 2, max_len), (0, max_len),
+               (5, 9), (8, min(25, max_len)), (max_len // 2, max_len), (3, 3)]
+    group = []
+    for g, (lo, hi) in enumerate(windows):
+        for _ in range(70):
+            L = int(rng.integers(lo, hi + 1))
+            base = rng.integers(0, alphabet, size=L)
+            seqs.append(base.tolist())
+            group.append(g)
+    rep = dg.from_list(seqs)
+    n = rep.n
+    group = np.array(group)
+    # rows: the first 3 sequences of every group against all later members of the same group (67-69
+    # partners: two full one-pattern chunks and a ragged tail shared with the next row), and against a
+    # mixed window of other groups
+    pl = []
+    for g in range(len(windows)):
+        idx = np.flatnonzero(group == g)
+        for a in idx[:3]:
+            for b in idx[idx > a]:
+                pl.append((a, b))
+        a = idx[3]
+        for b in rng.permutation(n)[:96]:
+            pl.append((a, int(b)))
+    pl = np.array(pl, dtype=np.uint32)
+    ws = sq.workspace_bytes(binding.OP_ALL_PAIRS, n, int(rep.offsets[-1]), max_len, 0, 1, 0, 1000)
+    sq.set_workspace(ws)
+    sq.pack(torch.from_numpy(rep.seqs).cuda(), torch.from_numpy(rep.offsets).cuda(),
+            alphabet=alphabet, max_len=max_len)
+    want = oracle.edit_distance_pairs(rep.seqs, rep.offsets, pl, -1)
+    pt = torch.from_numpy(pl.view(np.int32)).cuda()
+    for md in (-1, 0, 1, 3, 7, 40):
+        d = sq.edit_distance(pt, pl.shape[0], md)
+        w = want if md < 0 else np.minimum(want, md + 1)
+        assert np.array_equal(_u16(d)[:pl.shape[0]], w), md
+    sq.close()
+
+
 def test_empty_inputs_and_short_sequences():
     binding, sq = _ctx()
     # n = 0
