@@ -610,7 +610,12 @@ def run_ours(args):
     # ---- rooflines ---------------------------------------------------------------------------
     hbm_peak, peak_src = measured_peaks()
     int_peak = {name: sq.int_peak(kind, 2048) for kind, name in
-                ((0, "lop3"), (1, "iadd"), (3, "imad"), (4, "umin"), (5, "lop3+imad"))}
+                ((0, "lop3"), (1, "iadd"), (3, "imad"), (4, "umin"), (5, "lop3+imad"),
+                 (8, "lop3+imad_fresh_operands"), (9, "dp_column_mix_7lop3_4imad"))}
+    # LOP3 share of the DP column's own instruction mix: the ceiling the register file sets
+    int_peak["lop3_inside_dp_column_mix"] = int_peak["dp_column_mix_7lop3_4imad"] * 7.0 / 11.0
+    # the product's own column chain alone (shared-memory resident, no global memory), as LOP3 per second
+    int_peak["lop3_dp_chain_alone"] = sq.dp_chain_peak(20, 2000) * ALU_OPS_PER_COLUMN_WORD
     B = P["bands"]
     K = args.steps
     rec = n * B                                    # (sequence, band) records
@@ -642,6 +647,8 @@ def run_ours(args):
             k["bound"] = "alu"
             k["achieved_Gops"] = ops / (ms / K * 1e-3) / 1e9
             k["frac"] = k["achieved_Gops"] * 1e9 / int_peak["lop3"]
+            k["frac_of_lop3_inside_dp_column_mix"] = k["achieved_Gops"] * 1e9 / int_peak["lop3_inside_dp_column_mix"]
+            k["frac_of_dp_chain_alone"] = k["achieved_Gops"] * 1e9 / int_peak["lop3_dp_chain_alone"]
         if name == "minhash":
             L = rep.lengths
             upd = float(np.maximum(L - P["k"] + 1, 0).sum()) * P["H"]

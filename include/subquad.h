@@ -329,8 +329,19 @@ const char* sq_profile_name(int kernel_class);   /* NULL past the last class */
  * runs `iters` dependent-free instructions of `kind` per thread on a full grid and returns
  * achieved lane-operations per second in *ops_per_s (host).
  * kind: 0 LOP3, 1 IADD3, 2 SHF, 3 IMAD, 4 min.u32, 5 LOP3+IMAD mix, 6 POPC, 7 byte-wise sum of
- * absolute differences (vabsdiff4 ... add; the instruction of the bag-distance filter). */
+ * absolute differences (vabsdiff4 ... add; the instruction of the bag-distance filter); 8 LOP3 / IMAD
+ * alternating with three FRESH register operands each and 9 the DP column's mix (7 LOP3 : 4 IMAD, fresh
+ * operands): what the register file feeds two pipes at once (kinds 0-7 reuse two loop-invariant operands).
+ * Kinds 5, 8 and 9 count the instructions of both pipes. */
 int  sq_int_peak(sq_ctx* ctx, int kind, int iters, double* ops_per_s);
+
+/* The column chain of the single-word DP kernel ALONE (App. F.3, Eq. 46 as the
+ * Myers/Hyyro column step): tables and texts resident in shared memory with synthetic contents, no
+ * global memory, every warp slot of the device filled; `iters` chains of `text_len` (1..31) columns
+ * per lane.  *lane_columns_per_s (host) = achieved (lane, text column) steps per second; times 7 it is
+ * the LOP3 rate this formulation of the column reaches at best -- the ceiling bench.py quotes beside
+ * the plain LOP3 peak.  Needs a workspace (one 1 KB sink).  SQ_ERR_INVALID_ARG on bad arguments. */
+int  sq_dp_chain_peak(sq_ctx* ctx, int text_len, int iters, double* lane_columns_per_s);
 
 #ifdef __cplusplus
 }

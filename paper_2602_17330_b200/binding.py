@@ -28,7 +28,7 @@ OPT_SORT_KEY_BYTES, OPT_SCHED_MIN_BYTES = 1, 2
 EXPORTS = ["sq_create", "sq_destroy", "sq_workspace_bytes", "sq_set_workspace", "sq_pack",
            "sq_minhash", "sq_lsh_candidates", "sq_lsh_prepare", "sq_lsh_emit_range", "sq_candidates_stream_host", "sq_edit_distance", "sq_edit_distance_hits", "sq_edit_distance_hits_static", "sq_edit_distance_weighted", "sq_affinity_graph", "sq_all_pairs",
            "sq_join", "sq_join_host", "sq_batch_size", "sq_set_option", "sq_pipeline_host", "sq_pipeline_host_csr", "sq_packed_n", "sq_packed_stride", "sq_last_raw_pairs",
-           "sq_kernel_launches", "sq_last_cuda_error", "sq_strerror", "sq_int_peak",
+           "sq_kernel_launches", "sq_last_cuda_error", "sq_strerror", "sq_int_peak", "sq_dp_chain_peak",
            "sq_profile_enable", "sq_profile_reset", "sq_profile_read", "sq_profile_name"]
 
 
@@ -119,6 +119,8 @@ def load_library():
     L.sq_strerror.argtypes = [i32]
     L.sq_int_peak.restype = i32
     L.sq_int_peak.argtypes = [vp, i32, i32, C.POINTER(C.c_double)]
+    L.sq_dp_chain_peak.restype = i32
+    L.sq_dp_chain_peak.argtypes = [vp, i32, i32, C.POINTER(C.c_double)]
     L.sq_profile_enable.restype = i32
     L.sq_profile_enable.argtypes = [vp, i32]
     L.sq_profile_reset.restype = i32
@@ -408,4 +410,10 @@ class SubQuad:
     def int_peak(self, kind: int, iters: int = 4096) -> float:
         out = C.c_double(0.0)
         self._check(self.lib.sq_int_peak(self.h, kind, iters, C.byref(out)))
+        return out.value
+
+    def dp_chain_peak(self, text_len: int = 20, iters: int = 2000) -> float:
+        """(lane, text column) steps per second of the single-word DP column chain alone"""
+        out = C.c_double(0.0)
+        self._check(self.lib.sq_dp_chain_peak(self.h, text_len, iters, C.byref(out)))
         return out.value

@@ -70,6 +70,62 @@ constexpr int kEdRuns = 8;      // Peq tables resident per warp
     Mv = Ph & Xv;                                                                                 \
   }
 
+// the unrolled chain of a 32-byte / 16-byte slot, entered at column NCOL - L
+#define SQ_W1_CHAIN31(L) \
+  switch (L) { \
+    case 31: SQ_W1_COL(0, EqA, EqB) \
+    case 30: SQ_W1_COL(1, EqB, EqA) \
+    case 29: SQ_W1_COL(2, EqA, EqB) \
+    case 28: SQ_W1_COL(3, EqB, EqA) \
+    case 27: SQ_W1_COL(4, EqA, EqB) \
+    case 26: SQ_W1_COL(5, EqB, EqA) \
+    case 25: SQ_W1_COL(6, EqA, EqB) \
+    case 24: SQ_W1_COL(7, EqB, EqA) \
+    case 23: SQ_W1_COL(8, EqA, EqB) \
+    case 22: SQ_W1_COL(9, EqB, EqA) \
+    case 21: SQ_W1_COL(10, EqA, EqB) \
+    case 20: SQ_W1_COL(11, EqB, EqA) \
+    case 19: SQ_W1_COL(12, EqA, EqB) \
+    case 18: SQ_W1_COL(13, EqB, EqA) \
+    case 17: SQ_W1_COL(14, EqA, EqB) \
+    case 16: SQ_W1_COL(15, EqB, EqA) \
+    case 15: SQ_W1_COL(16, EqA, EqB) \
+    case 14: SQ_W1_COL(17, EqB, EqA) \
+    case 13: SQ_W1_COL(18, EqA, EqB) \
+    case 12: SQ_W1_COL(19, EqB, EqA) \
+    case 11: SQ_W1_COL(20, EqA, EqB) \
+    case 10: SQ_W1_COL(21, EqB, EqA) \
+    case 9: SQ_W1_COL(22, EqA, EqB) \
+    case 8: SQ_W1_COL(23, EqB, EqA) \
+    case 7: SQ_W1_COL(24, EqA, EqB) \
+    case 6: SQ_W1_COL(25, EqB, EqA) \
+    case 5: SQ_W1_COL(26, EqA, EqB) \
+    case 4: SQ_W1_COL(27, EqB, EqA) \
+    case 3: SQ_W1_COL(28, EqA, EqB) \
+    case 2: SQ_W1_COL(29, EqB, EqA) \
+    case 1: SQ_W1_COL(30, EqA, EqB) \
+    default: break; \
+  }
+#define SQ_W1_CHAIN15(L) \
+  switch (L) { \
+    case 15: SQ_W1_COL(0, EqA, EqB) \
+    case 14: SQ_W1_COL(1, EqB, EqA) \
+    case 13: SQ_W1_COL(2, EqA, EqB) \
+    case 12: SQ_W1_COL(3, EqB, EqA) \
+    case 11: SQ_W1_COL(4, EqA, EqB) \
+    case 10: SQ_W1_COL(5, EqB, EqA) \
+    case 9: SQ_W1_COL(6, EqA, EqB) \
+    case 8: SQ_W1_COL(7, EqB, EqA) \
+    case 7: SQ_W1_COL(8, EqA, EqB) \
+    case 6: SQ_W1_COL(9, EqB, EqA) \
+    case 5: SQ_W1_COL(10, EqA, EqB) \
+    case 4: SQ_W1_COL(11, EqB, EqA) \
+    case 3: SQ_W1_COL(12, EqA, EqB) \
+    case 2: SQ_W1_COL(13, EqB, EqA) \
+    case 1: SQ_W1_COL(14, EqA, EqB) \
+    default: break; \
+  }
+
 template <int STRIDE, bool SCHED>
 __global__ void __launch_bounds__(kEdWarps * 32, 64 / kEdWarps)
 edit_pairs_w1_kernel(const uint8_t* __restrict__ packed, int64_t n,
@@ -181,61 +237,7 @@ edit_pairs_w1_kernel(const uint8_t* __restrict__ packed, int64_t n,
           asm volatile("ld.shared.u32 %0, [%1];" : "=r"(EqA) : "r"(ad), "r"(ones));
           asm volatile("ld.shared.u32 %0, [%1];" : "=r"(EqB) : "r"(ad), "r"(ones));
         }
-        if (STRIDE == 32) {
-          switch (Lmax) {
-            case 31: SQ_W1_COL(0, EqA, EqB)
-            case 30: SQ_W1_COL(1, EqB, EqA)
-            case 29: SQ_W1_COL(2, EqA, EqB)
-            case 28: SQ_W1_COL(3, EqB, EqA)
-            case 27: SQ_W1_COL(4, EqA, EqB)
-            case 26: SQ_W1_COL(5, EqB, EqA)
-            case 25: SQ_W1_COL(6, EqA, EqB)
-            case 24: SQ_W1_COL(7, EqB, EqA)
-            case 23: SQ_W1_COL(8, EqA, EqB)
-            case 22: SQ_W1_COL(9, EqB, EqA)
-            case 21: SQ_W1_COL(10, EqA, EqB)
-            case 20: SQ_W1_COL(11, EqB, EqA)
-            case 19: SQ_W1_COL(12, EqA, EqB)
-            case 18: SQ_W1_COL(13, EqB, EqA)
-            case 17: SQ_W1_COL(14, EqA, EqB)
-            case 16: SQ_W1_COL(15, EqB, EqA)
-            case 15: SQ_W1_COL(16, EqA, EqB)
-            case 14: SQ_W1_COL(17, EqB, EqA)
-            case 13: SQ_W1_COL(18, EqA, EqB)
-            case 12: SQ_W1_COL(19, EqB, EqA)
-            case 11: SQ_W1_COL(20, EqA, EqB)
-            case 10: SQ_W1_COL(21, EqB, EqA)
-            case 9: SQ_W1_COL(22, EqA, EqB)
-            case 8: SQ_W1_COL(23, EqB, EqA)
-            case 7: SQ_W1_COL(24, EqA, EqB)
-            case 6: SQ_W1_COL(25, EqB, EqA)
-            case 5: SQ_W1_COL(26, EqA, EqB)
-            case 4: SQ_W1_COL(27, EqB, EqA)
-            case 3: SQ_W1_COL(28, EqA, EqB)
-            case 2: SQ_W1_COL(29, EqB, EqA)
-            case 1: SQ_W1_COL(30, EqA, EqB)
-            default: break;
-          }
-        } else {
-          switch (Lmax) {
-            case 15: SQ_W1_COL(0, EqA, EqB)
-            case 14: SQ_W1_COL(1, EqB, EqA)
-            case 13: SQ_W1_COL(2, EqA, EqB)
-            case 12: SQ_W1_COL(3, EqB, EqA)
-            case 11: SQ_W1_COL(4, EqA, EqB)
-            case 10: SQ_W1_COL(5, EqB, EqA)
-            case 9: SQ_W1_COL(6, EqA, EqB)
-            case 8: SQ_W1_COL(7, EqB, EqA)
-            case 7: SQ_W1_COL(8, EqA, EqB)
-            case 6: SQ_W1_COL(9, EqB, EqA)
-            case 5: SQ_W1_COL(10, EqA, EqB)
-            case 4: SQ_W1_COL(11, EqB, EqA)
-            case 3: SQ_W1_COL(12, EqA, EqB)
-            case 2: SQ_W1_COL(13, EqB, EqA)
-            case 1: SQ_W1_COL(14, EqA, EqB)
-            default: break;
-          }
-        }
+        if (STRIDE == 32) { SQ_W1_CHAIN31(Lmax) } else { SQ_W1_CHAIN15(Lmax) }
         const uint32_t mask = maskm << ((Lmax - nlen) & 31);       // (a lane that failed the filter: unused)
         int d = nlen + __popc(Pv & mask) - __popc(Mv & mask);
         if (!pass || (max_d >= 0 && d > max_d)) d = max_d + 1;
@@ -347,6 +349,45 @@ int launch_edit_w1(sq_ctx* c, const uint8_t* packedB, int64_t nB, const uint32_t
       nullptr, nullptr));
   SQ_LAUNCH_CHECK(c);
   return SQ_OK;
+}
+
+// The one-pattern column chain ALONE: tables and texts resident in shared memory (synthetic contents), no
+// global memory, every scheduler full.  What it reaches is the ceiling of this formulation of the column
+// step (the register file feeds the ALU and the FMA pipe ~1.8 operand vectors per cycle);
+// sq_dp_chain_peak reports it in lane-columns per second.
+__global__ void __launch_bounds__(kEdWarps * 32, 64 / kEdWarps)
+edit_chain_probe_kernel(int iters, int Lmax, uint32_t* __restrict__ sink) {
+  constexpr int NCOL = 31, LSTR = 36;
+  __shared__ uint32_t peq_sm[kEdWarps][kEdRuns * 33];
+  __shared__ uint32_t text_raw[kEdWarps][32 * LSTR / 4];
+  const uint32_t lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  uint32_t* peq = peq_sm[w];
+  for (uint32_t q = lane; q < (uint32_t)kEdRuns * 33; q += 32) peq[q] = (q * 2654435761u) >> 7;
+  for (uint32_t q = lane; q < 32u * LSTR / 4; q += 32) text_raw[w][q] = ((q * 0x01010101u) & 0x0F0F0F0Fu) + 0x01020304u;
+  __syncwarp();
+  const uint32_t two = blockDim.x / (kEdWarps * 16), one = blockDim.x / (kEdWarps * 32);
+  const uint32_t four = blockDim.x / (kEdWarps * 8);
+  const uint32_t pq = (uint32_t)__cvta_generic_to_shared(peq);
+  const uint32_t t0 = (uint32_t)__cvta_generic_to_shared(&text_raw[w][0]) + lane * LSTR;
+  const uint32_t tbase = t0 - (uint32_t)(NCOL - Lmax);
+  uint32_t acc = 0;
+  for (int it = 0; it < iters; ++it) {
+    uint32_t ones;
+    asm volatile("ld.shared.u32 %0, [%1+1020];" : "=r"(ones) : "r"(pq) : "memory");
+    uint32_t Pv = ones ^ (acc & 0xFFu), Mv = 0u;
+    uint32_t resN, EqA, EqB;
+    {
+      uint32_t r0, ad;
+      asm("ld.shared.u8 %0, [%1];" : "=r"(r0) : "r"(t0), "r"(ones));
+      asm("ld.shared.u8 %0, [%1+1];" : "=r"(resN) : "r"(t0), "r"(ones));
+      asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(ad) : "r"(r0), "r"(four), "r"(pq));
+      asm volatile("ld.shared.u32 %0, [%1];" : "=r"(EqA) : "r"(ad), "r"(ones));
+      asm volatile("ld.shared.u32 %0, [%1];" : "=r"(EqB) : "r"(ad), "r"(ones));
+    }
+    SQ_W1_CHAIN31(Lmax)
+    acc = acc * 3u + (Pv ^ Mv);
+  }
+  if (acc == 0x12345u) sink[threadIdx.x] = acc;      // practically never true: keeps the chain live
 }
 
 template <int W>
@@ -582,4 +623,37 @@ int sq_edit_distance_impl(sq_ctx* c, const uint32_t* pairs, int64_t n_pairs, int
                           uint16_t* dist_out) {
   if (c->n < 0) return SQ_ERR_NOT_PACKED;
   return sq_edit_distance_ab(c, c->packed, c->n, c->max_len, pairs, n_pairs, max_d, dist_out, false);
+}
+
+extern "C" int sq_dp_chain_peak(sq_ctx* c, int text_len, int iters, double* lane_columns_per_s) {
+  if (!c || !lane_columns_per_s || iters < 1 || text_len < 1 || text_len > 31) return SQ_ERR_INVALID_ARG;
+  if (!c->ws) return SQ_ERR_WORKSPACE;
+  SqDeviceGuard guard(c);
+  const size_t top = c->scratch_top;
+  uint32_t* sink = sq_scratch<uint32_t>(c, 256);     // handed back at once: practically never written
+  c->scratch_top = top;
+  if (!sink) return SQ_ERR_WORKSPACE;
+  const int blocks = c->sm_count * (64 / kEdWarps);
+  cudaEvent_t e0, e1;
+  SQ_CUDA(c, cudaEventCreate(&e0));
+  if (cudaEventCreate(&e1) != cudaSuccess) { c->last_err = cudaGetLastError(); cudaEventDestroy(e0); return SQ_ERR_CUDA; }
+  float best = 1e30f;
+  for (int rep = 0; rep < 4; ++rep) {
+    cudaEventRecord(e0, c->stream);
+    edit_chain_probe_kernel<<<blocks, kEdWarps * 32, 0, c->stream>>>(iters, text_len, sink);
+    c->launches++;
+    cudaEventRecord(e1, c->stream);
+    if (cudaEventSynchronize(e1) != cudaSuccess || cudaGetLastError() != cudaSuccess) {
+      c->last_err = cudaGetLastError();
+      cudaEventDestroy(e0); cudaEventDestroy(e1);
+      return SQ_ERR_CUDA;
+    }
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    if (rep > 0 && ms < best) best = ms;
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  *lane_columns_per_s = (double)blocks * kEdWarps * 32.0 * (double)iters * (double)text_len / (best * 1e-3);
+  return SQ_OK;
 }

@@ -29,6 +29,16 @@ int_peak_kernel(int iters, uint32_t seed, uint32_t* __restrict__ sink) {
         }
         if (KIND == 6) asm volatile("popc.b32 %0, %0;" : "+r"(r[q]));
         if (KIND == 7) asm volatile("vabsdiff4.u32.u32.u32.add %0, %0, %1, %2;" : "+r"(r[q]) : "r"(k1), "r"(k2));
+        // 8, 9: what the register file feeds TWO pipes at once when every operand is a fresh register
+        // (the streams above reuse two loop-invariant operands, which the operand reuse cache serves)
+        if (KIND == 8) {          // LOP3 / IMAD alternating, three fresh operands each
+          if (q & 1) asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(r[q]) : "r"(r[(q + 3) & 7]), "r"(r[(q + 5) & 7]));
+          else asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(r[q]) : "r"(r[(q + 3) & 7]), "r"(r[(q + 5) & 7]));
+        }
+        if (KIND == 9) {          // the mix of the DP column: 7 LOP3 (three fresh operands) : 4 multiply-adds (two fresh)
+          if ((u * 8 + q) % 11 < 7) asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(r[q]) : "r"(r[(q + 3) & 7]), "r"(r[(q + 5) & 7]));
+          else asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(r[q]) : "r"(r[(q + 3) & 7]), "r"(k2));
+        }
       }
     }
   }
@@ -41,7 +51,7 @@ int_peak_kernel(int iters, uint32_t seed, uint32_t* __restrict__ sink) {
 }  // namespace
 
 extern "C" int sq_int_peak(sq_ctx* c, int kind, int iters, double* ops_per_s) {
-  if (!c || !ops_per_s || iters < 1 || kind < 0 || kind > 7) return SQ_ERR_INVALID_ARG;
+  if (!c || !ops_per_s || iters < 1 || kind < 0 || kind > 9) return SQ_ERR_INVALID_ARG;
   if (!c->ws) return SQ_ERR_WORKSPACE;
   SqDeviceGuard guard(c);
   // 256 words of the free scratch (handed back at once: the kernels practically never write them)
@@ -64,7 +74,9 @@ extern "C" int sq_int_peak(sq_ctx* c, int kind, int iters, double* ops_per_s) {
       case 4: int_peak_kernel<4><<<blocks, 256, 0, c->stream>>>(iters, 12345u + rep, sink); break;
       case 5: int_peak_kernel<5><<<blocks, 256, 0, c->stream>>>(iters, 12345u + rep, sink); break;
       case 6: int_peak_kernel<6><<<blocks, 256, 0, c->stream>>>(iters, 12345u + rep, sink); break;
-      default: int_peak_kernel<7><<<blocks, 256, 0, c->stream>>>(iters, 12345u + rep, sink); break;
+      case 7: int_peak_kernel<7><<<blocks, 256, 0, c->stream>>>(iters, 12345u + rep, sink); break;
+      case 8: int_peak_kernel<8><<<blocks, 256, 0, c->stream>>>(iters, 12345u + rep, sink); break;
+      default: int_peak_kernel<9><<<blocks, 256, 0, c->stream>>>(iters, 12345u + rep, sink); break;
     }
     c->launches++;
     cudaEventRecord(e1, c->stream);

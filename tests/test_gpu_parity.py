@@ -730,3 +730,24 @@ def test_all_pairs_long_thresholded_band(L_lo, L_hi, max_edits, max_d):
     assert np.array_equal(_u32(pairs)[:cnt], want_p)
     assert np.array_equal(_u16(dist)[:cnt], want_d)
     sq.close()
+
+
+def test_roofline_probes_are_consistent():
+    """The denominators bench.py quotes: the column chain alone cannot beat the plain LOP3 stream, and
+    two pipes fed with fresh register operands stay below the sum of the pipes' own peaks."""
+    binding, sq = _ctx()
+    sq.set_workspace(1 << 20)
+    lop3 = sq.int_peak(0, 1024)
+    imad = sq.int_peak(3, 1024)
+    both_fresh = sq.int_peak(8, 1024)
+    mix = sq.int_peak(9, 1024)
+    chain = sq.dp_chain_peak(20, 500) * 7
+    assert lop3 > 1e12 and imad > 1e12
+    assert lop3 * 0.9 < both_fresh < (lop3 + imad) * 1.02
+    assert lop3 * 0.9 < mix < (lop3 + imad) * 1.02
+    assert 0.3 * lop3 < chain < 1.02 * lop3
+    with pytest.raises(binding.SubQuadError):
+        sq.dp_chain_peak(0, 10)
+    with pytest.raises(binding.SubQuadError):
+        sq.dp_chain_peak(32, 10)
+    sq.close()
