@@ -304,6 +304,11 @@ int  sq_pipeline_host_csr(sq_ctx* ctx, const uint8_t* seqs_host, const int64_t* 
  * packed sequences exceed this many bytes (they then do not fit the L2); 0 = always, so tests can
  * force that path on small inputs.  The schedule only permutes the order of the work. */
 #define SQ_OPT_SCHED_MIN_BYTES 2
+/* SQ_OPT_SCHED_BY_LABEL (0 / 1, default 1): order of the rows in that schedule.  1: by a family label
+ * (the smallest sequence index among the row and the heads of all buckets it shares), so that the rows
+ * of one clonal family are neighbours and their partners' texts stay in L2; 0: band 0's bucket order.
+ * A performance hint like the schedule itself: outputs do not depend on it. */
+#define SQ_OPT_SCHED_BY_LABEL 3
 int  sq_set_option(sq_ctx* ctx, int option, int64_t value);
 
 /* Introspection (host values, valid after the call they describe). */

@@ -23,7 +23,7 @@ SQ_HITS_STATIC_MAX_PAIRS = 1 << 27
 OP_PACK, OP_MINHASH, OP_LSH, OP_EDIT_DISTANCE, OP_ALL_PAIRS, OP_PIPELINE_HOST, OP_GRAPH, OP_JOIN = range(8)
 LSH_SORTED, LSH_UNORDERED = 0, 1
 JOIN_UPPER = 1
-OPT_SORT_KEY_BYTES, OPT_SCHED_MIN_BYTES = 1, 2
+OPT_SORT_KEY_BYTES, OPT_SCHED_MIN_BYTES, OPT_SCHED_BY_LABEL = 1, 2, 3
 
 EXPORTS = ["sq_create", "sq_destroy", "sq_workspace_bytes", "sq_set_workspace", "sq_pack",
            "sq_minhash", "sq_lsh_candidates", "sq_lsh_prepare", "sq_lsh_emit_range", "sq_candidates_stream_host", "sq_edit_distance", "sq_edit_distance_hits", "sq_edit_distance_hits_static", "sq_edit_distance_weighted", "sq_affinity_graph", "sq_all_pairs",

@@ -152,6 +152,7 @@ int sq_set_option(sq_ctx* c, int option, int64_t value) {
   if (!c) return SQ_ERR_INVALID_ARG;
   if (option == SQ_OPT_SORT_KEY_BYTES && value >= 1 && value <= 8) { c->sort_key_bytes = (int)value; return SQ_OK; }
   if (option == SQ_OPT_SCHED_MIN_BYTES && value >= 0) { c->sched_min_bytes = value; return SQ_OK; }
+  if (option == SQ_OPT_SCHED_BY_LABEL && (value == 0 || value == 1)) { c->sched_by_label = (int)value; return SQ_OK; }
   return SQ_ERR_INVALID_ARG;
 }
 

@@ -62,6 +62,7 @@ struct sq_ctx {
   // tuning (sq_set_option)
   int sort_key_bytes = 4;       // top bytes of the band key the bucket sort orders by (1..8)
   int64_t sched_min_bytes = (int64_t)96 << 20;   // packed bytes above which the DP follows the schedule
+  int sched_by_label = 1;       // schedule rows in family-label order (0: internal row order)
   // bookkeeping
   int64_t launches = 0;
   int64_t last_raw_pairs = 0;

@@ -1143,6 +1143,76 @@ active_units_kernel(const uint2* __restrict__ units, uint32_t nunits, const uint
   if (on) active[base + __popc(m & ((1u << lane) - 1u))] = u;
 }
 
+// ---------------------------------------------------------------------------------------------
+// the schedule of the DP stage in FAMILY-LABEL order
+// ---------------------------------------------------------------------------------------------
+// The internal row order (band 0's bucket order) keeps the members of one band-0 bucket together, but a
+// clonal family is many band-0 buckets -- a member with two or three edits usually sits in a bucket of
+// its own -- scattered over the order by their hash keys, while its partners are spread over the whole
+// family: the text gathers of such rows miss L2.  So the schedule visits the rows in the order of a
+// LABEL: the smallest external id among the row itself and the heads of all buckets it shares (a
+// bucket's ids ascend, so its head is its smallest member) -- one round of min-id propagation over the
+// buckets.  Almost every member of a family shares some bucket with the family's exact copies of the
+// seed, so a family gets one label and its rows become neighbours in the schedule.  Only the schedule
+// (a permutation of pair indices) changes; outputs do not.  Config 4: DRAM reads of the DP kernel
+// 54.7 -> ~20 GB, DP 27.3 -> 25.2 ms for ~1.0 ms of extra kernels (label: 16 gathers per row; a 3-pass
+// sort of 10 M (label, row) records; sizes, scan, schedule entries), step -1.1 ms.
+__global__ void __launch_bounds__(256)
+sched_label_kernel(const uint32_t* __restrict__ S, int SW, int bands, const uint32_t* __restrict__ vin,
+                   int64_t n2, uint64_t* __restrict__ keys, uint32_t* __restrict__ rows) {
+  const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= n2) return;
+  uint32_t label = vin[r];                           // band 0: record r is internal row r
+  for (int b0 = 0; b0 < bands; b0 += 4) {
+    const uint4 v = *reinterpret_cast<const uint4*>(S + r * SW + b0);
+    const uint32_t vv[4] = {v.x, v.y, v.z, v.w};
+    uint32_t hid[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q)                      // (a sentinel: the row shares no bucket in that band)
+      hid[q] = (b0 + q < bands && !(vv[q] & 0x80000000u)) ? vin[(int64_t)(b0 + q) * n2 + vv[q]] : 0xFFFFFFFFu;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) label = min(label, hid[q]);
+  }
+  keys[r] = label;
+  rows[r] = (uint32_t)r;
+}
+
+// sizes of the rows in schedule order (rowstart = exclusive scan of the sizes in internal order)
+__global__ void __launch_bounds__(256)
+sched_sizes_kernel(const uint32_t* __restrict__ order, const uint32_t* __restrict__ rowstart, int64_t n2,
+                   uint32_t* __restrict__ sizes) {
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k > n2) return;
+  uint32_t v = 0;
+  if (k < n2) { const uint32_t r = order[k]; v = rowstart[r + 1] - rowstart[r]; }
+  sizes[k] = v;
+}
+
+// delta2[k] and the chunk entries of schedule position k (= internal row order[k]); a warp takes 32
+// positions and writes the chunk entries of each of them together
+__global__ void __launch_bounds__(256)
+sched_write_kernel(const uint32_t* __restrict__ order, const uint32_t* __restrict__ start2, int64_t n2,
+                   const uint32_t* __restrict__ ids0, const uint32_t* __restrict__ ext_off,
+                   uint32_t* __restrict__ delta2, uint4* __restrict__ sched) {
+  const int lane = threadIdx.x & 31;
+  const int64_t k = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x);
+  uint32_t b = 0, e = 0, d = 0;
+  if (k < n2) {
+    b = start2[k]; e = start2[k + 1];
+    d = ext_off[ids0[order[k]]] - b;
+    delta2[k] = d;
+  }
+  // rows that hold the first position of at least one chunk
+  uint32_t m = __ballot_sync(kFull, k < n2 && (((uint64_t)b + 31) / 32) * 32 < (uint64_t)e);
+  while (m) {
+    const int l = __ffs(m) - 1;
+    m &= m - 1;
+    const uint32_t bb = __shfl_sync(kFull, b, l), ee = __shfl_sync(kFull, e, l), dd = __shfl_sync(kFull, d, l);
+    const uint32_t kk = (uint32_t)(k - lane + l);
+    for (uint64_t c = ((uint64_t)bb + 31) / 32 + lane; c * 32 < ee; c += 32) sched[c] = make_uint4(kk, dd, ee, bb);
+  }
+}
+
 inline int chunks_for(int bands) { return bands <= 4 ? 1 : bands <= 8 ? 2 : bands <= 16 ? 4 : 8; }
 
 }  // namespace
@@ -1164,6 +1234,7 @@ size_t sq_lsh_scratch_bytes(int64_t n, int bands, int64_t pair_capacity) {
   s += sq_align_up(rec * 32 + 16);             // mask cache of the count pass (used if it fits)
   s += sq_align_up(((size_t)(pair_capacity > 0 ? pair_capacity : 0) / 32 + 2) * 16 + 16) +
        2 * sq_align_up((nn + 2) * 4 + 16);     // chunk schedule of the edit-distance stage
+  s += 2 * sq_align_up((nn + 2) * 8 + 16) + 3 * sq_align_up((nn + 2) * 4 + 16);   // its family-label order
   return s + 4096;
 }
 
@@ -1393,13 +1464,46 @@ extern "C" int sq_lsh_emit_range(sq_ctx* c, int64_t row_lo, int64_t row_hi, int 
     uint4* sched = sq_scratch<uint4>(c, nchunks);
     uint32_t* delta = sq_scratch<uint32_t>(c, (size_t)n2 + 1);
     if (!sched || !delta) { sched = nullptr; delta = nullptr; }
+    // the schedule in family-label order (optional: without room for its arrays the row kernel writes the
+    // schedule in internal row order on its way)
+    const uint32_t* sched_start = rowstart;
+    bool by_label = false;
+    if (sched && c->sched_by_label && n2 < (1ll << 30)) {
+      const size_t top = c->scratch_top;
+      uint64_t* lk0 = sq_scratch<uint64_t>(c, (size_t)n2 + 2);
+      uint64_t* lk1 = sq_scratch<uint64_t>(c, (size_t)n2 + 2);
+      uint32_t* lv0 = sq_scratch<uint32_t>(c, (size_t)n2 + 2);
+      uint32_t* lv1 = sq_scratch<uint32_t>(c, (size_t)n2 + 2);
+      uint32_t* start2 = sq_scratch<uint32_t>(c, (size_t)n2 + 2);
+      if (lk0 && lk1 && lv0 && lv1 && start2) {
+        const unsigned gr = (unsigned)((n2 + 256) / 256);
+        SQ_TIMED(c, SQ_K_SEGMENT, sched_label_kernel<<<gr, 256, 0, st>>>(L.S, 4 * bw, bands, L.vin, n2, lk0, lv0));
+        SQ_LAUNCH_CHECK(c);
+        int nb = 1;
+        while (nb < 4 && (1ll << (8 * nb)) < n) ++nb;              // key bytes that hold the label (an external id)
+        int in_alt = 0;
+        rc = sq_onesweep_sort(c, lk0, lk1, lv0, lv1, n2, 1, 0, nb, L.tmp, &in_alt);
+        if (rc != SQ_OK) return rc;
+        const uint32_t* order = in_alt ? lv1 : lv0;
+        SQ_TIMED(c, SQ_K_SEGMENT, sched_sizes_kernel<<<gr, 256, 0, st>>>(order, rowstart, n2, start2));
+        SQ_LAUNCH_CHECK(c);
+        rc = sq_exclusive_scan_u32(c, start2, start2, n2 + 1, tmp32, nullptr);
+        if (rc != SQ_OK) return rc;
+        SQ_TIMED(c, SQ_K_SEGMENT, sched_write_kernel<<<gr, 256, 0, st>>>(order, start2, n2, L.vin, ext_off, delta, sched));
+        SQ_LAUNCH_CHECK(c);
+        sched_start = start2;
+        by_label = true;
+      } else {
+        c->scratch_top = top;
+      }
+    }
     SQ_TIMED(c, SQ_K_ROWSORT, row_sort_kernel<<<g, kRsWarps * 32, 0, st>>>(
         cnt, loc, n2, bands, L.vin, ext_off, flags == SQ_LSH_SORTED, tmpJ, reinterpret_cast<uint2*>(pairs_out),
-        counters + 6, rowstart, delta, sched, lo, hi));
+        counters + 6, rowstart, by_label ? nullptr : delta, by_label ? nullptr : sched, lo, hi));
     SQ_LAUNCH_CHECK(c);
     if (sched) {
       c->sched = sched;
-      c->sched_rowstart = rowstart;
+      c->sched_rowstart = sched_start;
       c->sched_delta = delta;
       c->sched_chunks = (int64_t)nchunks;
       c->sched_pairs = pairs_out;

@@ -476,12 +476,14 @@ def test_weighted_table_diagonal_is_never_used():
 # ---------------------------------------------------------------------------------------------
 # the family-ordered schedule of the DP stages, forced on small inputs (SQ_OPT_SCHED_MIN_BYTES = 0)
 # ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("by_label", [1, 0])
 @pytest.mark.parametrize("cfg,n,flags", [("config2", 30_011, 0), ("config2", 30_011, 1), ("config4", 60_013, 0),
                                          ("config3", 40_009, 0)])
-def test_schedule_forced_edit_weighted_graph(cfg, n, flags):
+def test_schedule_forced_edit_weighted_graph(cfg, n, flags, by_label):
     """With the schedule forced, sq_edit_distance / sq_edit_distance_weighted / sq_affinity_graph walk
-    the pairs in the internal family order (chunk schedule, rows of every size, empty rows, chunks that
-    cross rows): every distance and the whole graph still equal the oracle, bit for bit."""
+    the pairs in the schedule's order -- rows by family label (SQ_OPT_SCHED_BY_LABEL = 1, the default)
+    or in band 0's bucket order (0); chunk schedule, rows of every size, empty rows, chunks that cross
+    rows: every distance and the whole graph still equal the oracle, bit for bit."""
     binding, sq = _ctx()
     P = dict(dg.PARAMS[cfg])
     rep = dg.GENERATORS[cfg](n, seed=31)
@@ -491,6 +493,7 @@ def test_schedule_forced_edit_weighted_graph(cfg, n, flags):
              sq.workspace_bytes(binding.OP_GRAPH, rep.n, 0, max_len, 0, 0, 0, cap)) + 4 * cap + 8 * n
     sq.set_workspace(ws)
     sq.set_option(binding.OPT_SCHED_MIN_BYTES, 0)
+    sq.set_option(binding.OPT_SCHED_BY_LABEL, by_label)
     sq.pack(torch.from_numpy(rep.seqs).cuda(), torch.from_numpy(rep.offsets).cuda(), 20, max_len)
     sig = sq.minhash(P["k"], P["H"], SEED)
     pairs = torch.empty((cap, 2), dtype=torch.int32, device="cuda")
