@@ -1466,9 +1466,13 @@ extern "C" int sq_lsh_emit_range(sq_ctx* c, int64_t row_lo, int64_t row_hi, int 
     if (!sched || !delta) { sched = nullptr; delta = nullptr; }
     // the schedule in family-label order (optional: without room for its arrays the row kernel writes the
     // schedule in internal row order on its way)
+    // -- when the DP stages will follow the schedule: the packed sequences exceed sched_min_bytes (smaller
+    // inputs sit in L2 anyway; the graph step, whose criterion is the size of the signatures, then walks
+    // the internal row order the row kernel writes on its way)
     const uint32_t* sched_start = rowstart;
     bool by_label = false;
-    if (sched && c->sched_by_label && n2 < (1ll << 30)) {
+    const bool sched_used = (size_t)c->n * (size_t)c->stride > (size_t)c->sched_min_bytes;
+    if (sched && c->sched_by_label && sched_used && n2 < (1ll << 30)) {
       const size_t top = c->scratch_top;
       uint64_t* lk0 = sq_scratch<uint64_t>(c, (size_t)n2 + 2);
       uint64_t* lk1 = sq_scratch<uint64_t>(c, (size_t)n2 + 2);
