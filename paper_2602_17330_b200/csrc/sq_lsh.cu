@@ -1472,7 +1472,9 @@ extern "C" int sq_lsh_emit_range(sq_ctx* c, int64_t row_lo, int64_t row_hi, int 
     const uint32_t* sched_start = rowstart;
     bool by_label = false;
     const bool sched_used = (size_t)c->n * (size_t)c->stride > (size_t)c->sched_min_bytes;
-    if (sched && c->sched_by_label && sched_used && n2 < (1ll << 30)) {
+    // (and only for the whole repertoire: the label kernels walk all rows, a call for a slice of the rows --
+    // the streamed / sharded entry points make many -- keeps the schedule the row kernel writes for free)
+    if (sched && c->sched_by_label && sched_used && whole && n2 < (1ll << 30)) {
       const size_t top = c->scratch_top;
       uint64_t* lk0 = sq_scratch<uint64_t>(c, (size_t)n2 + 2);
       uint64_t* lk1 = sq_scratch<uint64_t>(c, (size_t)n2 + 2);
