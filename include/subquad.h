@@ -215,7 +215,8 @@ int  sq_edit_distance_weighted(sq_ctx* ctx, const uint32_t* pairs, int64_t n_pai
  * PAPER.md L71-73 Eq. 1, L185 Alg. 1 step 12; Jaccard estimate from the sketches L495-497 Eq. 30,
  * thresholded at tau = 0.7 in L269 / L638).  Edge (i, j), i < j, is kept iff dist[p] <= max_d AND
  * the signatures of i and j agree in at least `min_matches` of the H columns (the caller passes
- * min_matches = ceil(tau * H); 0 = no sketch filter, sig may then be NULL).
+ * min_matches = ceil(tau * H); 0 = no sketch filter, sig may then be NULL; else sig = uint32[n][H],
+ * H a multiple of 32, 16-byte aligned: SQ_ERR_INVALID_ARG otherwise).
  * weight = 1 - d / max(len_i, len_j) in fp32 (1 for two empty sequences).
  * pairs/dist: as produced by sq_lsh_candidates + sq_edit_distance (first index non-decreasing).
  * Output, device: row_ptr int64[n+1], col uint32[capacity] (ascending inside a row when the pairs

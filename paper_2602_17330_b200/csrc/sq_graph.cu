@@ -16,16 +16,16 @@
 
 namespace {
 
-// one pair, whole warp
-__device__ __forceinline__ void graph_keep_one(const uint2* __restrict__ pairs,
-                                               const uint16_t* __restrict__ dist, int64_t p, int max_d,
-                                               const uint32_t* __restrict__ sig, int H, int min_matches,
-                                               int64_t n, uint32_t* __restrict__ keep,
-                                               uint32_t* __restrict__ row_cnt, int lane);
-
-// SCHED: warp k walks positions [32k, 32k+32) of the family-ordered schedule left by
-// sq_lsh_candidates (sq_common.cuh) -- the signature rows of one family stay in L2.
-template <bool SCHED>
+// A warp takes 32 pairs (positions [32k, 32k+32) of the family-ordered schedule left by sq_lsh_candidates
+// when SCHED -- the signature rows of one family stay in L2 -- else pairs [32k, 32k+32)) and works on
+// FOUR pairs at a time, eight lanes per pair: lane l8 of a group compares columns [l8 * H/8, +H/8) of the
+// two signature rows, read by 16-byte loads (a row of H = 64 columns is two loads per lane, the eight
+// lanes of a group cover 128 contiguous bytes per load); the equal columns are summed over the group
+// with three shuffles.  Row i's share of the signature stays in registers while i does not change (the
+// pairs arrive grouped by i).  Round 1 gave a whole warp to every pair (two 4-byte loads and a ballot
+// per 32 columns: ~45 warp instructions per pair); this needs ~12.
+// CPL4 = 16-byte pieces per lane = H / 32.
+template <bool SCHED, int CPL4>
 __global__ void __launch_bounds__(256)
 graph_keep_kernel(const uint2* __restrict__ pairs, const uint16_t* __restrict__ dist, int64_t n_pairs,
                   int max_d, const uint32_t* __restrict__ sig, int H, int min_matches, int64_t n,
@@ -34,14 +34,11 @@ graph_keep_kernel(const uint2* __restrict__ pairs, const uint16_t* __restrict__ 
                   const uint32_t* __restrict__ delta) {
   const int lane = threadIdx.x & 31;
   const int64_t wk = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  if (!SCHED) {
-    if (wk < n_pairs) graph_keep_one(pairs, dist, wk, max_d, sig, H, min_matches, n, keep, row_cnt, lane);
-    return;
-  }
   const int64_t q0 = wk * 32;
   if (q0 >= n_pairs) return;
-  int64_t p = q0 + lane;                              // lane t decodes position q0 + t
-  if (p < n_pairs) {
+  int64_t p = q0 + lane;                              // lane t owns position q0 + t
+  const bool valid = p < n_pairs;
+  if (SCHED && valid) {
     const uint4 ch = sched[wk];
     const uint32_t q = (uint32_t)p;
     if (q < ch.z) p = (int64_t)(uint32_t)(ch.y + q);
@@ -51,32 +48,51 @@ graph_keep_kernel(const uint2* __restrict__ pairs, const uint16_t* __restrict__ 
       p = (int64_t)(uint32_t)(delta[r] + q);
     }
   }
-  const int cntp = (int)min((int64_t)32, n_pairs - q0);
-  for (int t = 0; t < cntp; ++t) {
-    const int64_t pt = __shfl_sync(0xFFFFFFFFu, p, t);
-    graph_keep_one(pairs, dist, pt, max_d, sig, H, min_matches, n, keep, row_cnt, lane);
+  uint2 pr = make_uint2(0xFFFFFFFFu, 0xFFFFFFFFu);
+  bool ok = false;
+  if (valid) {
+    pr = pairs[p];
+    ok = pr.x < (uint64_t)n && pr.y < (uint64_t)n && (int)dist[p] <= max_d;
   }
-}
-
-__device__ __forceinline__ void graph_keep_one(const uint2* __restrict__ pairs,
-                                               const uint16_t* __restrict__ dist, int64_t p, int max_d,
-                                               const uint32_t* __restrict__ sig, int H, int min_matches,
-                                               int64_t n, uint32_t* __restrict__ keep,
-                                               uint32_t* __restrict__ row_cnt, int lane) {
-  const uint2 pr = pairs[p];
-  bool ok = pr.x < (uint64_t)n && pr.y < (uint64_t)n && (int)dist[p] <= max_d;
-  if (ok && min_matches > 0) {
-    const uint32_t* a = sig + (int64_t)pr.x * H;
-    const uint32_t* b = sig + (int64_t)pr.y * H;
-    int m = 0;
-    for (int c = lane; c < H; c += 32) m += __popc(__ballot_sync(0xFFFFFFFFu, a[c] == b[c]));
-    // (H is a multiple of 32, so every lane runs the same trips and every ballot is full)
-    ok = m >= min_matches;
+  if (min_matches > 0) {
+    const int sub = lane >> 3, l8 = lane & 7;
+    uint4 ra[CPL4];
+    uint32_t cur_i = 0xFFFFFFFFu;
+    int mine = 0;                                     // equal columns of this lane's own pair
+#pragma unroll 1
+    for (int g = 0; g < 8; ++g) {
+      const int t = 4 * g + sub;                      // the pair this group of eight lanes works on
+      const uint32_t it = __shfl_sync(0xFFFFFFFFu, pr.x, t), jt = __shfl_sync(0xFFFFFFFFu, pr.y, t);
+      const bool okt = __shfl_sync(0xFFFFFFFFu, ok ? 1 : 0, t) != 0;
+      int m = 0;
+      if (okt) {
+        if (it != cur_i) {
+          const uint4* a = reinterpret_cast<const uint4*>(sig + (int64_t)it * H) + l8 * CPL4;
+#pragma unroll
+          for (int q = 0; q < CPL4; ++q) ra[q] = a[q];
+          cur_i = it;
+        }
+        const uint4* b = reinterpret_cast<const uint4*>(sig + (int64_t)jt * H) + l8 * CPL4;
+#pragma unroll
+        for (int q = 0; q < CPL4; ++q) {
+          const uint4 v = b[q];
+          m += (v.x == ra[q].x) + (v.y == ra[q].y) + (v.z == ra[q].z) + (v.w == ra[q].w);
+        }
+      }
+      m += __shfl_xor_sync(0xFFFFFFFFu, m, 1);
+      m += __shfl_xor_sync(0xFFFFFFFFu, m, 2);
+      m += __shfl_xor_sync(0xFFFFFFFFu, m, 4);
+      // pair t's count sits in group t & 3; its owner is lane t
+      const int got = __shfl_sync(0xFFFFFFFFu, m, (lane & 3) * 8);
+      if ((lane >> 2) == g) mine = got;
+    }
+    ok = ok && mine >= min_matches;
   }
-  if (lane == 0) {
-    keep[p] = ok ? 1u : 0u;
-    if (ok) atomicAdd(&row_cnt[pr.x], 1u);
-  }
+  if (valid) keep[p] = ok ? 1u : 0u;
+  // kept pairs per row: one atomic per run of equal i inside the warp
+  const uint32_t key = ok ? pr.x : 0xFFFFFFFFu;
+  const uint32_t peers = __match_any_sync(0xFFFFFFFFu, key);
+  if (ok && lane == __ffs(peers) - 1) atomicAdd(&row_cnt[pr.x], (uint32_t)__popc(peers));
 }
 
 __global__ void __launch_bounds__(256)
@@ -119,7 +135,8 @@ extern "C" int sq_affinity_graph(sq_ctx* c, const uint32_t* pairs, const uint16_
   *n_edges = 0;
   if (c->n < 0) return SQ_ERR_NOT_PACKED;
   if (n_pairs < 0 || capacity < 0 || max_d < 0 || min_matches < 0) return SQ_ERR_INVALID_ARG;
-  if (min_matches > 0 && (!sig || H < 32 || (H % 32) != 0 || H > SQ_MAX_H || min_matches > H))
+  if (min_matches > 0 && (!sig || H < 32 || (H % 32) != 0 || H > SQ_MAX_H || min_matches > H ||
+                          (reinterpret_cast<uintptr_t>(sig) & 15) != 0))      // rows are read by 16-byte loads
     return SQ_ERR_INVALID_ARG;
   if (n_pairs >= (1ll << 32) - 1) return SQ_ERR_UNSUPPORTED;
   const int64_t n = c->n;
@@ -146,18 +163,27 @@ extern "C" int sq_affinity_graph(sq_ctx* c, const uint32_t* pairs, const uint16_
   SQ_CUDA(c, cudaMemsetAsync(c->dflags, 0, 64, st));
   if (n_pairs > 0) {
     if (!pairs || !dist) return SQ_ERR_INVALID_ARG;
-    if (use_sched) {
-      const int64_t blocks = ((n_pairs + 31) / 32 * 32 + 255) / 256;
-      SQ_TIMED(c, SQ_K_MISC, graph_keep_kernel<true><<<(unsigned)blocks, 256, 0, st>>>(
-          reinterpret_cast<const uint2*>(pairs), dist, n_pairs, max_d, sig, H, min_matches, n, keep, row_cnt,
-          sched, srow, sdel));
-    } else {
-      const int64_t blocks = (n_pairs * 32 + 255) / 256;
-      if (blocks >= (1ll << 31)) return SQ_ERR_UNSUPPORTED;
-      SQ_TIMED(c, SQ_K_MISC, graph_keep_kernel<false><<<(unsigned)blocks, 256, 0, st>>>(
-          reinterpret_cast<const uint2*>(pairs), dist, n_pairs, max_d, sig, H, min_matches, n, keep, row_cnt,
-          nullptr, nullptr, nullptr));
+    const int64_t blocks = ((n_pairs + 31) / 32 * 32 + 255) / 256;       // a warp per 32 pairs
+    if (blocks >= (1ll << 31)) return SQ_ERR_UNSUPPORTED;
+    const uint2* pp = reinterpret_cast<const uint2*>(pairs);
+#define SQ_GRAPH_LAUNCH(SCHED_, C4_)                                                                       \
+    SQ_TIMED(c, SQ_K_MISC, (graph_keep_kernel<SCHED_, C4_><<<(unsigned)blocks, 256, 0, st>>>(               \
+        pp, dist, n_pairs, max_d, sig, H, min_matches, n, keep, row_cnt, use_sched ? sched : nullptr,        \
+        use_sched ? srow : nullptr, use_sched ? sdel : nullptr)))
+#define SQ_GRAPH_DISPATCH(SCHED_)                                                                          \
+    switch (min_matches > 0 ? H / 32 : 1) {                                                                \
+      case 1: SQ_GRAPH_LAUNCH(SCHED_, 1); break;                                                           \
+      case 2: SQ_GRAPH_LAUNCH(SCHED_, 2); break;                                                           \
+      case 3: SQ_GRAPH_LAUNCH(SCHED_, 3); break;                                                           \
+      case 4: SQ_GRAPH_LAUNCH(SCHED_, 4); break;                                                           \
+      case 5: SQ_GRAPH_LAUNCH(SCHED_, 5); break;                                                           \
+      case 6: SQ_GRAPH_LAUNCH(SCHED_, 6); break;                                                           \
+      case 7: SQ_GRAPH_LAUNCH(SCHED_, 7); break;                                                           \
+      default: SQ_GRAPH_LAUNCH(SCHED_, 8); break;                                                          \
     }
+    if (use_sched) { SQ_GRAPH_DISPATCH(true) } else { SQ_GRAPH_DISPATCH(false) }
+#undef SQ_GRAPH_DISPATCH
+#undef SQ_GRAPH_LAUNCH
     SQ_LAUNCH_CHECK(c);
     int rc = sq_exclusive_scan_u32(c, keep, keep, n_pairs + 1, tmp, c->dflags);
     if (rc != SQ_OK) return rc;
