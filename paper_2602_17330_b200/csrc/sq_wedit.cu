@@ -11,7 +11,7 @@
 // prof[c][x] = cost(a_x, c), one byte per pattern position, 32 bytes per residue c -- and a DP
 // column step is: two 16-byte loads of the text residue's profile row, then per pattern row one
 // byte extract and  new = min(up + indel, min(diag + cost, old + indel))  on a register-resident
-// column (rows padded to a multiple of 8, picked per run).
+// column (rows padded to a multiple of 4, picked per run).
 // Longer sequences: one thread per pair, the DP column in shared memory [row][thread].
 #include "sq_common.cuh"
 
@@ -30,10 +30,11 @@ __device__ __forceinline__ void we_column(int (&D)[32], const uint32_t* __restri
     const uint4 v = *reinterpret_cast<const uint4*>(prow + 4 * q);
     cw[4 * q] = v.x; cw[4 * q + 1] = v.y; cw[4 * q + 2] = v.z; cw[4 * q + 3] = v.w;
   }
-  if (MR % 16) {                          // MR = 8 or 24: one more 8-byte piece
+  if (MR % 16 >= 8) {                     // one more 8-byte piece
     const uint2 v = *reinterpret_cast<const uint2*>(prow + (MR / 16) * 4);
     cw[(MR / 16) * 4] = v.x; cw[(MR / 16) * 4 + 1] = v.y;
   }
+  if (MR % 8 >= 4) cw[MR / 4 - 1] = prow[MR / 4 - 1];   // and / or a 4-byte one (MR is a multiple of 4)
   int diag = y * indel;                   // D(0, y)
   int up = diag + indel;                  // D(0, y+1)
 #pragma unroll
@@ -136,9 +137,13 @@ wedit_short_kernel(const uint8_t* __restrict__ packed, int64_t n, const uint2* _
     if (max_d >= 0 && diff * indel > max_d) d = max_d + 1;
     else if (m == 0) d = nlen * indel;
     else if (nlen == 0) d = m * indel;
+    // (the pattern rows of a run are padded to a multiple of 4: the column step is MR unrolled cells)
     else if (m <= 8) d = we_dp<8>(pq, m, text, nlen, indel);
+    else if (m <= 12) d = we_dp<12>(pq, m, text, nlen, indel);
     else if (m <= 16) d = we_dp<16>(pq, m, text, nlen, indel);
+    else if (m <= 20) d = we_dp<20>(pq, m, text, nlen, indel);
     else if (m <= 24) d = we_dp<24>(pq, m, text, nlen, indel);
+    else if (m <= 28) d = we_dp<28>(pq, m, text, nlen, indel);
     else d = we_dp<32>(pq, m, text, nlen, indel);
   }
   if (!valid) return;
