@@ -97,17 +97,25 @@ graph_keep_kernel(const uint2* __restrict__ pairs, const uint16_t* __restrict__ 
 
 __global__ void __launch_bounds__(256)
 graph_edge_kernel(const uint2* __restrict__ pairs, const uint16_t* __restrict__ dist, int64_t n_pairs,
-                  const uint32_t* __restrict__ slot, const uint8_t* __restrict__ packed, int stride,
+                  const uint32_t* __restrict__ slot, const uint8_t* __restrict__ len8,
                   uint32_t* __restrict__ col, float* __restrict__ weight) {
   const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= n_pairs) return;
   const uint32_t s = slot[p];
   if (slot[p + 1] == s) return;                 // not kept (the scan covers n_pairs + 1 entries)
   const uint2 pr = pairs[p];
-  const int la = packed[(int64_t)pr.x * stride + stride - 1], lb = packed[(int64_t)pr.y * stride + stride - 1];
+  const int la = len8[pr.x], lb = len8[pr.y];      // (one byte per sequence: the table stays in L2)
   const int L = la > lb ? la : lb;
   col[s] = pr.y;
   weight[s] = L > 0 ? 1.0f - (float)dist[p] / (float)L : 1.0f;
+}
+
+// the lengths of all sequences as one byte each (the slots' length bytes are a stride apart: 32 bytes of
+// DRAM traffic per lookup, two lookups per edge)
+__global__ void __launch_bounds__(256)
+graph_len_kernel(const uint8_t* __restrict__ packed, int stride, int64_t n, uint8_t* __restrict__ len8) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) len8[i] = packed[i * stride + stride - 1];
 }
 
 __global__ void __launch_bounds__(256)
@@ -200,8 +208,12 @@ extern "C" int sq_affinity_graph(sq_ctx* c, const uint32_t* pairs, const uint16_
   if (edges > capacity) { SQ_CUDA(c, cudaStreamSynchronize(st)); return SQ_ERR_CAPACITY; }
   if (edges > 0) {
     if (!col || !weight) return SQ_ERR_INVALID_ARG;
+    // (row_cnt has been copied into row_ptr: its buffer takes the byte-per-sequence length table)
+    uint8_t* len8 = reinterpret_cast<uint8_t*>(row_cnt);
+    SQ_TIMED(c, SQ_K_MISC, graph_len_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(c->packed, c->stride, n, len8));
+    SQ_LAUNCH_CHECK(c);
     SQ_TIMED(c, SQ_K_MISC, graph_edge_kernel<<<(unsigned)((n_pairs + 255) / 256), 256, 0, st>>>(
-        reinterpret_cast<const uint2*>(pairs), dist, n_pairs, keep, c->packed, c->stride, col, weight));
+        reinterpret_cast<const uint2*>(pairs), dist, n_pairs, keep, len8, col, weight));
     SQ_LAUNCH_CHECK(c);
   }
   SQ_CUDA(c, cudaStreamSynchronize(st));
